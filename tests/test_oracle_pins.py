@@ -1,0 +1,462 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix (no GPU).
+
+Pin ids follow SURVEY.md §8(c) / DESIGN.md.  None of these compares the oracle with
+itself: expected values are the paper's (tests/golden), closed forms, invariants,
+lattice constants computed outside oracle/, or brute force.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+from oracle import orc
+from paper_2110_02621_b200 import inputs
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _gold(name):
+    out = {}
+    for line in open(os.path.join(GOLD, name)):
+        line = line.split("#")[0].split()
+        if len(line) == 2:
+            out[line[0]] = float(line[1])
+    return out
+
+
+def custom(dim, pos, tag, rho, vel=None, dp=1.0 / 64, rho0=(1000.0,), c0=(10.0,), g=(0, 0, 0),
+           **kw):
+    """Hand-built configuration (arrays given directly; no generator)."""
+    pos = np.asarray(pos, np.float64)
+    if pos.shape[1] == 2:
+        pos = np.concatenate([pos, np.zeros((len(pos), 1))], 1)
+    lo = pos.min(0) - 4 * dp
+    hi = pos.max(0) + 4 * dp
+    cfg = dict(dim=dim, n_phases=len(rho0), dp=dp, h=1.3 * dp, rho0=list(rho0), c0=list(c0),
+               g=list(g), cfl=0.25, penalty_strength=1.0, penalty_phase_mask=0,
+               free_surface_mask=1, flags=orc.FLAG_REINIT | orc.FLAG_WALL_VEL_MIRROR,
+               domain_min=list(lo), domain_max=list(hi))
+    cfg.update(kw)
+    cfg["pos"] = pos.astype(np.float32)
+    cfg["vel"] = np.zeros_like(cfg["pos"]) if vel is None else np.asarray(vel, np.float32)
+    cfg["rho"] = np.asarray(rho, np.float32)
+    cfg["tag"] = np.asarray(tag, np.int32)
+    return cfg
+
+
+def run(cfg):
+    o = orc.Oracle(cfg)
+    o.set_particles(cfg["pos"], cfg["vel"], cfg["rho"], cfg["tag"])
+    return o
+
+
+def lattice(dim, n, dp):
+    ax = (np.arange(n) + 0.5) * dp
+    return np.stack([g.ravel() for g in np.meshgrid(*([ax] * dim), indexing="ij")], 1)
+
+
+# ------------------------------------------------------------------ P1 kernel
+@pytest.mark.parametrize("dim", [2, 3])
+def test_P1_kernel_unit_integral_and_derivative(dim):
+    h = 0.37
+    r = np.linspace(0, 2 * h, 200001)
+    w = np.array([orc.kernel_w(dim, h, x) for x in r[::100]])
+    rr = r[::100]
+    jac = 2 * math.pi * rr if dim == 2 else 4 * math.pi * rr ** 2
+    integral = np.trapezoid(w * jac, rr)
+    assert abs(integral - 1.0) < 1e-6
+    assert orc.kernel_w(dim, h, 2 * h) == 0.0 and orc.kernel_w(dim, h, 2.5 * h) == 0.0
+    assert orc.kernel_dw(dim, h, 0.0) == 0.0
+    for x in (0.1 * h, 0.7 * h, 1.3 * h, 1.9 * h):
+        e = 1e-6 * h
+        fd = (orc.kernel_w(dim, h, x + e) - orc.kernel_w(dim, h, x - e)) / (2 * e)
+        assert abs(fd - orc.kernel_dw(dim, h, x)) < 1e-6 * abs(orc.kernel_dw(dim, h, 0.7 * h))
+        assert orc.kernel_dw(dim, h, x) < 0
+
+
+# ------------------------------------------------------------------ P2 lattice constants
+def test_P2_lattice_constants_golden():
+    g = _gold("lattice_constants.txt")
+    assert abs(orc.sigma0(2, 1.3, 1.0) - g["sigma0_2d"]) < 2e-9
+    assert abs(orc.sigma0(3, 1.3, 1.0) - g["sigma0_3d"]) < 2e-9
+    assert abs(orc.kernel_w(2, 1.3, 0.0) - g["w0_2d"]) < 2e-9
+    assert abs(orc.kernel_w(3, 1.3, 0.0) - g["w0_3d"]) < 2e-9
+
+
+@pytest.mark.parametrize("dim,n", [(2, 9), (3, 9)])
+def test_P2_partition_of_unity_and_neighbour_count(dim, n):
+    g = _gold("lattice_constants.txt")
+    dp = 1.0 / 64
+    pos = lattice(dim, n, dp)
+    cfg = custom(dim, pos, np.zeros(len(pos)), np.full(len(pos), 1000.0), dp=dp)
+    o = run(cfg)
+    f = o.fields()
+    centre = np.argmin(np.linalg.norm(pos - pos.mean(0), axis=1))
+    key = "%dd" % dim
+    assert abs(f["sigma"][centre] * dp ** dim - g["sigma0_" + key]) < 2e-9
+    off, ids = o.neighbours()
+    assert off[centre + 1] - off[centre] == int(g["neigh_" + key])
+    # half-space sum: particle on the top face of the block sees own layer and below only
+    top = np.argmin(np.linalg.norm(pos - (pos.mean(0) + np.eye(dim)[dim - 1] * (n // 2) * dp), axis=1))
+    assert abs(f["sigma"][top] * dp ** dim - g["halfspace_" + key]) < 2e-9
+
+
+# ------------------------------------------------------------------ P3 momentum sum
+@pytest.mark.parametrize("dim", [2, 3])
+def test_P3_linear_pressure_gives_M1_gradient(dim):
+    """Eq. 2.10 on a full lattice with an (almost) uniform density and a linear p:
+    a = -M1 grad p / rho, M1 the first-moment lattice constant."""
+    g = _gold("lattice_constants.txt")
+    dp, n, c = 1.0 / 64, 9, 10.0
+    pos = lattice(dim, n, dp)
+    k = np.round(pos[:, 0] / dp - 0.5)
+    rho = 1000.0 + k * 2.0 ** -10            # exactly representable in float32
+    o = run(custom(dim, pos, np.zeros(len(pos)), rho, dp=dp, c0=(c,)))
+    f = o.fields()
+    centre = np.argmin(np.linalg.norm(pos - pos.mean(0), axis=1))
+    gradp = c * c * 2.0 ** -10 / dp
+    expect = -g["M1_%dd" % dim] * gradp / rho[centre]
+    assert abs(f["acc"][centre, 0] - expect) < 2e-5 * abs(expect)
+    assert np.all(np.abs(f["acc"][centre, 1:]) < 1e-9 * abs(expect))
+
+
+@pytest.mark.parametrize("dim", [2, 3])
+def test_P7_linear_velocity_gives_M1_divergence(dim):
+    """Eq. 2.9 with uniform p, rho reduces to Eq. 2.5: d rho/dt = -rho M1 div v."""
+    g = _gold("lattice_constants.txt")
+    dp, n, A = 1.0 / 64, 9, 0.5
+    pos = lattice(dim, n, dp)
+    vel = np.zeros((len(pos), 3))
+    vel[:, 0] = A * pos[:, 0]
+    vel[:, 1] = -0.25 * A * pos[:, 1]
+    o = run(custom(dim, pos, np.zeros(len(pos)), np.full(len(pos), 1000.0), vel=vel, dp=dp,
+                   flags=0))
+    o.step(1, dts=[1e-13])
+    f = o.fields()
+    centre = np.argmin(np.linalg.norm(pos - pos.mean(0), axis=1))
+    expect = -1000.0 * g["M1_%dd" % dim] * (A - 0.25 * A)
+    assert abs(f["drho"][centre] - expect) < 1e-6 * abs(expect)
+
+
+# ------------------------------------------------------------------ P4 wall extrapolation
+@pytest.mark.parametrize("multi", [False, True])
+def test_P4_wall_pressure_exact_for_linear_hydrostatic_field(multi):
+    dp, nx, K, c = 1.0 / 64, 12, 10, 10.0
+    fl = lattice(2, nx, dp)
+    fl = fl[fl[:, 1] < K * dp]
+    k = np.round(fl[:, 1] / dp - 0.5)
+    rho_f = 1000.0 + (K - k) * 2.0 ** -10
+    gmag = c * c * 2.0 ** -10 / (dp * 1000.0)
+    H = (K + 0.5) * dp
+    wl = np.array([[(i + 0.5) * dp, -(j + 0.5) * dp] for i in range(nx) for j in range(3)])
+    pos = np.concatenate([fl, wl])
+    tag = np.concatenate([np.zeros(len(fl)), -np.ones(len(wl))])
+    rho = np.concatenate([rho_f, np.full(len(wl), 1000.0)])
+    kw = dict(rho0=(1000.0, 1.0), c0=(c, c)) if multi else dict(c0=(c,))
+    o = run(custom(2, pos, tag, rho, dp=dp, g=(0, -gmag, 0), **kw))
+    f = o.fields()
+    pw = f["p"][len(fl):]
+    expect = 1000.0 * gmag * (H - wl[:, 1])
+    # rho_f is uniform to 1e-5, so Eq. 2.12 reproduces the linear field to that level
+    near = wl[:, 1] > -2.4 * dp                  # the third layer has no fluid neighbour
+    assert np.max(np.abs(pw - expect)[near]) < 3e-5 * expect.max()
+    assert np.all(pw[~near] == 0.0)              # reading A7
+    # dropping the lever term would miss by more than one lattice unit of pressure
+    assert 1000.0 * gmag * dp > 1e3 * 3e-5 * expect.max() / 40
+
+
+# ------------------------------------------------------------------ P5 / P17 whole step
+def test_P5_resting_column_relaxes_to_hydrostatic_and_P17_mass():
+    """BASELINE.json north_star: closed-form p = rho0 g (H - z) in a resting column
+    (PAPER.md:224).  The scheme is low-dissipation, so the column rings acoustically about
+    the hydrostatic state; the time average over the ringing is compared."""
+    cfg = inputs.dam_break_2d(dp=0.02, tank=(0.6, 0.9), column=(0.6, 0.6))
+    o = run(cfg)
+    nf, H = cfg["n_fluid"], cfg["H"]
+    m0 = o.stats()["mass"]
+    o.step(1000)
+    psum, cnt = np.zeros(nf), 0
+    for _ in range(40):
+        o.step(50)
+        psum += o.fields()["p"][:nf]
+        cnt += 1
+    f = o.fields()
+    y = f["pos"][:nf, 1]
+    pa = 1000.0 * 9.81 * (H - y)
+    pavg = psum / cnt
+    rel = math.sqrt(np.mean((pavg - pa) ** 2)) / (1000.0 * 9.81 * H)
+    assert rel < 0.03
+    slope = np.polyfit(y, pavg, 1)[0]
+    assert abs(slope / (-1000.0 * 9.81) - 1.0) < 0.03
+    s = o.stats()
+    assert s["mass"] == m0 and abs(m0 - 1000.0 * cfg["dp"] ** 2 * nf) < 1e-9 * m0
+    assert s["escaped"] == 0
+    assert np.abs(f["vel"][:nf]).max() < 0.1 * math.sqrt(9.81 * H)
+
+
+def test_P14_potential_energy_of_paper_column():
+    """T_tot = 1226.25 J for L = 1 m, H = 0.5 m of water; the lattice
+    midpoint rule is exact for a linear integrand, for every dp of PAPER.md:222."""
+    T = _gold("paper_values.txt")["T_tot_J"]
+    for dp in (0.01, 0.005):
+        cfg = inputs.dam_break_2d(dp=dp, tank=(1.0, 1.0), column=(1.0, 0.5))
+        nf = cfg["n_fluid"]
+        m = 1000.0 * dp ** 2
+        ep = np.sum(m * 9.81 * cfg["pos"][:nf, 1].astype(np.float64))
+        assert abs(ep - T) < 1e-4 * T
+    o = run(inputs.dam_break_2d(dp=0.02, tank=(1.0, 1.0), column=(1.0, 0.5)))
+    assert abs(o.stats()["mass"] - 1000.0 * 1.0 * 0.5) < 1e-9
+
+
+# ------------------------------------------------------------------ P6 neighbour search
+def test_P6_cell_list_equals_brute_force():
+    cfg = inputs.dam_break_2d()
+    o = run(cfg)
+    o.step(150)
+    a, b = o.neighbours(), o.neighbours_bruteforce()
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+    cfg = inputs.box_sweep_3d(n=8)
+    o = run(cfg)
+    a, b = o.neighbours(), o.neighbours_bruteforce()
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+    assert o.stats()["npairs"] == int((a[0][1:] - a[0][:-1])[:cfg["n_fluid"]].sum())
+
+
+def test_f32_contract_grid_walk_equals_brute_force():
+    for cfg in (inputs.dam_break_2d(), inputs.box_sweep_3d(n=10), inputs.shuffled(inputs.box_2d(n=20, jitter=0.3))):
+        a = orc.f32_neighbours(cfg, cfg["pos"], cfg["tag"], grid=False)
+        b = orc.f32_neighbours(cfg, cfg["pos"], cfg["tag"], grid=True)
+        assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+        cell_id, perm, cs, ce = orc.f32_cells(cfg, cfg["pos"], cfg["tag"])
+        n = len(cfg["tag"])
+        assert sorted(perm.tolist()) == list(range(n))
+        nf = int((cfg["tag"] >= 0).sum())
+        for blk in (perm[:nf], perm[nf:]):
+            key = cell_id[blk].astype(np.int64) * n + blk
+            assert np.all(np.diff(key) > 0)          # sorted by cell, ids ascending within
+
+
+# ------------------------------------------------------------------ P7 / P18 Riemann terms
+def test_P7_riemann_reduces_to_plain_averages():
+    s = orc.riemann(1000.0, -0.3, 5000.0, 40.0, 1000.0, 0.2, 5000.0, 40.0)
+    assert s["pstar"] == 5000.0                     # U_L <= U_R: beta = 0
+    assert abs(s["Ustar"] - (-0.05)) < 1e-15
+    s = orc.riemann(1000.0, 0.3, 5000.0, 40.0, 1000.0, -0.2, 7000.0, 40.0)
+    # Eq. 2.8 by hand: beta = min(1.5, 40) = 1.5
+    assert abs(s["pstar"] - (6000.0 + 500.0 * 1.5 * 0.5)) < 1e-9
+    assert abs(s["Ustar"] - (0.05 + 0.5 * (-2000.0) / (40.0 * 1000.0))) < 1e-15
+    # limiter saturates at c
+    s = orc.riemann(1000.0, 30.0, 0.0, 40.0, 1000.0, -30.0, 0.0, 40.0)
+    assert abs(s["pstar"] - 500.0 * 40.0 * 60.0) < 1e-6
+
+
+def test_P18_acoustic_extension_equals_paper_at_equal_c():
+    rng = np.random.default_rng(3)
+    for _ in range(50):
+        rL, rR = rng.uniform(0.5, 1200.0, 2)
+        UL, UR = rng.uniform(-3, 3, 2)
+        pL, pR = rng.uniform(-1e3, 1e4, 2)
+        c = rng.uniform(10, 100)
+        a = orc.riemann(rL, UL, pL, c, rR, UR, pR, c, mode=1)
+        b = orc.riemann(rL, UL, pL, c, rR, UR, pR, c, mode=2)
+        for k in a:
+            assert abs(a[k] - b[k]) <= 1e-12 * max(1.0, abs(a[k]))
+    # symmetric under exchange of the two particles: p*(L,R) = p*(R,L) with
+    # U -> -U (e_ji = -e_ij)
+    a = orc.riemann(1000.0, 0.4, 3e3, 44.0, 1.2, -0.7, 1e3, 1400.0)
+    b = orc.riemann(1.2, 0.7, 1e3, 1400.0, 1000.0, -0.4, 3e3, 44.0)
+    assert abs(a["pstar"] - b["pstar"]) < 1e-9 * abs(a["pstar"])
+    assert abs(a["Ustar"] + b["Ustar"]) < 1e-12
+
+
+# ------------------------------------------------------------------ P8 antisymmetry
+@pytest.mark.parametrize("dim,two_phase", [(2, False), (3, False), (2, True)])
+def test_P8_total_momentum_of_internal_forces_vanishes(dim, two_phase):
+    rng = np.random.default_rng(11)
+    dp = 1.0 / 64
+    pos = lattice(dim, 6, dp) + rng.uniform(-0.2 * dp, 0.2 * dp, (6 ** dim, dim))
+    n = len(pos)
+    vel = np.zeros((n, 3))
+    vel[:, :dim] = rng.uniform(-1, 1, (n, dim))
+    if two_phase:
+        tag = (pos[:, 1] > 3 * dp).astype(int)
+        rho0, c0 = (1000.0, 1.0), (20.0, 20.0 * math.sqrt(1000.0))
+        rho = np.where(tag == 0, 1000.0, 1.0) * (1 + rng.uniform(0, 0.01, n))
+    else:
+        tag, rho0, c0 = np.zeros(n, int), (1000.0,), (20.0,)
+        rho = 1000.0 * (1 + rng.uniform(0, 0.01, n))
+    o = run(custom(dim, pos, tag, rho, vel=vel, dp=dp, rho0=rho0, c0=c0))
+    f = o.fields()
+    m = np.array(rho0)[tag] * dp ** dim
+    tot = (m[:, None] * f["acc"]).sum(0)
+    scale = np.abs(m[:, None] * f["acc"]).sum()
+    assert np.all(np.abs(tot) < 1e-12 * scale)
+    # two isolated particles: m_i a_i = -m_j a_j exactly as vectors
+    p2 = np.array([[0.0] * dim, [1.1 * dp] + [0.3 * dp] * (dim - 1)])
+    v2 = np.zeros((2, 3)); v2[0, 0], v2[1, 0] = 0.7, -0.4
+    o = run(custom(dim, p2, tag[:2] * 0, [1004.0, 1001.0], vel=v2, dp=dp, c0=(20.0,)))
+    a = o.fields()["acc"]
+    assert np.allclose(a[0], -a[1], rtol=1e-13, atol=0) and abs(a[0, 0]) > 0
+
+
+# ------------------------------------------------------------------ P9 / P10
+def test_P9_continuity_scalar_identity_two_particles():
+    """(v_i - v*).grad_i W_ij = (U* - U_L) W'(r) because v*.e = U* (SURVEY P9); with
+    U* - U_L = [(p_i - p_j)/c - rho_j v_ij.e] / (rho_i + rho_j) for equal c."""
+    dp, c = 1.0 / 64, 20.0
+    f32 = lambda a: np.asarray(a, np.float32).astype(np.float64)   # the oracle sees float32 inputs
+    pos = f32([[0.0, 0.0, 0.0], [0.9 * dp, 0.5 * dp, -0.4 * dp]])
+    vel = f32([[0.3, -0.2, 0.5], [-0.1, 0.4, 0.2]])
+    rho = np.array([1003.0, 1001.0])
+    o = run(custom(3, pos, [0, 0], rho, vel=vel, dp=dp, c0=(c,), flags=0))
+    o.step(1, dts=[1e-14])
+    d = pos[0] - pos[1]
+    r = np.linalg.norm(d)
+    e = -d / r
+    p = c * c * (rho - 1000.0)
+    vij_e = (vel[0] - vel[1]) @ e
+    dU = ((p[0] - p[1]) / c - rho[1] * vij_e) / (rho[0] + rho[1])
+    V1 = 1000.0 * dp ** 3 / rho[1]
+    expect = 2 * rho[0] * V1 * dU * orc.kernel_dw(3, 1.3 * dp, r)
+    got = o.fields()["drho"][0]
+    assert abs(got - expect) < 1e-9 * abs(expect)
+
+
+def test_P10_galilean_invariance():
+    rng = np.random.default_rng(5)
+    dp = 1.0 / 64
+    pos = lattice(3, 5, dp) + rng.uniform(-0.2 * dp, 0.2 * dp, (125, 3))
+    vel = rng.uniform(-1, 1, (125, 3))
+    rho = 1000.0 * (1 + rng.uniform(0, 0.01, 125))
+    out = []
+    for boost in (np.zeros(3), np.array([3.0, -2.0, 1.0])):
+        o = run(custom(3, pos, np.zeros(125), rho, vel=vel + boost, dp=dp, c0=(20.0,), flags=0))
+        a0 = o.fields()["acc"].copy()
+        o.step(1, dts=[1e-14])
+        out.append((a0, o.fields()["drho"].copy()))
+    assert np.allclose(out[0][0], out[1][0], rtol=0, atol=1e-5 * np.abs(out[0][0]).max())
+    assert np.allclose(out[0][1], out[1][1], rtol=0, atol=1e-5 * np.abs(out[0][1]).max())
+    # uniform v, p, rho on a lattice: d rho/dt = 0
+    pos = lattice(3, 7, dp)
+    o = run(custom(3, pos, np.zeros(343), np.full(343, 1002.0), vel=np.tile([1.0, 2.0, 3.0], (343, 1)),
+                   dp=dp, c0=(20.0,), flags=0))
+    o.step(1, dts=[1e-14])
+    assert np.abs(o.fields()["drho"]).max() < 1e-6      # pair terms are O(1e3) each
+
+
+def test_P11_tangential_flow_along_mirror_wall_keeps_density():
+    dp, nx = 1.0 / 64, 15
+    fl = lattice(2, nx, dp)
+    fl = fl[fl[:, 1] < 6 * dp]
+    wl = np.array([[(i + 0.5) * dp, -(j + 0.5) * dp] for i in range(nx) for j in range(3)])
+    pos = np.concatenate([fl, wl])
+    tag = np.concatenate([np.zeros(len(fl)), -np.ones(len(wl))])
+    vel = np.zeros((len(pos), 3)); vel[:len(fl), 0] = 0.8
+    o = run(custom(2, pos, tag, np.full(len(pos), 1002.0), vel=vel, dp=dp, c0=(20.0,), flags=orc.FLAG_WALL_VEL_MIRROR))
+    o.step(1, dts=[1e-14])
+    f = o.fields()
+    centre = np.argmin(np.linalg.norm(fl - np.array([nx / 2 * dp, 0.5 * dp]), axis=1))
+    assert abs(f["drho"][centre]) < 1e-8
+    # the mirrored wall velocity is minus the fluid's tangential velocity
+    wc = len(fl) + np.argmin(np.linalg.norm(wl - np.array([nx / 2 * dp, -0.5 * dp]), axis=1))
+    assert abs(f["vel"][wc, 0] + float(np.float32(0.8))) < 1e-12
+
+
+# ------------------------------------------------------------------ P12 integrator
+def test_P12_free_fall_is_exact_and_dt_body_force():
+    dp, g = 0.05, 9.81
+    v0 = np.array([[0.25, 0.125, 0.0]])     # exactly representable in float32
+    cfg = custom(3, np.array([[0.0, 0.0, 10.0]]), [0], [1000.0], vel=v0, dp=dp, c0=(0.05,), g=(0, 0, -g),
+                 domain_min=[-5, -5, -5], domain_max=[5, 5, 15])
+    o = run(cfg)
+    dts = o.step(7)
+    assert abs(dts[0] - 0.25 * math.sqrt(1.3 * dp / g)) < 1e-15
+    t = dts.sum()
+    f = o.fields()
+    expect = np.array([0.25 * t, 0.125 * t, 10.0 - 0.5 * g * t * t])
+    assert np.allclose(f["pos"][0], expect, rtol=0, atol=1e-12)
+    assert np.allclose(f["vel"][0], [0.25, 0.125, -g * t], rtol=0, atol=1e-12)
+    # CFL branch, Eq. 2.23 with U_max = current max |v| (reading A17)
+    cfg = custom(3, np.array([[0.0, 0.0, 0.0]]), [0], [1000.0], vel=[[3.0, 4.0, 0.0]], dp=dp, c0=(50.0,))
+    assert abs(run(cfg).step(1)[0] - 0.25 * 1.3 * dp / 55.0) < 1e-15
+
+
+# ------------------------------------------------------------------ P13 reinitialisation
+def test_P13_reinitialisation_cases():
+    s0 = 1.0095
+    assert orc.reinit_density(1001.0, 1000.0, 1.002 * s0, s0, 1) == pytest.approx(1002.0, abs=1e-10)
+    got = orc.reinit_density(1004.0, 1000.0, 0.6 * s0, s0, 1)   # free surface: rho_s < rho*
+    assert got == pytest.approx(600.0 + 404.0 * 1000.0 / 1004.0, abs=1e-10)
+    lo = orc.reinit_density(1003.0, 1000.0, 1.003 * s0 * (1 - 1e-12), s0, 1)
+    hi = orc.reinit_density(1003.0, 1000.0, 1.003 * s0 * (1 + 1e-12), s0, 1)
+    assert abs(lo - hi) < 1e-6                                   # continuous at rho_s = rho*
+    assert orc.reinit_density(1004.0, 1.0, 0.9 * s0, s0, 0) == pytest.approx(0.9, abs=1e-12)  # Eq. 2.18
+
+
+# ------------------------------------------------------------------ P15 penalty
+def _wall_patch(nx, dp):
+    return np.array([[(i + 0.5) * dp, -(j + 0.5) * dp] for i in range(nx) for j in range(3)])
+
+
+def test_P15_penalty_zero_on_lattice_and_pushes_along_normal():
+    dp, nx, c = 1.0 / 64, 13, 20.0
+    wl = _wall_patch(nx, dp)
+    x0 = (nx // 2 + 0.5) * dp
+
+    def acc(y, mask, rho=1003.0):
+        pos = np.concatenate([[[x0, y]], wl])
+        tag = np.concatenate([[0], -np.ones(len(wl))])
+        rho_a = np.concatenate([[rho], np.full(len(wl), 1000.0)])
+        return run(custom(2, pos, tag, rho_a, dp=dp, c0=(c,), penalty_phase_mask=mask)).fields()["acc"][0]
+
+    # undisturbed lattice position: normal distance dp >= dp/2 -> no penalty
+    assert np.array_equal(acc(0.5 * dp, 1), acc(0.5 * dp, 0))
+    assert np.array_equal(acc(0.0 * dp + 1e-9, 1), acc(0.0 * dp + 1e-9, 0))   # exactly dp/2 away
+    # closer than dp/2 to the first layer: extra push along +n_w = +y, none along x
+    d = acc(-0.2 * dp, 1) - acc(-0.2 * dp, 0)
+    assert d[1] > 0 and abs(d[0]) < 1e-9 * d[1]
+    # closed form of reading A8/A9b for this geometry (flat wall, n = (0,1)):
+    # sum over first-layer particles of 2 V0/rho_i * gamma*(1-delta)^2*|p_i s| * |W'(r)|
+    rho_i, y = 1003.0, -0.2 * dp
+    p_i = c * c * (rho_i - 1000.0)
+    tot = 0.0
+    for w in wl[np.isclose(wl[:, 1], -0.5 * dp)]:
+        dvec = np.array([x0, y]) - w
+        r = np.linalg.norm(dvec)
+        if r >= 2.6 * dp:
+            continue
+        delta = 2 * dvec[1] / dp
+        if -1 < delta < 1:
+            tot += 2 * dp ** 2 / rho_i * (1 - delta) ** 2 * abs(p_i * dvec[1] / r) * -orc.kernel_dw(2, 1.3 * dp, r)
+    assert tot > 0 and abs(d[1] - tot) < 1e-6 * tot      # float32-rounded input positions
+    # scales linearly with gamma_p and vanishes with p_i
+    assert np.allclose(acc(-0.2 * dp, 1, rho=1000.0), acc(-0.2 * dp, 0, rho=1000.0))
+
+
+# ------------------------------------------------------------------ P16 normals
+def test_P16_wall_normals():
+    cfg = inputs.dam_break_2d()
+    o = run(cfg)
+    n, pos, dp = o.normals(), cfg["pos"].astype(np.float64), cfg["dp"]
+
+    def at(x, y):
+        i = np.argmin(np.abs(pos[:, 0] - x * dp) + np.abs(pos[:, 1] - y * dp))
+        assert cfg["tag"][i] == -1
+        return n[i]
+
+    assert np.allclose(at(40.5, -0.5), [0, 1, 0], atol=2e-5)        # floor, first layer: into fluid
+    assert np.allclose(at(40.5, -1.5), [0, 0, 0], atol=0)            # middle layer: degenerate -> 0
+    assert np.allclose(at(40.5, -2.5), [0, -1, 0], atol=2e-5)       # outer layer: away from the wall bulk
+    assert np.allclose(at(-0.5, 30.5), [1, 0, 0], atol=2e-5)        # left wall
+    assert np.allclose(at(-0.5, -0.5), [math.sqrt(0.5)] * 2 + [0], atol=2e-5)   # corner -> diagonal
+    assert np.all(n[cfg["tag"] >= 0] == 0)
+
+
+def test_long_run_keeps_particles_inside_P17():
+    cfg = inputs.dam_break_2d()
+    o = run(cfg)
+    o.step(1500)
+    s = o.stats()
+    assert s["escaped"] == 0 and s["mass"] == pytest.approx(2000.0, rel=1e-12)
+    assert 1.2 < s["x_front"] < 4.0 and s["ek"] > 0
