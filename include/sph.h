@@ -1,0 +1,172 @@
+/* include/sph.h — C ABI of libsph, the B200 (sm_100a) implementation of the per-time-step
+ * particle pipeline of arXiv 2110.02621 (Rezavand, Zhang, Hu: "Generalised and efficient wall
+ * boundary condition treatment in GPU-accelerated SPH").
+ *
+ * Citations are PAPER.md:<line> (+ equation).  "Reading Axx" refers to DESIGN.md §3.
+ *
+ * Conventions
+ *  - No torch types, no C++ types, no exceptions cross this boundary.
+ *  - Every function returns 0 (SPH_OK) or a negative sph_error; sph_last_error() gives text.
+ *  - Pointers named *_dev are DEVICE pointers owned by the caller (e.g. torch tensors);
+ *    pointers named *_host are HOST pointers owned by the caller.  The library copies in
+ *    at sph_set_particles* and out at sph_get_fields*; it never keeps a caller pointer.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Calls are
+ *    asynchronous on that stream unless stated; the *_host variants and the calls that
+ *    return values to the host synchronise the stream before returning.
+ *  - Particle arrays are in the CALLER'S ORDER: pos[n*3], vel[n*3] (xyz interleaved, z ignored
+ *    in 2-D), rho[n], tag[n].  tag = phase id 0..n_phases-1 for fluid (phase 0 the heaviest),
+ *    SPH_TAG_WALL for wall dummy particles.  Results come back in the same
+ *    order; the internal cell-sorted order is visible only through sph_debug_*.
+ *  - Arithmetic is float32 on the device ("fully developed on single precision");
+ *    density is held as the deviation rho - rho0 of the particle's phase.
+ *  - There is no CPU fallback: every call fails with SPH_ECUDA if no CUDA device is usable.
+ */
+#ifndef SPH_H_
+#define SPH_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sph_ctx sph_ctx; /* opaque; owned by the library; one per simulation */
+
+enum { SPH_MAX_PHASES = 4, SPH_TAG_WALL = -1 };
+
+enum sph_flags {
+  SPH_FLAG_REINIT = 1,          /* density reinitialisation each step, Eq. 2.17/2.18 */
+  SPH_FLAG_WALL_VEL_MIRROR = 2  /* v_w = 2 v_wall - <v_f> (Adami-style mirror; reading A6), else v_w = v_wall */
+};
+
+enum sph_error {
+  SPH_OK = 0,
+  SPH_EINVAL = -1,      /* bad argument / tag out of range / called before sph_set_particles */
+  SPH_ENOMEM = -2,      /* device or host allocation failed */
+  SPH_ECUDA = -3,       /* CUDA runtime error (no device, launch failure, ...) */
+  SPH_ENONFINITE = -4,  /* a non-finite position or velocity was seen (reported by sph_get_stats) */
+  SPH_EDTUNDERFLOW = -5 /* the time step fell below 1e-12 (reported by sph_get_stats) */
+};
+
+/* Physical and numerical parameters: the paper's statement of the problem. */
+typedef struct {
+  int32_t dim;                   /* 2 or 3   */
+  int32_t n_phases;              /* 1..SPH_MAX_PHASES  */
+  double dp;                     /* initial particle spacing dx */
+  double h;                      /* smoothing length (paper: 1.3 dx; support 2h) */
+  double rho0[SPH_MAX_PHASES];   /* reference density per phase  */
+  double c0[SPH_MAX_PHASES];     /* speed of sound per phase, Eq. 2.3 (reading A2, A3) */
+  double g[3];                   /* body acceleration */
+  double g_osc_amp[3];           /* g(t) = g + g_osc_amp * sin(2 pi t / g_osc_period)   (config 3)   */
+  double g_osc_period;           /* 0 = constant gravity                                             */
+  double cfl;                    /* 0.25 in Eq. 2.23 and 2.24 */
+  double penalty_strength;       /* gamma_p (paper: 1) */
+  uint32_t penalty_phase_mask;   /* bit k: phase k receives F_p, Eq. 2.13 (reading A11) PAPER.md:120 */
+  uint32_t free_surface_mask;    /* bit k: phase k uses continuity Eq. 2.9/2.21 + reinit Eq. 2.17;
+                                    otherwise summation Eq. 2.4 + reinit Eq. 2.18 (reading A13, A15) */
+  uint32_t flags;                /* sph_flags */
+  uint32_t reserved;
+  double domain_min[3];          /* box of the cell grid; particles outside are binned in the edge */
+  double domain_max[3];          /* cells and counted as escaped (reading A23)                      */
+} sph_params;
+
+typedef struct {
+  double t;          /* simulated time                                  */
+  double dt;         /* last time step used                             */
+  int64_t steps;     /* steps taken since sph_set_particles             */
+  int64_t n_fluid;
+  int64_t n_wall;
+  int64_t n_pairs;   /* directed pairs (i fluid, j any tag, j != i, r < 2h) at the current positions */
+  double e_kin;      /* sum 1/2 m |v|^2 over fluid                      */
+  double mass;       /* sum m over fluid (m = rho0_phase dp^dim, reading A19) */
+  double x_front;    /* max x over phase-0 particles within 3 dp of the floor (floor = domain_min[dim-1] + 3 dp) */
+  int64_t escaped;   /* fluid particles outside [domain_min, domain_max) at the last cell build */
+  int64_t nonfinite; /* non-finite positions/velocities seen so far     */
+} sph_stats;
+
+/* Stages timed by sph_set_profiling (indices into sph_get_timings' array). */
+enum sph_stage {
+  SPH_STAGE_PREDICT = 0,   /* dt reduction + reinit (Eq. 2.17/2.18) + half kick + drift (Eq. 2.19-2.20) + cell hash */
+  SPH_STAGE_SORT = 1,      /* device radix sort of (cell id, index) */
+  SPH_STAGE_REORDER = 2,   /* gather into sorted SoA float4 + cell ranges */
+  SPH_STAGE_WALL = 3,      /* wall extrapolation Eq. 2.12 (both calls of a step) */
+  SPH_STAGE_PASS_A = 4,    /* sigma + continuity Eq. 2.9 + density update Eq. 2.21 / 2.4 + EOS */
+  SPH_STAGE_PASS_B = 5,    /* momentum Eq. 2.10/2.11 + penalty Eq. 2.13 + second kick Eq. 2.22 */
+  SPH_STAGE_COUNT = 6
+};
+
+/* Create a context.  Validates the parameters (SPH_EINVAL), selects the current CUDA device. */
+int sph_create(const sph_params* params, sph_ctx** out);
+
+/* Free everything the context owns.  NULL is allowed. */
+void sph_destroy(sph_ctx* ctx);
+
+/* Load n particles (fluid + wall).  One-off set-up work happens here (PAPER.md:101, :139-143,
+ * SURVEY §8(c) O-0): masses, the static wall cell list, wall normals Eq. 2.16 (in float64,
+ * reading A10), the first fluid cell list, sigma_i, wall extrapolation and (dv/dt)^0 (reading
+ * A18).  Resets t = 0.  May be called again to restart from a checkpoint.
+ * Synchronises the stream (it sizes allocations from the tag counts). */
+int sph_set_particles(sph_ctx* ctx, int64_t n, const float* pos_dev, const float* vel_dev,
+                      const float* rho_dev, const int32_t* tag_dev, void* stream);
+int sph_set_particles_host(sph_ctx* ctx, int64_t n, const float* pos_host, const float* vel_host,
+                           const float* rho_host, const int32_t* tag_host, void* stream);
+
+/* Advance n_steps kick-drift-kick steps (Eq. 2.19-2.24); dt is computed on
+ * the device each step from Eq. 2.23-2.24 (reading A17).  Asynchronous; no host sync per step. */
+int sph_step(sph_ctx* ctx, int32_t n_steps, void* stream);
+
+/* Same, with a caller-given dt sequence (host array of n_steps doubles) so that the oracle and
+ * the device can be driven by identical time steps in parity runs. */
+int sph_step_dt(sph_ctx* ctx, int32_t n_steps, const double* dt_host, void* stream);
+
+/* Copy fields out in the caller's particle order.  Any pointer may be NULL.
+ * pos, vel, acc: n*3; rho, p: n.  Wall entries: vel = extrapolated v_w, p = p_w (Eq. 2.12),
+ * rho = rho0[0] + p_w / c0[0]^2, acc = 0.  The _host variant synchronises. */
+int sph_get_fields(sph_ctx* ctx, float* pos_dev, float* vel_dev, float* rho_dev, float* p_dev,
+                   float* acc_dev, void* stream);
+int sph_get_fields_host(sph_ctx* ctx, float* pos_host, float* vel_host, float* rho_host,
+                        float* p_host, float* acc_host, void* stream);
+
+/* Integral quantities; runs small reduction kernels and synchronises.  Returns SPH_ENONFINITE /
+ * SPH_EDTUNDERFLOW (with *out filled) if the run has gone bad. */
+int sph_get_stats(sph_ctx* ctx, sph_stats* out, void* stream);
+
+/* Per-stage device times.  With profiling on, sph_step brackets every stage with CUDA events
+ * on the caller's stream; sph_get_timings synchronises and returns the accumulated milliseconds
+ * per stage since the last call (ms_host[SPH_STAGE_COUNT]) and the number of steps they cover. */
+int sph_set_profiling(sph_ctx* ctx, int32_t on);
+int sph_get_timings(sph_ctx* ctx, float* ms_host, int32_t* n_steps_host);
+
+/* Number of cells of the grid (cell edge 2h(1+2^-10), reading A24). */
+int64_t sph_num_cells(const sph_ctx* ctx);
+
+/* Integer contract, all HOST pointers, synchronises:
+ * cell_id[n]: cell of every particle, caller order; perm[n]: fluid ids in cell-sorted order
+ * followed by wall ids in cell-sorted order; cell_start/cell_end[2*ncell]: ranges in the fluid
+ * block then in the wall block (both 0 for an empty cell).  Any pointer may be NULL. */
+int sph_debug_cells(sph_ctx* ctx, int32_t* cell_id_host, int32_t* perm_host,
+                    int32_t* cell_start_host, int32_t* cell_end_host, void* stream);
+
+/* Neighbour lists in CSR form, caller ids, ascending within a row: fluid i -> all j != i with
+ * r2 < 4h^2 (float32 rule of reading A24); wall i -> fluid j only.  offsets_host[n+1];
+ * ids_host may be NULL (count only) and holds at most cap entries.  *total_host = number of
+ * entries needed. */
+int sph_debug_neighbours(sph_ctx* ctx, int64_t* offsets_host, int32_t* ids_host, int64_t cap,
+                         int64_t* total_host, void* stream);
+
+/* Wall normals Eq. 2.16 in caller order (n*3, zero for fluid entries); HOST pointer. */
+int sph_debug_normals(sph_ctx* ctx, float* normals_host, void* stream);
+
+/* Per-particle number density sigma_i (first n floats) and d rho/dt (next n floats) of the last
+ * pass A, caller order, zero for wall entries; sigma_drho_host holds 2*n floats (HOST). */
+int sph_debug_sigma(sph_ctx* ctx, float* sigma_drho_host, void* stream);
+
+/* Number of kernel launches issued by the library since sph_create (bench.py's gpu_launches). */
+int64_t sph_launch_count(const sph_ctx* ctx);
+
+const char* sph_last_error(const sph_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPH_H_ */
