@@ -41,6 +41,8 @@ struct DP {
   int nx, ny, nz;
   float dmin[3], dmax[3];
   double cmax, cfl, hD;
+  double massD[SPH_MAX_PHASES];
+  double hinvD, a_over_s0, sigma0D;
   double g[3], gamp[3], gperiod;
 };
 
@@ -84,7 +86,8 @@ __device__ __forceinline__ float warp_sum(float v) {
 __global__ void k_load_fluid(DP p, int nf, const int* __restrict__ fid, const float* __restrict__ pos,
                              const float* __restrict__ vel, const float* __restrict__ rho,
                              const int* __restrict__ tag, float4* __restrict__ TP,
-                             float4* __restrict__ TV, unsigned* __restrict__ ID,
+                             float4* __restrict__ TV, double2* __restrict__ TDxy, double* __restrict__ TDz,
+                             unsigned* __restrict__ ID,
                              unsigned* __restrict__ keys, unsigned* __restrict__ vals) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= nf) return;
@@ -93,6 +96,8 @@ __global__ void k_load_fluid(DP p, int nf, const int* __restrict__ fid, const fl
   float x = pos[3 * o], y = pos[3 * o + 1], z = p.dim == 3 ? pos[3 * o + 2] : 0.0f;
   float drho = (float)((double)rho[o] - (double)p.rho0[ph]);
   TP[i] = make_float4(x, y, z, drho);
+  TDxy[i] = make_double2((double)x, (double)y);
+  TDz[i] = (double)z;
   TV[i] = make_float4(vel[3 * o], vel[3 * o + 1], p.dim == 3 ? vel[3 * o + 2] : 0.0f,
                       __int_as_float(ph));
   ID[i] = (unsigned)o;
@@ -263,14 +268,35 @@ __global__ void k_cell_bounds(const unsigned* __restrict__ keys, int n, int ncel
 }
 
 __global__ void k_reorder(int n, const unsigned* __restrict__ vals, const float4* __restrict__ TP,
-                          const float4* __restrict__ TV, const unsigned* __restrict__ IDin,
-                          float4* __restrict__ P, float4* __restrict__ V, unsigned* __restrict__ IDout) {
+                          const float4* __restrict__ TV, const double2* __restrict__ TDxy,
+                          const double* __restrict__ TDz, const unsigned* __restrict__ IDin,
+                          float4* __restrict__ P, float4* __restrict__ V, double2* __restrict__ Dxy,
+                          double* __restrict__ Dz, float4* __restrict__ L, unsigned* __restrict__ IDout) {
   int s = blockIdx.x * blockDim.x + threadIdx.x;
   if (s >= n) return;
   unsigned v = vals[s];
-  P[s] = TP[v];
+  const float4 r = TP[v];
+  P[s] = r;
   if (TV) V[s] = TV[v];
+  if (TDxy) {
+    // float64 master position; (P.xyz, L.xyz) is its two-float image: hi = float32 rounding, lo = remainder
+    const double2 xy = TDxy[v];
+    const double z = TDz[v];
+    Dxy[s] = xy;
+    Dz[s] = z;
+    L[s] = make_float4((float)(xy.x - (double)r.x), (float)(xy.y - (double)r.y), (float)(z - (double)r.z), 0.f);
+  }
   IDout[s] = IDin[v];
+}
+
+// Static wall positions as float64 (exact images of the caller's float32), for the sigma sum.
+__global__ void k_wall_double(int n, const float4* __restrict__ WP, double2* __restrict__ Dxy,
+                              double* __restrict__ Dz) {
+  int s = blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= n) return;
+  const float4 r = WP[s];
+  Dxy[s] = make_double2((double)r.x, (double)r.y);
+  Dz[s] = (double)r.z;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -330,11 +356,26 @@ __device__ __forceinline__ void walk(const DP& p, const float4* __restrict__ P, 
 
 constexpr int PW = 8;  // warps per block in the pair kernels
 
+// W(r)/alpha_d = (1 - q/2)^4 (1 + 2q) in float64 from a float64 separation (reading A1).  Used only
+// for the number density sigma_i, whose relative error is amplified by c0^2 ~ 200 g H into the
+// pressure (DESIGN.md §4 "precision").  sqrt: one MUFU.RSQ64H seed + one Newton step (~1e-13).
+__device__ __forceinline__ double wendland64(const DP& p, double dx, double dy, double dz) {
+  const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(r2));
+  const double e = fma(-r2 * y, y, 1.0);
+  y = fma(0.5 * y, e, y);
+  const double q = r2 > 0.0 ? r2 * y * p.hinvD : 0.0;
+  const double t = fmax(fma(-0.5, q, 1.0), 0.0), t2 = t * t;
+  return t2 * t2 * fma(2.0, q, 1.0);
+}
+
 // Wall extrapolation, Eq. 2.12 (readings A4-A7); a_w = 0, v_wall = 0.
 template <bool MULTI, bool WITH_VEL>
 __global__ void __launch_bounds__(PW * 32)
 k_wall(DP p, const SS* __restrict__ S, int nw, float4* __restrict__ WP, float4* __restrict__ WV,
-       const float4* __restrict__ P, const float4* __restrict__ V, const int* __restrict__ lbF) {
+       const float4* __restrict__ P, const float4* __restrict__ V, const float4* __restrict__ LO,
+       const int* __restrict__ lbF) {
   __shared__ unsigned qs[PW][64];
   const int w = blockIdx.x * PW + (threadIdx.x >> 5);
   if (w >= nw) return;
@@ -342,8 +383,9 @@ k_wall(DP p, const SS* __restrict__ S, int nw, float4* __restrict__ WP, float4* 
   const float4 pw = WP[w];
   float sW = 0, sp = 0, sWr = 0, srx = 0, sry = 0, srz = 0, svx = 0, svy = 0, svz = 0;
   walk(p, P, lbF, pw.x, pw.y, pw.z, -1, qs[threadIdx.x >> 5], [&](int j) {
-    const float4 pj = P[j];
-    const float dx = pw.x - pj.x, dy = pw.y - pj.y, dz = pw.z - pj.z;  // r_wf
+    const float4 pj = P[j], lj = LO[j];
+    // r_wf with the low-order part of the fluid position (two-float positions)
+    const float dx = (pw.x - pj.x) - lj.x, dy = (pw.y - pj.y) - lj.y, dz = (pw.z - pj.z) - lj.z;
     const float r2 = dist2(dx, dy, dz);
     const float r = r2 > 0.f ? r2 * rsqrtf(r2) : 0.f;
     const float q = r * p.hinv, t = fmaf(-0.5f, q, 1.0f), t2 = t * t;
@@ -390,9 +432,10 @@ k_wall(DP p, const SS* __restrict__ S, int nw, float4* __restrict__ WP, float4* 
 template <bool MULTI>
 __global__ void __launch_bounds__(PW * 32)
 k_pass_a(DP p, const SS* __restrict__ S, int nf, int init, const float4* __restrict__ P,
-         const float4* __restrict__ V, const int* __restrict__ lbF, const float4* __restrict__ WP,
-         const float4* __restrict__ WV, const int* __restrict__ lbW, float4* __restrict__ Pout,
-         float* __restrict__ SIG, float* __restrict__ DRHO, const unsigned* __restrict__ IDin,
+         const float4* __restrict__ V, const double2* __restrict__ Dxy, const double* __restrict__ Dz,
+         const int* __restrict__ lbF, const float4* __restrict__ WP, const float4* __restrict__ WV,
+         const double2* __restrict__ WDxy, const double* __restrict__ WDz, const int* __restrict__ lbW,
+         float4* __restrict__ Pout, float* __restrict__ SIG, float* __restrict__ DRHO, const unsigned* __restrict__ IDin,
          unsigned* __restrict__ IDout) {
   __shared__ unsigned qs[PW][64];
   const int i = blockIdx.x * PW + (threadIdx.x >> 5);
@@ -400,16 +443,21 @@ k_pass_a(DP p, const SS* __restrict__ S, int nf, int init, const float4* __restr
   const int lane = threadIdx.x & 31;
   unsigned* q = qs[threadIdx.x >> 5];
   const float4 pi = P[i], vi = V[i];
+  const double2 xyi = Dxy[i];
+  const double zi = p.dim == 3 ? Dz[i] : 0.0;
+  const bool d3 = p.dim == 3;
   const int phi = MULTI ? __float_as_int(vi.w) : 0;
   const float rhoi = p.rho0[phi] + pi.w, prsi = p.c2[phi] * pi.w, ci = p.c0[phi], ZL = rhoi * ci;
-  float sig = 0.f, acc = 0.f;
+  double sig = 0.0;
+  float acc = 0.f;
   walk(p, P, lbF, pi.x, pi.y, pi.z, i, q, [&](int j) {
     const float4 pj = P[j], vj = V[j];
-    const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;  // r_ij
+    const double2 xyj = Dxy[j];
+    sig += wendland64(p, xyi.x - xyj.x, xyi.y - xyj.y, d3 ? zi - Dz[j] : 0.0);
+    const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;  // r_ij (float32 image)
     const float r2 = dist2(dx, dy, dz);
     const float r = r2 > 0.f ? r2 * rsqrtf(r2) : 0.f;
     const float qq = r * p.hinv, t = fmaf(-0.5f, qq, 1.0f), t2 = t * t;
-    sig = fmaf(p.alpha * t2 * t2, fmaf(2.0f, qq, 1.0f), sig);
     const float Fg = p.gradc * t2 * t;  // W'(r)/r
     const int phj = MULTI ? __float_as_int(vj.w) : 0;
     const float rhoj = p.rho0[phj] + pj.w;
@@ -422,11 +470,12 @@ k_pass_a(DP p, const SS* __restrict__ S, int nf, int init, const float4* __restr
   float accw = 0.f;
   walk(p, WP, lbW, pi.x, pi.y, pi.z, -1, q, [&](int j) {
     const float4 pj = WP[j], vj = WV[j];  // (x, y, z, p_w), v_w
+    const double2 xyj = WDxy[j];
+    sig += wendland64(p, xyi.x - xyj.x, xyi.y - xyj.y, d3 ? zi - WDz[j] : 0.0);
     const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
     const float r2 = dist2(dx, dy, dz);
     const float r = r2 > 0.f ? r2 * rsqrtf(r2) : 0.f;
     const float qq = r * p.hinv, t = fmaf(-0.5f, qq, 1.0f), t2 = t * t;
-    sig = fmaf(p.alpha * t2 * t2, fmaf(2.0f, qq, 1.0f), sig);
     const float Fg = p.gradc * t2 * t;
     const float rhow = fmaf(pj.w, p.inv_c2[phi], p.rho0[phi]);  // reading A5
     const float ZR = rhow * ci;
@@ -434,19 +483,22 @@ k_pass_a(DP p, const SS* __restrict__ S, int nf, int init, const float4* __restr
     const float num = fmaf(ZR, vd, (prsi - pj.w) * r);
     accw = fmaf(Fg, __fdividef(num, ZL + ZR), accw);
   });
-  sig = warp_sum(sig);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) sig += __shfl_xor_sync(FULL, sig, o);
   acc = warp_sum(acc);
   accw = warp_sum(accw);
   if (lane == 0) {
-    sig += p.w0;                                            // self term (reading A14)
+    // sigma_i / sigma0 - 1 in float64 (self term W(0) = alpha, reading A14), stored as float32:
+    // the density of Eq. 2.17 / 2.18 is rho0 (1 + dev), so the deviation carries the precision.
+    const float dev = (float)(p.a_over_s0 * (1.0 + sig) - 1.0);
     const float drho = 2.0f * rhoi * fmaf(p.V0, accw, acc);  // Eq. 2.9
     float d = pi.w;
     if (!init) {
       if ((p.fs_mask >> phi) & 1u) d = fmaf(S->dt, drho, d);          // Eq. 2.21
-      else d = p.rho0[phi] * fmaf(sig, p.inv_sigma0, -1.0f);          // Eq. 2.4 / 2.18
+      else d = p.rho0[phi] * dev;                                      // Eq. 2.4 / 2.18
     }
     Pout[i] = make_float4(pi.x, pi.y, pi.z, d);
-    SIG[i] = sig;
+    SIG[i] = dev;
     DRHO[i] = drho;
     IDout[i] = IDin[i];
   }
@@ -457,21 +509,23 @@ k_pass_a(DP p, const SS* __restrict__ S, int nf, int init, const float4* __restr
 template <bool MULTI>
 __global__ void __launch_bounds__(PW * 32)
 k_pass_b(DP p, const SS* __restrict__ S, int nf, const float4* __restrict__ P,
-         const float4* __restrict__ V, const int* __restrict__ lbF, const float4* __restrict__ WP,
-         const float4* __restrict__ WN, const int* __restrict__ lbW, float4* __restrict__ Vout,
+         const float4* __restrict__ V, const float4* __restrict__ LO, const int* __restrict__ lbF,
+         const float4* __restrict__ WP, const float4* __restrict__ WN, const int* __restrict__ lbW,
+         float4* __restrict__ Vout,
          float4* __restrict__ ACC) {
   __shared__ unsigned qs[PW][64];
   const int i = blockIdx.x * PW + (threadIdx.x >> 5);
   if (i >= nf) return;
   const int lane = threadIdx.x & 31;
   unsigned* q = qs[threadIdx.x >> 5];
-  const float4 pi = P[i], vi = V[i];
+  const float4 pi = P[i], vi = V[i], li = LO[i];
   const int phi = MULTI ? __float_as_int(vi.w) : 0;
   const float rhoi = p.rho0[phi] + pi.w, prsi = p.c2[phi] * pi.w, ZL = rhoi * p.c0[phi];
   float ax = 0.f, ay = 0.f, az = 0.f;
   walk(p, P, lbF, pi.x, pi.y, pi.z, i, q, [&](int j) {
-    const float4 pj = P[j], vj = V[j];
-    const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
+    const float4 pj = P[j], vj = V[j], lj = LO[j];
+    const float dx = (pi.x - pj.x) + (li.x - lj.x), dy = (pi.y - pj.y) + (li.y - lj.y),
+                dz = (pi.z - pj.z) + (li.z - lj.z);
     const float r2 = dist2(dx, dy, dz);
     const float rinv = r2 > 0.f ? rsqrtf(r2) : 0.f;
     const float qq = r2 * rinv * p.hinv, t = fmaf(-0.5f, qq, 1.0f);
@@ -490,7 +544,7 @@ k_pass_b(DP p, const SS* __restrict__ S, int nf, const float4* __restrict__ P,
   const bool pen = (p.pen_mask >> phi) & 1u;
   walk(p, WP, lbW, pi.x, pi.y, pi.z, -1, q, [&](int j) {
     const float4 pj = WP[j];
-    const float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
+    const float dx = (pi.x - pj.x) + li.x, dy = (pi.y - pj.y) + li.y, dz = (pi.z - pj.z) + li.z;
     const float r2 = dist2(dx, dy, dz);
     const float rinv = r2 > 0.f ? rsqrtf(r2) : 0.f;
     const float r = r2 * rinv;
@@ -579,8 +633,10 @@ k_dt(DP p, SS* __restrict__ S, int nf, const float4* __restrict__ V, const doubl
 // cell hash of the new position.
 __global__ void __launch_bounds__(256)
 k_predict(DP p, SS* __restrict__ S, int nf, const float4* __restrict__ P, const float4* __restrict__ V,
-          const float4* __restrict__ ACC, const float* __restrict__ SIG, float4* __restrict__ TP,
-          float4* __restrict__ TV, unsigned* __restrict__ keys, unsigned* __restrict__ vals) {
+          const float4* __restrict__ ACC, const float* __restrict__ SIG, const double2* __restrict__ Dxy,
+          const double* __restrict__ Dz, float4* __restrict__ TP, float4* __restrict__ TV,
+          double2* __restrict__ TDxy, double* __restrict__ TDz,
+          unsigned* __restrict__ keys, unsigned* __restrict__ vals) {
   const int i = blockIdx.x * 256 + threadIdx.x;
   if (i >= nf) return;
   float4 r = P[i], v = V[i];
@@ -588,16 +644,26 @@ k_predict(DP p, SS* __restrict__ S, int nf, const float4* __restrict__ P, const 
   const int ph = __float_as_int(v.w);
   if (p.flags & SPH_FLAG_REINIT) {
     const float rho0 = p.rho0[ph];
-    const float ds = rho0 * fmaf(SIG[i], p.inv_sigma0, -1.0f);  // rho0 sigma/sigma0 - rho0
+    const float ds = rho0 * SIG[i];  // rho0 sigma/sigma0 - rho0; SIG holds sigma/sigma0 - 1
     float d = ds;
-    if (((p.fs_mask >> ph) & 1u) && r.w > ds) d = fmaf(r.w - ds, __fdividef(rho0, rho0 + r.w), ds);
+    // Eq. 2.17 for rho* > rho_s: rho - rho0 = rho_s (rho* - rho0) / rho*  (same value as
+    // rho_s + (rho* - rho_s) rho0 / rho*, without the cancellation of two O(rho0) terms)
+    if (((p.fs_mask >> ph) & 1u) && r.w > ds) d = r.w * ((rho0 + ds) / (rho0 + r.w));
     r.w = d;
   }
-  const float dt = S->dt, hdt = 0.5f * dt;
+  const float hdt = 0.5f * S->dt;
   v.x = fmaf(hdt, a.x, v.x); v.y = fmaf(hdt, a.y, v.y); v.z = fmaf(hdt, a.z, v.z);
-  r.x = fmaf(dt, v.x, r.x); r.y = fmaf(dt, v.y, r.y); r.z = fmaf(dt, v.z, r.z);
+  // Eq. 2.20 on the float64 master position: r.xyz is its float32 rounding, which is
+  // what the cell hash and the neighbour test see (integer contract, reading A24).
+  double2 xy = Dxy[i];
+  double zd = Dz[i];
+  const double dtd = S->dt_d;
+  xy.x = fma(dtd, (double)v.x, xy.x); xy.y = fma(dtd, (double)v.y, xy.y); zd = fma(dtd, (double)v.z, zd);
+  r.x = (float)xy.x; r.y = (float)xy.y; r.z = (float)zd;
   TP[i] = r;
   TV[i] = v;
+  TDxy[i] = xy;
+  TDz[i] = zd;
   const bool fin = isfinite(r.x) && isfinite(r.y) && isfinite(r.z);
   if (!fin) atomicAdd(&S->nonfinite, 1ull);
   bool out = r.x < p.dmin[0] || r.x >= p.dmax[0] || r.y < p.dmin[1] || r.y >= p.dmax[1];
@@ -680,9 +746,9 @@ __global__ void k_get_wall(DP p, int nw, const float4* __restrict__ WP, const fl
 }
 
 __global__ void k_scatter_f(int n, const float* __restrict__ src, const unsigned* __restrict__ ID,
-                            float* dst) {
+                            float* dst, float scale, float shift) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < n) dst[ID[i]] = src[i];
+  if (i < n) dst[ID[i]] = scale * (src[i] + shift);
 }
 
 __global__ void k_scatter_n(int n, const float4* __restrict__ src, const unsigned* __restrict__ ID,
@@ -695,7 +761,8 @@ __global__ void k_scatter_n(int n, const float4* __restrict__ src, const unsigne
 }
 
 struct StatAcc {
-  double ek, mass;
+  double ek;
+  unsigned long long count[SPH_MAX_PHASES];  // fluid particles per phase (mass = sum count * m_phase, exact)
   unsigned long long pairs;
   unsigned xfront_bits;  // ordered encoding of float
 };
@@ -707,27 +774,31 @@ __device__ __forceinline__ unsigned f2ord(float f) {
 
 __global__ void __launch_bounds__(256)
 k_stats(DP p, int nf, const float4* __restrict__ P, const float4* __restrict__ V, StatAcc* out) {
-  double ek = 0, ms = 0;
+  double ek = 0;
+  unsigned cnt[SPH_MAX_PHASES] = {0, 0, 0, 0};
   float xf = -INFINITY;
   const int up = p.dim - 1;
   const float zlim = p.dmin[up] + 6.0f * p.dp;
   for (int i = blockIdx.x * 256 + threadIdx.x; i < nf; i += gridDim.x * 256) {
     const float4 r = P[i], v = V[i];
     const int ph = __float_as_int(v.w);
-    const double m = (double)p.mass[ph];
-    ek += 0.5 * m * ((double)v.x * v.x + (double)v.y * v.y + (double)v.z * v.z);
-    ms += m;
+    ek += 0.5 * p.massD[ph] * ((double)v.x * v.x + (double)v.y * v.y + (double)v.z * v.z);
+#pragma unroll
+    for (int k = 0; k < SPH_MAX_PHASES; ++k) cnt[k] += (ph == k);
     const float zz = up == 2 ? r.z : r.y;
     if (ph == 0 && zz < zlim) xf = fmaxf(xf, r.x);
   }
   for (int o = 16; o > 0; o >>= 1) {
     ek += __shfl_xor_sync(FULL, ek, o);
-    ms += __shfl_xor_sync(FULL, ms, o);
+#pragma unroll
+    for (int k = 0; k < SPH_MAX_PHASES; ++k) cnt[k] += __shfl_xor_sync(FULL, cnt[k], o);
     xf = fmaxf(xf, __shfl_xor_sync(FULL, xf, o));
   }
   if ((threadIdx.x & 31) == 0) {
     atomicAdd(&out->ek, ek);
-    atomicAdd(&out->mass, ms);
+#pragma unroll
+    for (int k = 0; k < SPH_MAX_PHASES; ++k)
+      if (cnt[k]) atomicAdd(&out->count[k], (unsigned long long)cnt[k]);
     atomicMax(&out->xfront_bits, f2ord(xf));
   }
 }
@@ -821,7 +892,9 @@ struct sph_ctx {
   int64_t launches = 0;
   // fluid
   float4 *P0 = nullptr, *V0 = nullptr, *P1 = nullptr, *V1 = nullptr, *TP = nullptr, *TV = nullptr,
-         *ACC = nullptr;
+         *ACC = nullptr, *LO = nullptr;
+  double2 *Dxy = nullptr, *TDxy = nullptr, *WDxy = nullptr;
+  double *Dz = nullptr, *TDz = nullptr, *WDz = nullptr;
   float *SIG = nullptr, *DRHO = nullptr;
   unsigned *ID0 = nullptr, *ID1 = nullptr;
   unsigned *keyA = nullptr, *valA = nullptr, *keyB = nullptr, *valB = nullptr, *hist = nullptr,
@@ -871,7 +944,7 @@ int dalloc(sph_ctx* c, T** p, size_t count) {
 
 void free_all(sph_ctx* c) {
   void* ptrs[] = {c->P0, c->V0, c->P1, c->V1, c->TP, c->TV, c->ACC, c->SIG, c->DRHO, c->ID0, c->ID1,
-                  c->keyA, c->valA, c->keyB, c->valB, c->hist, c->rowsum, c->lbF, c->lbW, c->WP,
+                  c->keyA, c->valA, c->keyB, c->valB, c->hist, c->rowsum, c->lbF, c->lbW, c->WP, c->LO, c->Dxy, c->TDxy, c->WDxy, c->Dz, c->TDz, c->WDz,
                   c->WV, c->WN, c->WID, c->S, c->dt_seq, c->stat};
   for (void* p : ptrs)
     if (p) cudaFree(p);
@@ -922,11 +995,11 @@ int launch_wall(sph_ctx* c, cudaStream_t st, bool with_vel, const float4* P, con
   if (c->nw == 0 || c->nf == 0) return SPH_OK;
   int grid = cdiv(c->nw, PW);
   if (c->multi) {
-    if (with_vel) LAUNCH((k_wall<true, true>), grid, PW * 32, st, c->dp, c->S, (int)c->nw, c->WP, c->WV, P, V, c->lbF);
-    else LAUNCH((k_wall<true, false>), grid, PW * 32, st, c->dp, c->S, (int)c->nw, c->WP, c->WV, P, V, c->lbF);
+    if (with_vel) LAUNCH((k_wall<true, true>), grid, PW * 32, st, c->dp, c->S, (int)c->nw, c->WP, c->WV, P, V, c->LO, c->lbF);
+    else LAUNCH((k_wall<true, false>), grid, PW * 32, st, c->dp, c->S, (int)c->nw, c->WP, c->WV, P, V, c->LO, c->lbF);
   } else {
-    if (with_vel) LAUNCH((k_wall<false, true>), grid, PW * 32, st, c->dp, c->S, (int)c->nw, c->WP, c->WV, P, V, c->lbF);
-    else LAUNCH((k_wall<false, false>), grid, PW * 32, st, c->dp, c->S, (int)c->nw, c->WP, c->WV, P, V, c->lbF);
+    if (with_vel) LAUNCH((k_wall<false, true>), grid, PW * 32, st, c->dp, c->S, (int)c->nw, c->WP, c->WV, P, V, c->LO, c->lbF);
+    else LAUNCH((k_wall<false, false>), grid, PW * 32, st, c->dp, c->S, (int)c->nw, c->WP, c->WV, P, V, c->LO, c->lbF);
   }
   return SPH_OK;
 }
@@ -938,28 +1011,29 @@ int pipeline_after_hash(sph_ctx* c, cudaStream_t st, int init, Prof& pf) {
   int rc = radix_sort(c, st, nf, c->keyA, c->valA, c->keyB, c->valB, &ks, &vs);
   if (rc) return rc;
   pf.mark();  // end sort
-  if (nf > 0) LAUNCH(k_reorder, cdiv(nf, 256), 256, st, nf, vs, c->TP, c->TV, c->ID0, c->P1, c->V1, c->ID1);
+  if (nf > 0) LAUNCH(k_reorder, cdiv(nf, 256), 256, st, nf, vs, c->TP, c->TV, c->TDxy, c->TDz, c->ID0, c->P1, c->V1,
+                     c->Dxy, c->Dz, c->LO, c->ID1);
   LAUNCH(k_cell_bounds, cdiv(nf + 1, 256), 256, st, ks, nf, (int)c->ncell, c->lbF);
   pf.mark();  // end reorder
   launch_wall(c, st, true, c->P1, c->V1);
   pf.mark();  // end wall 1
   if (nf > 0) {
     if (c->multi)
-      LAUNCH((k_pass_a<true>), cdiv(nf, PW), PW * 32, st, c->dp, c->S, nf, init, c->P1, c->V1, c->lbF, c->WP,
-             c->WV, c->lbW, c->P0, c->SIG, c->DRHO, c->ID1, c->ID0);
+      LAUNCH((k_pass_a<true>), cdiv(nf, PW), PW * 32, st, c->dp, c->S, nf, init, c->P1, c->V1, c->Dxy, c->Dz, c->lbF, c->WP,
+             c->WV, c->WDxy, c->WDz, c->lbW, c->P0, c->SIG, c->DRHO, c->ID1, c->ID0);
     else
-      LAUNCH((k_pass_a<false>), cdiv(nf, PW), PW * 32, st, c->dp, c->S, nf, init, c->P1, c->V1, c->lbF, c->WP,
-             c->WV, c->lbW, c->P0, c->SIG, c->DRHO, c->ID1, c->ID0);
+      LAUNCH((k_pass_a<false>), cdiv(nf, PW), PW * 32, st, c->dp, c->S, nf, init, c->P1, c->V1, c->Dxy, c->Dz, c->lbF, c->WP,
+             c->WV, c->WDxy, c->WDz, c->lbW, c->P0, c->SIG, c->DRHO, c->ID1, c->ID0);
   }
   pf.mark();  // end pass A
   launch_wall(c, st, false, c->P0, c->V1);
   pf.mark();  // end wall 2
   if (nf > 0) {
     if (c->multi)
-      LAUNCH((k_pass_b<true>), cdiv(nf, PW), PW * 32, st, c->dp, c->S, nf, c->P0, c->V1, c->lbF, c->WP, c->WN,
+      LAUNCH((k_pass_b<true>), cdiv(nf, PW), PW * 32, st, c->dp, c->S, nf, c->P0, c->V1, c->LO, c->lbF, c->WP, c->WN,
              c->lbW, c->V0, c->ACC);
     else
-      LAUNCH((k_pass_b<false>), cdiv(nf, PW), PW * 32, st, c->dp, c->S, nf, c->P0, c->V1, c->lbF, c->WP, c->WN,
+      LAUNCH((k_pass_b<false>), cdiv(nf, PW), PW * 32, st, c->dp, c->S, nf, c->P0, c->V1, c->LO, c->lbF, c->WP, c->WN,
              c->lbW, c->V0, c->ACC);
   }
   pf.mark();  // end pass B
@@ -986,7 +1060,7 @@ int do_steps(sph_ctx* c, int32_t n_steps, const double* dt_host, cudaStream_t st
     pf.mark();  // start
     LAUNCH(k_dt, dt_grid, 256, st, c->dp, c->S, nf, c->V0, dt_host ? c->dt_seq : nullptr, s);
     if (nf > 0)
-      LAUNCH(k_predict, cdiv(nf, 256), 256, st, c->dp, c->S, nf, c->P0, c->V0, c->ACC, c->SIG, c->TP, c->TV,
+      LAUNCH(k_predict, cdiv(nf, 256), 256, st, c->dp, c->S, nf, c->P0, c->V0, c->ACC, c->SIG, c->Dxy, c->Dz, c->TP, c->TV, c->TDxy, c->TDz,
              c->keyA, c->valA);
     pf.mark();  // end predict
     int rc = pipeline_after_hash(c, st, 0, pf);
@@ -1030,7 +1104,7 @@ int sph_create(const sph_params* prm, sph_ctx** out) {
     bool live = k < prm->n_phases;
     double r0 = live ? prm->rho0[k] : 1.0, c0 = live ? prm->c0[k] : 1.0;
     d.rho0[k] = (float)r0; d.c0[k] = (float)c0; d.c2[k] = (float)(c0 * c0);
-    d.inv_c2[k] = (float)(1.0 / (c0 * c0)); d.mass[k] = (float)(r0 * V0);
+    d.inv_c2[k] = (float)(1.0 / (c0 * c0)); d.mass[k] = (float)(r0 * V0); d.massD[k] = live ? r0 * V0 : 0.0;
     if (live) cmax = std::max(cmax, c0);
   }
   // sigma0: full undisturbed lattice incl. self term (readings A12, A14)
@@ -1047,6 +1121,7 @@ int sph_create(const sph_params* prm, sph_ctx** out) {
           }
         }
     d.sigma0 = (float)s; d.inv_sigma0 = (float)(1.0 / s);
+    d.sigma0D = s; d.a_over_s0 = alpha / s; d.hinvD = 1.0 / h;
   }
   d.gamma_p = (float)prm->penalty_strength; d.two_over_dp = (float)(2.0 / dp);
   d.pen_mask = prm->penalty_phase_mask; d.fs_mask = prm->free_surface_mask; d.flags = prm->flags;
@@ -1108,6 +1183,8 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
   int rc = 0;
   rc |= dalloc(c, &c->P0, nf); rc |= dalloc(c, &c->V0, nf); rc |= dalloc(c, &c->P1, nf);
   rc |= dalloc(c, &c->V1, nf); rc |= dalloc(c, &c->TP, cap); rc |= dalloc(c, &c->TV, nf);
+  rc |= dalloc(c, &c->LO, nf); rc |= dalloc(c, &c->Dxy, nf); rc |= dalloc(c, &c->TDxy, nf);
+  rc |= dalloc(c, &c->Dz, nf); rc |= dalloc(c, &c->TDz, nf); rc |= dalloc(c, &c->WDxy, nw); rc |= dalloc(c, &c->WDz, nw);
   rc |= dalloc(c, &c->ACC, nf); rc |= dalloc(c, &c->SIG, nf); rc |= dalloc(c, &c->DRHO, nf);
   rc |= dalloc(c, &c->ID0, cap); rc |= dalloc(c, &c->ID1, nf);
   rc |= dalloc(c, &c->keyA, cap); rc |= dalloc(c, &c->valA, cap); rc |= dalloc(c, &c->keyB, cap);
@@ -1135,8 +1212,10 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
     unsigned *ks, *vs;
     rc = radix_sort(c, st, nw, c->keyA, c->valA, c->keyB, c->valB, &ks, &vs);
     if (rc) { cudaFree(idx); return rc; }
-    LAUNCH(k_reorder, cdiv(nw, 256), 256, st, nw, vs, c->TP, (const float4*)nullptr, c->ID0, c->WP,
+    LAUNCH(k_reorder, cdiv(nw, 256), 256, st, nw, vs, c->TP, (const float4*)nullptr, (const double2*)nullptr,
+           (const double*)nullptr, c->ID0, c->WP, (float4*)nullptr, (double2*)nullptr, (double*)nullptr,
            (float4*)nullptr, c->WID);
+    LAUNCH(k_wall_double, cdiv(nw, 256), 256, st, nw, c->WP, c->WDxy, c->WDz);
     LAUNCH(k_cell_bounds, cdiv(nw + 1, 256), 256, st, ks, nw, (int)c->ncell, c->lbW);
     LAUNCH(k_normals, cdiv(nw, 128), 128, st, c->dp, nw, c->WP, c->lbW, c->WN);
   } else {
@@ -1146,7 +1225,7 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
   // ---- fluid: load, then the common pipeline in init mode (dt = 0: sigma_i, p_w, (dv/dt)^0) ----
   if (nf > 0) {
     CK(cudaMemcpyAsync(idx, fid.data(), sizeof(int) * nf, cudaMemcpyHostToDevice, st));
-    LAUNCH(k_load_fluid, cdiv(nf, 256), 256, st, c->dp, nf, idx, pos, vel, rho, tag, c->TP, c->TV, c->ID0,
+    LAUNCH(k_load_fluid, cdiv(nf, 256), 256, st, c->dp, nf, idx, pos, vel, rho, tag, c->TP, c->TV, c->TDxy, c->TDz, c->ID0,
            c->keyA, c->valA);
   }
   Prof pf(c, st);
@@ -1240,7 +1319,7 @@ int sph_get_stats(sph_ctx* c, sph_stats* out, void* stream) {
   if (!c->loaded) { c->err = "no particles"; return SPH_EINVAL; }
   cudaStream_t st = (cudaStream_t)stream;
   StatAcc z;
-  z.ek = 0; z.mass = 0; z.pairs = 0; z.xfront_bits = 0;
+  memset(&z, 0, sizeof(z));
   CK(cudaMemcpyAsync(c->stat, &z, sizeof(z), cudaMemcpyHostToDevice, st));
   const int nf = (int)c->nf;
   if (nf) {
@@ -1253,7 +1332,9 @@ int sph_get_stats(sph_ctx* c, sph_stats* out, void* stream) {
   CK(cudaMemcpyAsync(&hs, c->S, sizeof(hs), cudaMemcpyDeviceToHost, st));
   CK(cudaStreamSynchronize(st));
   out->t = hs.t; out->dt = hs.dt_d; out->steps = hs.steps; out->n_fluid = c->nf; out->n_wall = c->nw;
-  out->n_pairs = (int64_t)z.pairs; out->e_kin = z.ek; out->mass = z.mass;
+  out->n_pairs = (int64_t)z.pairs; out->e_kin = z.ek;
+  out->mass = 0.0;
+  for (int k = 0; k < SPH_MAX_PHASES; ++k) out->mass += (double)z.count[k] * c->dp.massD[k];
   {
     unsigned u = z.xfront_bits;
     float f;
@@ -1392,8 +1473,8 @@ int sph_debug_sigma(sph_ctx* c, float* sigma, void* stream) {
   CK(cudaMalloc((void**)&d, n * 8));
   CK(cudaMemsetAsync(d, 0, n * 8, st));
   if (c->nf) {
-    LAUNCH(k_scatter_f, cdiv(c->nf, 256), 256, st, (int)c->nf, c->SIG, c->ID0, d);
-    LAUNCH(k_scatter_f, cdiv(c->nf, 256), 256, st, (int)c->nf, c->DRHO, c->ID0, d + n);
+    LAUNCH(k_scatter_f, cdiv(c->nf, 256), 256, st, (int)c->nf, c->SIG, c->ID0, d, c->dp.sigma0, 1.0f);
+    LAUNCH(k_scatter_f, cdiv(c->nf, 256), 256, st, (int)c->nf, c->DRHO, c->ID0, d + n, 1.0f, 0.0f);
   }
   cudaError_t e = cudaMemcpyAsync(sigma, d, c->n * 4, cudaMemcpyDeviceToHost, st);
   if (e == cudaSuccess) e = cudaMemcpyAsync(sigma + c->n, d + n, c->n * 4, cudaMemcpyDeviceToHost, st);

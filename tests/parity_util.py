@@ -1,0 +1,56 @@
+"""Helpers shared by the GPU parity tests: run the same seeded float32 inputs through the
+CPU oracle (oracle/, double precision) and through libsph (CUDA, via the ctypes binding) and
+compare field by field with the error metric of DESIGN.md §3 (reading A26).
+
+No method arithmetic lives here."""
+import numpy as np
+
+from oracle import orc
+from paper_2110_02621_b200 import sph
+
+TOL = 1e-4   # BASELINE.json north_star: max relative error 1e-4 against the float32-rounded oracle
+G0 = 9.81
+
+
+def make_pair(cfg):
+    o = orc.Oracle(cfg)
+    o.set_particles(cfg["pos"], cfg["vel"], cfg["rho"], cfg["tag"])
+    g = sph.Sph(cfg)
+    g.set_particles(cfg["pos"], cfg["vel"], cfg["rho"], cfg["tag"])
+    return o, g
+
+
+def scales(cfg):
+    """Field scales S of reading A26: rho -> rho0 of the particle's phase, p -> rho0[0] |g| H,
+    a -> |g| (or 1 if g = 0), v -> sqrt(|g| H)."""
+    gm = float(np.linalg.norm(cfg["g"])) or 1.0
+    H = float(cfg.get("H", 1.0))
+    tag = cfg["tag"]
+    rho0 = np.asarray(cfg["rho0"], np.float64)
+    rs = np.where(tag >= 0, rho0[np.clip(tag, 0, None)], rho0[0])
+    return dict(rho=rs, p=rho0[0] * gm * H, acc=gm, vel=np.sqrt(gm * H), pos=H)
+
+
+def rel_err(cfg, name, x_gpu, x_ref, mask=None):
+    """max_i |x_gpu - f32(x_ref)| / max(|x_ref|, S)   (vector fields: Euclidean norms)."""
+    S = scales(cfg)[name]
+    ref = np.asarray(x_ref, np.float64).astype(np.float32).astype(np.float64)
+    got = np.asarray(x_gpu, np.float64)
+    if mask is None:
+        mask = np.ones(len(ref), bool)
+    if ref.ndim == 2:
+        d = np.linalg.norm(got - ref, axis=1)
+        m = np.linalg.norm(ref, axis=1)
+    else:
+        d = np.abs(got - ref)
+        m = np.abs(ref)
+    den = np.maximum(m, S)
+    e = (d / den)[mask]
+    return float(e.max()) if e.size else 0.0
+
+
+def compare_fields(cfg, o, g, names=("rho", "p", "acc"), fluid_only=True):
+    fo = o.fields()
+    fg = g.get_fields(device=False)
+    mask = cfg["tag"] >= 0 if fluid_only else None
+    return {k: rel_err(cfg, k, fg[k], fo[k], mask) for k in names}

@@ -1,0 +1,353 @@
+"""GPU parity tests: libsph (CUDA, through the C ABI) against the CPU oracle on the same
+seeded inputs.  Integer work bit-exact, floating point to 1e-4 (reading A26).
+
+Run on a B200 with `pytest -m gpu`.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import orc
+from paper_2110_02621_b200 import inputs, sph
+
+from parity_util import TOL, compare_fields, make_pair, rel_err
+
+pytestmark = pytest.mark.gpu
+
+
+def _cfgs_small():
+    return {
+        "cfg0": inputs.dam_break_2d(),
+        "cfg0_shuffled": inputs.shuffled(inputs.dam_break_2d(), seed=3),
+        "box2d_jitter": inputs.shuffled(inputs.box_2d(n=37, jitter=0.3, seed=11), seed=5),
+        "box2d_two_phase": inputs.box_2d(n=30, jitter=0.1, seed=2, two_phase=True),
+        "box3d_13": inputs.box_sweep_3d(n=13),
+        "box3d_20_shuffled": inputs.shuffled(inputs.box_sweep_3d(n=20), seed=9),
+    }
+
+
+SMALL = _cfgs_small()
+
+
+# ------------------------------------------------------------------------- integer contract
+@pytest.mark.parametrize("name", list(SMALL))
+def test_cells_permutation_ranges_bit_exact(name):
+    cfg = SMALL[name]
+    g = sph.Sph(cfg)
+    g.set_particles(cfg["pos"], cfg["vel"], cfg["rho"], cfg["tag"])
+    cid, perm, cs, ce = g.debug_cells()
+    rcid, rperm, rcs, rce = orc.f32_cells(cfg, cfg["pos"], cfg["tag"])
+    assert g.num_cells() * 2 == len(rcs)
+    assert np.array_equal(cid, rcid)
+    assert np.array_equal(perm, rperm)
+    assert np.array_equal(cs, rcs) and np.array_equal(ce, rce)
+
+
+@pytest.mark.parametrize("name", list(SMALL))
+def test_neighbour_lists_bit_exact(name):
+    cfg = SMALL[name]
+    g = sph.Sph(cfg)
+    g.set_particles(cfg["pos"], cfg["vel"], cfg["rho"], cfg["tag"])
+    off, ids = g.debug_neighbours()
+    roff, rids = orc.f32_neighbours(cfg, cfg["pos"], cfg["tag"], grid=False)   # brute force
+    assert np.array_equal(off, roff)
+    assert np.array_equal(ids, rids)
+    fluid = cfg["tag"] >= 0
+    assert g.get_stats()["npairs"] == int((roff[1:] - roff[:-1])[fluid].sum())
+
+
+def test_neighbour_lists_after_steps_snapshot():
+    """Snapshot check (reading A25): take the GPU positions after 25 steps, feed them to the
+    oracle's float32 rule, compare lists and cell ids at those positions."""
+    cfg = inputs.dam_break_2d()
+    g = sph.Sph(cfg)
+    g.set_particles(cfg["pos"], cfg["vel"], cfg["rho"], cfg["tag"])
+    g.step(25)
+    pos = g.get_fields(device=False, which=("pos",))["pos"]
+    off, ids = g.debug_neighbours()
+    roff, rids = orc.f32_neighbours(cfg, pos, cfg["tag"], grid=False)
+    assert np.array_equal(off, roff) and np.array_equal(ids, rids)
+    cid, perm, cs, ce = g.debug_cells()
+    rcid, _, _, _ = orc.f32_cells(cfg, pos, cfg["tag"])
+    assert np.array_equal(cid, rcid)
+    # after steps the permutation is no longer unique (the sort starts from the previous order):
+    # check validity: a permutation, sorted by cell inside each class
+    n, nf = len(cid), cfg["n_fluid"]
+    assert sorted(perm.tolist()) == list(range(n))
+    assert np.all(np.diff(cid[perm[:nf]]) >= 0) and np.all(np.diff(cid[perm[nf:]]) >= 0)
+    assert np.all(cfg["tag"][perm[:nf]] >= 0) and np.all(cfg["tag"][perm[nf:]] < 0)
+
+
+# ------------------------------------------------------------------------- set-up fields
+@pytest.mark.parametrize("name", list(SMALL))
+def test_setup_sigma_normals_wall_state_acc0(name):
+    cfg = SMALL[name]
+    o, g = make_pair(cfg)
+    fo = o.fields()
+    fluid = cfg["tag"] >= 0
+    wall = ~fluid
+    sig, _ = g.debug_sigma()
+    s0 = orc.sigma0(cfg["dim"], cfg["h"], cfg["dp"])
+    assert np.max(np.abs(sig[fluid] - fo["sigma"][fluid])) < 2e-6 * s0
+    nrm = g.debug_normals()
+    assert np.max(np.abs(nrm - o.normals())) < 2e-6
+    assert np.array_equal(np.any(nrm != 0, axis=1), np.any(o.normals() != 0, axis=1))
+    e = compare_fields(cfg, o, g, names=("rho", "p", "acc", "vel", "pos"), fluid_only=False)
+    assert e["pos"] == 0.0 and e["rho"] < 1e-6
+    assert e["p"] < TOL and e["acc"] < TOL and e["vel"] < TOL, e
+    fg = g.get_fields(device=False)
+    assert np.all(fg["acc"][wall] == 0)
+
+
+# ------------------------------------------------------------------------- time stepping
+@pytest.mark.parametrize("name", list(SMALL))
+def test_fields_after_1_and_10_steps_same_dt(name):
+    """BASELINE.json north_star: density, pressure, acceleration after 1 and after 10 steps to
+    max relative error 1e-4 against the float32-rounded oracle; both sides driven by the
+    oracle's dt sequence (sph_step_dt) so that only the kernels' arithmetic differs."""
+    cfg = SMALL[name]
+    o, g = make_pair(cfg)
+    dts = o.step(1)
+    g.step(1, dts=dts)
+    e1 = compare_fields(cfg, o, g, names=("rho", "p", "acc", "vel", "pos"))
+    assert max(e1.values()) < TOL, ("1 step", e1)
+    dts = o.step(9)
+    g.step(9, dts=dts)
+    e10 = compare_fields(cfg, o, g, names=("rho", "p", "acc", "vel", "pos"))
+    assert max(e10.values()) < TOL, ("10 steps", e10)
+    _, drho = g.debug_sigma()
+    fo = o.fields()
+    fl = cfg["tag"] >= 0
+    sc = np.abs(fo["drho"][fl]).max() + 1e-30
+    assert np.max(np.abs(drho[fl] - fo["drho"][fl])) < 5e-4 * sc
+
+
+@pytest.mark.parametrize("name", ["cfg0", "box3d_13", "box2d_two_phase"])
+def test_device_dt_matches_oracle(name):
+    """sph_step computes dt on the device (Eq. 2.23-2.24, warp-shuffle max reduction)."""
+    cfg = SMALL[name]
+    o, g = make_pair(cfg)
+    dts = o.step(10)
+    g.step(10)
+    s = g.get_stats()
+    assert s["steps"] == 10
+    assert abs(s["dt"] - dts[-1]) < 2e-6 * dts[-1]
+    assert abs(s["t"] - dts.sum()) < 2e-6 * dts.sum()
+    e = compare_fields(cfg, o, g)
+    assert max(e.values()) < 3 * TOL, e   # dt itself differs in the 7th digit
+
+
+def test_moving_start_two_phase_unequal_c():
+    """Reading A3: per-phase speed of sound (config 2b), with an initial velocity field so the
+    Riemann dissipation term beta is active."""
+    cfg = inputs.box_2d(n=32, jitter=0.2, seed=4, two_phase=True)
+    cfg["c0"] = [cfg["c0"][0], cfg["c0"][0] * math.sqrt(1000.0)]
+    rng = np.random.Generator(np.random.PCG64(77))
+    v = rng.uniform(-0.3, 0.3, cfg["pos"].shape).astype(np.float32)
+    v[:, 2] = 0
+    cfg["vel"] = v
+    o, g = make_pair(cfg)
+    e0 = compare_fields(cfg, o, g)
+    assert max(e0.values()) < TOL, e0
+    dts = o.step(10)
+    g.step(10, dts=dts)
+    e = compare_fields(cfg, o, g, names=("rho", "p", "acc", "vel"))
+    assert max(e.values()) < TOL, e
+
+
+def test_oscillating_gravity_3d():
+    """Config 3's g(t) = g + amp sin(2 pi t / T) (reading A28)."""
+    cfg = inputs.box_sweep_3d(n=12)
+    cfg["g_osc_amp"] = [0.3 * 9.81, 0.0, 0.0]
+    cfg["g_osc_period"] = 0.01
+    o, g = make_pair(cfg)
+    dts = o.step(10)
+    g.step(10, dts=dts)
+    e = compare_fields(cfg, o, g, names=("rho", "p", "acc", "vel"))
+    assert max(e.values()) < TOL, e
+
+
+def test_penalty_active_near_wall():
+    """Fluid particles pushed to within dp/2 of the wall layer so F_p (Eq. 2.13) is non-zero."""
+    cfg = inputs.box_2d(n=24, jitter=0.0)
+    pos = cfg["pos"].copy()
+    nf = cfg["n_fluid"]
+    low = np.where(pos[:nf, 1] < cfg["dp"])[0]
+    pos[low, 1] -= np.float32(0.8 * cfg["dp"])      # 0.5 dp -> -0.3 dp: 0.2 dp from the wall layer
+    cfg["pos"] = pos
+    o, g = make_pair(cfg)
+    fo = o.fields()
+    assert np.abs(fo["acc"][low, 1]).max() > 50.0   # the penalty dominates there
+    e = compare_fields(cfg, o, g)
+    assert max(e.values()) < TOL, e
+    cfg2 = dict(cfg)
+    cfg2["penalty_phase_mask"] = 0
+    o2, g2 = make_pair(cfg2)
+    assert np.abs(o2.fields()["acc"][low, 1] - fo["acc"][low, 1]).max() > 1.0
+    e = compare_fields(cfg2, o2, g2)
+    assert max(e.values()) < TOL, e
+
+
+def test_flags_reinit_off_and_wall_velocity_zero():
+    cfg = inputs.box_2d(n=20, jitter=0.2, seed=8)
+    cfg["flags"] = 0
+    rng = np.random.Generator(np.random.PCG64(5))
+    v = rng.uniform(-0.2, 0.2, cfg["pos"].shape).astype(np.float32)
+    v[:, 2] = 0
+    cfg["vel"] = v
+    o, g = make_pair(cfg)
+    dts = o.step(5)
+    g.step(5, dts=dts)
+    e = compare_fields(cfg, o, g, names=("rho", "p", "acc", "vel"))
+    assert max(e.values()) < TOL, e
+    fg = g.get_fields(device=False)
+    assert np.all(fg["vel"][cfg["tag"] < 0] == 0)
+
+
+# ------------------------------------------------------------------------- long runs
+def test_cfg0_200_steps_integral_quantities():
+    """BASELINE.json config 0: 200 steps; total mass exact, x_front and E_k within 1 %."""
+    cfg = inputs.dam_break_2d()
+    o, g = make_pair(cfg)
+    m0 = g.get_stats()["mass"]
+    o.step(200)
+    g.step(200)
+    so, sg = o.stats(), g.get_stats()
+    assert sg["mass"] == m0                                   # conserved exactly
+    assert abs(sg["mass"] - so["mass"]) <= 1e-12 * so["mass"] and abs(m0 - 2000.0) < 1e-9
+    assert sg["escaped"] == 0 and sg["nonfinite"] == 0
+    assert abs(sg["t"] - so["t"]) < 1e-5 * so["t"]
+    assert abs(sg["ek"] - so["ek"]) < 0.01 * so["ek"]
+    assert abs(sg["x_front"] - so["x_front"]) < 0.01 * so["x_front"]
+    e = compare_fields(cfg, o, g, names=("pos", "vel", "rho"))
+    assert e["pos"] < 1e-3 and e["vel"] < 2e-2, e
+
+
+def test_cfg0_long_run_front_and_energy():
+    cfg = inputs.dam_break_2d()
+    o, g = make_pair(cfg)
+    m0 = g.get_stats()["mass"]
+    o.step(1500)
+    g.step(1500)
+    so, sg = o.stats(), g.get_stats()
+    assert sg["mass"] == m0 and abs(m0 - so["mass"]) <= 1e-12 * so["mass"]
+    assert sg["escaped"] == 0
+    assert abs(sg["ek"] - so["ek"]) < 0.01 * so["ek"]
+    assert abs(sg["x_front"] - so["x_front"]) < 0.01 * so["x_front"]
+
+
+# ------------------------------------------------------------------------- edge cases
+def test_edge_empty_and_single_class():
+    cfg = inputs.box_2d(n=10)
+    z3, z1, zi = np.zeros((0, 3), np.float32), np.zeros(0, np.float32), np.zeros(0, np.int32)
+    g = sph.Sph(cfg)
+    g.set_particles(z3, z3, z1, zi)
+    g.step(2)
+    s = g.get_stats()
+    assert s["n_fluid"] == 0 and s["n_wall"] == 0 and s["npairs"] == 0
+    # fluid only (no wall): a free-falling blob; walls only: nothing moves
+    fl = cfg["tag"] >= 0
+    for mask in (fl, ~fl):
+        sub = dict(cfg)
+        for k in ("pos", "vel", "rho", "tag"):
+            sub[k] = np.ascontiguousarray(cfg[k][mask])
+        o, g = make_pair(sub)
+        dts = o.step(3)
+        g.step(3, dts=dts)
+        e = compare_fields(sub, o, g, names=("rho", "p", "acc", "vel", "pos"), fluid_only=False)
+        assert max(e.values()) < TOL, e
+
+
+def test_edge_single_particle_free_fall():
+    cfg = inputs.box_2d(n=10)
+    cfg["pos"] = np.array([[0.05, 0.05, 0.0]], np.float32)
+    cfg["vel"] = np.array([[0.1, 0.2, 0.0]], np.float32)
+    cfg["rho"] = np.array([1000.0], np.float32)
+    cfg["tag"] = np.array([0], np.int32)
+    cfg["flags"] = 0
+    g = sph.Sph(cfg)
+    g.set_particles(cfg["pos"], cfg["vel"], cfg["rho"], cfg["tag"])
+    dts = np.full(20, 1e-4)
+    g.step(20, dts=dts)
+    f = g.get_fields(device=False)
+    t = 20e-4
+    assert abs(f["pos"][0, 1] - (0.05 + 0.2 * t - 0.5 * 9.81 * t * t)) < 1e-6
+    assert abs(f["vel"][0, 1] - (0.2 - 9.81 * t)) < 1e-5
+    assert f["acc"][0, 1] == pytest.approx(-9.81, rel=1e-6)
+
+
+def test_edge_escaped_particles_are_counted_and_binned():
+    cfg = inputs.box_2d(n=12, jitter=0.1)
+    pos = cfg["pos"].copy()
+    pos[0] = [-1.0, 0.02, 0.0]     # outside the grid box: clamped into an edge cell
+    pos[1] = [5.0, 7.0, 0.0]
+    cfg["pos"] = pos
+    g = sph.Sph(cfg)
+    g.set_particles(cfg["pos"], cfg["vel"], cfg["rho"], cfg["tag"])
+    cid, perm, cs, ce = g.debug_cells()
+    rcid, rperm, rcs, rce = orc.f32_cells(cfg, cfg["pos"], cfg["tag"])
+    assert np.array_equal(cid, rcid) and np.array_equal(perm, rperm)
+    off, ids = g.debug_neighbours()
+    roff, rids = orc.f32_neighbours(cfg, cfg["pos"], cfg["tag"], grid=True)
+    assert np.array_equal(off, roff) and np.array_equal(ids, rids)
+    g.step(1)
+    assert g.get_stats()["escaped"] == 2
+
+
+def test_edge_bad_arguments_fail_loudly():
+    cfg = inputs.box_2d(n=6)
+    bad = dict(cfg)
+    bad["dim"] = 4
+    with pytest.raises(sph.SphError):
+        sph.Sph(bad)
+    g = sph.Sph(cfg)
+    with pytest.raises(sph.SphError):
+        g.step(1)                   # before sph_set_particles
+    tag = cfg["tag"].copy()
+    tag[0] = 3                      # phase id out of range
+    with pytest.raises(sph.SphError):
+        g.set_particles(cfg["pos"], cfg["vel"], cfg["rho"], tag)
+
+
+def test_device_pointer_entry_and_restart():
+    """sph_set_particles / sph_get_fields with device pointers (torch tensors), and a restart
+    from a checkpoint: get_fields -> set_particles reproduces the state (reading A18)."""
+    import torch
+    cfg = inputs.box_2d(n=16, jitter=0.2, seed=3)
+    dev = {k: torch.from_numpy(cfg[k]).cuda() for k in ("pos", "vel", "rho", "tag")}
+    g = sph.Sph(cfg)
+    g.set_particles(dev["pos"], dev["vel"], dev["rho"], dev["tag"])
+    o = orc.Oracle(cfg)
+    o.set_particles(cfg["pos"], cfg["vel"], cfg["rho"], cfg["tag"])
+    dts = o.step(4)
+    g.step(4, dts=dts)
+    fd = g.get_fields(device=True)
+    torch.cuda.synchronize()
+    fh = g.get_fields(device=False)
+    for k in fd:
+        assert np.array_equal(fd[k].cpu().numpy(), fh[k])
+    fo = o.fields()
+    assert rel_err(cfg, "acc", fh["acc"], fo["acc"], cfg["tag"] >= 0) < TOL
+    # restart: the float32 checkpoint loaded into a new context and into a new oracle
+    g2 = sph.Sph(cfg)
+    g2.set_particles(fd["pos"], fd["vel"], fd["rho"], dev["tag"])
+    f2 = g2.get_fields(device=False)
+    fl = cfg["tag"] >= 0
+    assert np.array_equal(f2["pos"], fh["pos"]) and np.array_equal(f2["vel"][fl], fh["vel"][fl])
+    o2 = orc.Oracle(cfg)
+    o2.set_particles(fh["pos"], np.where(fl[:, None], fh["vel"], 0), fh["rho"], cfg["tag"])
+    for k in ("rho", "p", "acc"):
+        assert rel_err(cfg, k, f2[k], o2.fields()[k], fl) < TOL, k
+
+
+def test_stage_timings_and_launch_count():
+    cfg = inputs.box_sweep_3d(n=16)
+    g = sph.Sph(cfg)
+    g.set_particles(cfg["pos"], cfg["vel"], cfg["rho"], cfg["tag"])
+    l0 = g.launch_count()
+    g.set_profiling(True)
+    g.step(3)
+    ms, ns = g.get_timings()
+    assert ns == 3 and all(v > 0 for v in ms.values())
+    assert g.launch_count() > l0
