@@ -1,0 +1,400 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the whole SPH hot path on B200.
+
+Contract (driver): `python bench.py --gpus N --steps K --warmup W` prints ONE JSON line on rank 0.
+
+  step      one sph_step(1): dt reduction, reinit, kick, drift, cell hash, radix sort, reorder,
+            wall extrapolation x2, pair pass A, pair pass B (+ second kick) on one synthetic config
+  workload  BASELINE.json configs[1] (3-D dam break with box obstacle, ~0.68 M fluid + ~0.47 M wall)
+            unless --config says otherwise; inputs are seeded/synthetic (paper_2110_02621_b200.inputs)
+  value     fluid particle-steps/s with the state resident in HBM (CUDA events on the launching
+            stream; L2 flushed between timed steps; max over ranks)
+  e2e       same metric through the HOST-pointer C-ABI calls: sph_set_particles_host + K x
+            (sph_step(1) + sph_get_stats) + sph_get_fields_host, all inside the timed region
+  roofline  the dominant kernel (largest stage time) against the FP32 ALU peak
+  cpu_baseline  the CPU oracle (oracle/, as it stands) on the host cores, bounded sample
+
+N > 1: replicas only: every rank runs the same configuration independently, no
+data-path collective; value = particle-steps of all ranks / max-over-ranks time; scaling "weak".
+
+`--impl reference` times the CPU oracle instead (rank 0 only) and prints the same line shape.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "particle-steps/s"
+UNIT = "fluid particle-steps/s"
+
+# Algorithmic FP32 operation counts per neighbour hit (fma = 2), DESIGN.md §7.  They are the
+# paper's equations counted once, independent of the cell scheme; candidate tests are reported
+# separately (CAND_FLOPS each) because they are overhead of the 27-cell walk, not of the method.
+FLOPS_HIT = {"pass_a": 40.0, "pass_b": 50.0, "wall": 30.0}
+CAND_FLOPS = 8.0
+FP32_LANES_PER_SM = 128
+N_SM = 148
+
+
+def make_config_name(name):
+    return {"cfg0": "cfg0_dam_break_2d", "cfg1": "cfg1_dam_break_3d_box", "cfg1_small": "cfg1_dam_break_3d_box",
+            "cfg2a": "cfg2a_two_phase_2d", "cfg2b": "cfg2b_two_phase_2d", "cfg3": "cfg3_sloshing_spheres_3d",
+            "cfg3_4m": "cfg3_sloshing_spheres_3d"}.get(name, name)
+
+
+def make_config(name):
+    from paper_2110_02621_b200 import inputs
+    if name == "cfg0":
+        return inputs.dam_break_2d()
+    if name == "cfg1":
+        return inputs.dam_break_3d_box()
+    if name == "cfg1_small":
+        return inputs.dam_break_3d_box(dp=0.02)
+    if name == "cfg2a":
+        return inputs.two_phase_2d(equal_c=True)
+    if name == "cfg2b":
+        return inputs.two_phase_2d(equal_c=False)
+    if name == "cfg3":
+        return inputs.sloshing_spheres_3d()
+    if name == "cfg3_4m":
+        return inputs.sloshing_spheres_3d(dp=0.00585)
+    if name.startswith("cfg4_"):
+        return inputs.box_sweep_3d(n=int(name.split("_")[1]))
+    raise SystemExit("unknown --config %r" % name)
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs
+    (the recipe's clocks line, /opt/skills/guides/B200_PROFILING.md)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+    NAMES = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.rows = []
+        self.proc = None
+        self.idx = gpu_index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.idx), "--query-gpu=" + self.Q,
+                 "--format=csv,noheader,nounits", "-lms", "200"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=[], samples=0)
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, smax, pw, reasons = [], [], [], set()
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 8:
+                continue
+            try:
+                sm.append(float(f[1])); smax.append(float(f[2])); pw.append(float(f[3]))
+            except ValueError:
+                continue
+            for k, name in enumerate(self.NAMES):
+                if f[4 + k].lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=[], samples=0)
+        return dict(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(smax)),
+                    power_w_max=float(max(pw)), reasons=sorted(reasons), samples=len(sm))
+
+
+def stencil_candidates(cfg, g):
+    """Number of (fluid i, candidate j) distance tests the 27/9-cell walk performs at the current
+    positions, from the library's own cell ranges (host-side integer bookkeeping for the report:
+    sum over cells of n_f(c) * sum_{c' in stencil(c)} (n_f(c') + n_w(c')))."""
+    _, _, cs, ce = g.debug_cells()
+    nc = g.num_cells()
+    cnt = (ce - cs).astype(np.int64)
+    nf, nw = cnt[:nc], cnt[nc:]
+    edge = 2.0 * cfg["h"] * (1.0 + 1.0 / 1024.0)
+    dims = [max(1, int(np.ceil((cfg["domain_max"][k] - cfg["domain_min"][k]) / edge)))
+            for k in range(cfg["dim"])]
+    while len(dims) < 3:
+        dims.append(1)
+    nx, ny, nz = dims
+    assert nx * ny * nz == nc, (dims, nc)
+    tot = (nf + nw).reshape(nz, ny, nx)
+    wallc = nw.reshape(nz, ny, nx)
+
+    def box(a):
+        for ax in range(3):
+            if a.shape[ax] == 1:
+                continue
+            p = np.zeros_like(a)
+            sl = [slice(None)] * 3
+            p += a
+            s1, s2 = list(sl), list(sl)
+            s1[ax] = slice(1, None); s2[ax] = slice(None, -1)
+            p[tuple(s1)] += a[tuple(s2)]
+            p[tuple(s2)] += a[tuple(s1)]
+            a = p
+        return a
+
+    f3 = nf.reshape(nz, ny, nx)
+    cand_fluid_rows = int((f3 * box(tot)).sum())          # tests issued by the fluid pair passes
+    cand_wall_rows = int((wallc * box(f3)).sum())         # tests issued by the wall extrapolation
+    return cand_fluid_rows, cand_wall_rows
+
+
+def oracle_rate(cfg, steps, warmup=0):
+    """Time `steps` oracle steps (after `warmup`) on the host cores; returns
+    (fluid particle-steps/s, seconds, threads)."""
+    from oracle import orc
+    o = orc.Oracle(cfg)
+    o.set_particles(cfg["pos"], cfg["vel"], cfg["rho"], cfg["tag"])
+    if warmup:
+        o.step(warmup)
+    t0 = time.perf_counter()
+    o.step(steps)
+    dt = time.perf_counter() - t0
+    return cfg["n_fluid"] * steps / dt, dt, os.cpu_count() or 1
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle as it stands (this tier's reference arm), rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    full = (args.steps + args.warmup) <= 30 and args.config == "cfg1"
+    name = args.config if full else ("cfg1_small" if args.config == "cfg1" else args.config)
+    cfg = make_config(name)
+    rate, secs, cores = oracle_rate(cfg, args.steps, args.warmup)
+    sample = "%s (%d fluid + %d wall particles), %d steps after %d warm-up" % (
+        cfg["name"] + ("" if full or name == args.config else " at dp=0.02"), cfg["n_fluid"],
+        cfg["n_wall"], args.steps, args.warmup)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * secs / max(args.steps, 1),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": {"workload": make_config_name(args.config), "sample": sample},
+        "cpu_baseline": {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": rate, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def run_gpu(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2110_02621_b200 import sph
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: libsph has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    cfg = make_config(args.config)
+    nfl, nwl = cfg["n_fluid"], cfg["n_wall"]
+    K, W = args.steps, max(args.warmup, 0)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")  # > 126 MB L2
+
+    # ---- device-resident run ------------------------------------------------------------------
+    dev = {k: torch.from_numpy(cfg[k]).cuda() for k in ("pos", "vel", "rho", "tag")}
+    g = sph.Sph(cfg)
+    g.set_particles(dev["pos"], dev["vel"], dev["rho"], dev["tag"])
+    for _ in range(W):
+        flush.zero_()
+        g.step(1)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+    sampler = ClockSampler(local)
+    barrier()
+    sampler.start()
+    l0 = g.launch_count()
+    for k in range(K):
+        flush.zero_()              # L2 flush between timed iterations (outside the event pair)
+        ev[k][0].record()
+        g.step(1)
+        ev[k][1].record()
+    barrier()
+    launches = g.launch_count() - l0
+    clocks = sampler.stop()
+    ms = float(sum(a.elapsed_time(b) for a, b in ev))
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    st = g.get_stats()
+    if st["escaped"] or st["nonfinite"]:
+        raise SystemExit("bench run went bad: %r" % (st,))
+    value = world * nfl * K / (ms * 1e-3)
+    pairs_s = world * st["npairs"] * K / (ms * 1e-3)
+
+    # ---- per-stage times (CUDA events recorded by the library on the same stream) ---------------
+    g.set_profiling(True)
+    KP = min(K, 32)
+    for _ in range(KP):
+        flush.zero_()
+        g.step(1)
+    stage_ms, ns = g.get_timings()
+    g.set_profiling(False)
+    stage_ms = {k: v / max(ns, 1) for k, v in stage_ms.items()}
+    st = g.get_stats()
+    cand_f, cand_w = stencil_candidates(cfg, g)
+    off, _ = _neighbour_counts(g)
+    tag = cfg["tag"]
+    wall_pairs = int((off[1:] - off[:-1])[tag < 0].sum())
+    fluid_pairs = int(st["npairs"])
+    sm_max = clocks.get("sm_max_mhz") or 1965.0
+    peak = N_SM * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12       # TFLOP/s at max SM clock
+    kern = {}
+    for name, hits, cands, per_step in (("pass_a", fluid_pairs, cand_f, 1), ("pass_b", fluid_pairs, cand_f, 1),
+                                        ("wall", wall_pairs, cand_w, 2)):
+        t = stage_ms[name] * 1e-3 / per_step
+        if t <= 0:
+            continue
+        fl = FLOPS_HIT[name] * hits
+        kern[name] = {"ms": 1e3 * t, "hits": hits, "candidates": cands,
+                      "tflops_hit_only": fl / t / 1e12, "frac_hit_only": fl / t / 1e12 / peak,
+                      "tflops_with_candidates": (fl + CAND_FLOPS * cands) / t / 1e12,
+                      "frac_with_candidates": (fl + CAND_FLOPS * cands) / t / 1e12 / peak}
+    # HBM-bound stages: algorithmic bytes per fluid particle
+    hbm = _peaks().get("hbm_gbs", 6650.0)
+    bytes_pp = {"predict": 148.0, "sort": 16.0 * 2 * g_sort_passes(g), "reorder": 156.0}
+    for name, b in bytes_pp.items():
+        t = stage_ms[name] * 1e-3
+        if t > 0:
+            kern[name] = {"ms": 1e3 * t, "gbs": b * nfl / t / 1e9, "frac_hbm": b * nfl / t / 1e9 / hbm}
+    dom = max(("pass_a", "pass_b"), key=lambda k: stage_ms[k])
+    roofline = {"bound": "alu", "kernel": "k_" + dom, "achieved": kern[dom]["tflops_hit_only"],
+                "peak": peak, "unit": "TFLOP/s", "frac": kern[dom]["frac_hit_only"], "traffic": None,
+                "peak_source": "148 SM x 128 FP32 lanes x 2 x clocks.max.sm (DESIGN.md §7), not measured",
+                "achieved_with_candidates": kern[dom]["tflops_with_candidates"],
+                "frac_with_candidates": kern[dom]["frac_with_candidates"],
+                "flops_per_hit": FLOPS_HIT[dom], "flops_per_candidate": CAND_FLOPS}
+    g.close()
+
+    # ---- end to end through the HOST-pointer entry points ----------------------------------------
+    n = len(cfg["tag"])
+    pin = {k: torch.from_numpy(cfg[k]).pin_memory() for k in ("pos", "vel", "rho", "tag")}
+    out = {k: torch.empty(s, dtype=torch.float32).pin_memory() for k, s in
+           (("pos", (n, 3)), ("vel", (n, 3)), ("rho", (n,)))}
+    g2 = sph.Sph(cfg)
+    KE = K
+    g2.set_particles(pin["pos"].numpy(), pin["vel"].numpy(), pin["rho"].numpy(), pin["tag"].numpy())
+    g2.step(1)  # warm the allocator / module load outside the timed region
+    barrier()
+    t0 = time.perf_counter()
+    g2.set_particles(pin["pos"].numpy(), pin["vel"].numpy(), pin["rho"].numpy(), pin["tag"].numpy())
+    for _ in range(KE):
+        g2.step(1)
+        s2 = g2.get_stats()      # device -> host read of the step's result (t, dt, E_k, mass, pairs)
+    g2.get_fields_into_host(pos=out["pos"].numpy(), vel=out["vel"].numpy(), rho=out["rho"].numpy())
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    if world > 1:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    h2d = (n * (12 + 12 + 4 + 4)) / KE
+    d2h = (n * 4 + n * (12 + 12 + 4)) / KE + 88      # tag read-back + fields, + sph_stats per step
+    e2e = {"value": world * nfl * KE / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d,
+           "d2h_bytes_per_step": d2h,
+           "region": "sph_set_particles_host + %d x (sph_step(1) + sph_get_stats) + sph_get_fields_host" % KE}
+    g2.close()
+
+    # ---- CPU oracle on the host cores (rank 0, N = 1 only) -----------------------------------------
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        osteps = args.cpu_steps
+        rate, secs, cores = oracle_rate(cfg, osteps)
+        cpu = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": "%s full size (%d fluid + %d wall), %d steps, %.1f s" % (cfg["name"], nfl, nwl, osteps, secs)}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": cfg["name"], "n_fluid": nfl, "n_wall": nwl, "dim": cfg["dim"],
+                       "dp": cfg["dp"], "l2": "flushed between timed steps (256 MiB write)",
+                       "parallelism": "replicas only" if world > 1 else "1 gpu"},
+            "pair_interactions_per_s": pairs_s, "pairs_per_step": fluid_pairs,
+            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
+            "roofline": roofline, "kernels": kern, "stage_ms_per_step": stage_ms,
+            "cpu_baseline": cpu,
+        }
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def _neighbour_counts(g):
+    import ctypes as C
+    off = np.zeros(g.n + 1, np.int64)
+    tot = C.c_int64(0)
+    g._ck(g.L.sph_debug_neighbours(g.ctx, off.ctypes.data_as(C.c_void_p), None, 0, C.byref(tot), g._st()))
+    return off, tot.value
+
+
+def g_sort_passes(g):
+    bits = 1
+    while (1 << bits) < g.num_cells():
+        bits += 1
+    return (bits + 7) // 8
+
+
+def _peaks():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return json.load(f)
+    except Exception:
+        return {}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="cfg1")
+    ap.add_argument("--cpu-steps", type=int, default=5, help="oracle steps of the cpu_baseline leg")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_gpu(args)
+
+
+if __name__ == "__main__":
+    main()
