@@ -1,0 +1,219 @@
+// sph_aux.cuh — loading, time step, predictor, reorder, wall normals and near-wall flags.
+// Included by sph.cu only.  Citations: PAPER.md:<line>; readings Axx: DESIGN.md §3.
+#pragma once
+#include "sph_common.cuh"
+
+constexpr unsigned RES_MID = (512u << 22) | (512u << 12) | (512u << 2);  // zero residual on every axis
+
+// ------------------------------------------------------------------------------------------
+// Loading (sph_set_particles): split caller arrays into the fluid / wall structures.
+// ------------------------------------------------------------------------------------------
+__global__ void k_load(DP p, int n, int is_wall, const int* __restrict__ idx, const float* __restrict__ pos,
+                       const float* __restrict__ vel, const float* __restrict__ rho,
+                       const int* __restrict__ tag, uint4* __restrict__ TX, float4* __restrict__ TB,
+                       unsigned* __restrict__ ID, unsigned* __restrict__ keys, unsigned* __restrict__ vals) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int o = idx[i];
+  const int ph = is_wall ? 0 : tag[o];
+  uint4 x;
+  x.x = fx_from_double((double)pos[3 * o], p.O[0], p.Q);
+  x.y = fx_from_double((double)pos[3 * o + 1], p.O[1], p.Q);
+  x.z = p.dim == 3 ? fx_from_double((double)pos[3 * o + 2], p.O[2], p.Q) : 0u;
+  x.w = RES_MID | (unsigned)ph;
+  TX[i] = x;
+  if (is_wall) {
+    TB[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+  } else {
+    const float drho = (float)((double)rho[o] - (double)p.rho0[ph]);
+    TB[i] = make_float4(vel[3 * o], vel[3 * o + 1], p.dim == 3 ? vel[3 * o + 2] : 0.0f, drho);
+  }
+  ID[i] = (unsigned)o;
+  keys[i] = cell_key(p, fx_image(x.x, p.O[0], p.Q), fx_image(x.y, p.O[1], p.Q),
+                     p.dim == 3 ? fx_image(x.z, p.O[2], p.Q) : 0.0f);
+  vals[i] = (unsigned)i;
+}
+
+// Gather into cell-sorted order and derive the centred float32 image used by the candidate filter.
+__global__ void __launch_bounds__(256)
+k_reorder(DP p, int n, const unsigned* __restrict__ vals, const uint4* __restrict__ TX,
+          const float4* __restrict__ TB, const unsigned* __restrict__ IDin, uint4* __restrict__ X,
+          float4* __restrict__ B, float4* __restrict__ A, unsigned* __restrict__ IDout) {
+  const int s = blockIdx.x * 256 + threadIdx.x;
+  if (s >= n) return;
+  const unsigned v = vals[s];
+  const uint4 x = TX[v];
+  X[s] = x;
+  B[s] = TB[v];
+  A[s] = centred_image(p, x);
+  IDout[s] = IDin[v];
+}
+
+// ------------------------------------------------------------------------------------------
+// Time step, Eq. 2.23-2.24 (reading A17): grid-stride max |v|^2 with warp
+// shuffles, one atomicMax per block; the last block to finish computes dt and g(t^{n+1}).
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_dt(DP p, SS* __restrict__ S, int nf, const float4* __restrict__ B, const double* __restrict__ dt_seq,
+     int seq_idx) {
+  __shared__ float sm[8];
+  float m = 0.f;
+  for (int i = blockIdx.x * 256 + threadIdx.x; i < nf; i += gridDim.x * 256) {
+    const float4 v = B[i];
+    m = fmaxf(m, fmaf(v.z, v.z, fmaf(v.y, v.y, v.x * v.x)));
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) m = fmaxf(m, __shfl_xor_sync(FULL, m, o));
+  if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = m;
+  __syncthreads();
+  if (threadIdx.x != 0) return;
+  for (int w = 1; w < 8; ++w) m = fmaxf(m, sm[w]);
+  if (!(m == m) || isinf(m)) { atomicAdd(&S->nonfinite, 1ull); m = 0.f; }
+  atomicMax(&S->vmax2_bits, __float_as_uint(m));
+  __threadfence();
+  const unsigned done = atomicAdd(&S->blocks_done, 1u);
+  if (done != gridDim.x - 1) return;
+  __threadfence();
+  const double vmax = sqrt((double)__uint_as_float(atomicMax(&S->vmax2_bits, 0u)));
+  double g[3];
+  auto grav = [&](double t) {
+    const double s = p.gperiod > 0.0 ? sin(6.283185307179586476925286766559 * t / p.gperiod) : 0.0;
+    for (int k = 0; k < 3; ++k) g[k] = p.g[k] + p.gamp[k] * s;
+  };
+  double dt;
+  if (dt_seq) {
+    dt = dt_seq[seq_idx];
+  } else {
+    dt = p.cfl * p.hD / (p.cmax + vmax);  // Eq. 2.23
+    grav(S->t);
+    const double gn = sqrt(g[0] * g[0] + g[1] * g[1] + g[2] * g[2]);
+    if (gn > 0.0) dt = fmin(dt, p.cfl * sqrt(p.hD / gn));  // Eq. 2.24
+    if (!(dt > 1e-12)) S->dt_underflow = 1;
+  }
+  grav(S->t + dt);
+  S->g[0] = (float)g[0]; S->g[1] = (float)g[1]; S->g[2] = (float)g[2];
+  S->dt_d = dt;
+  S->dt = (float)dt;
+  S->t += dt;
+  S->steps += 1;
+  S->vmax2_bits = 0u;
+  S->blocks_done = 0u;
+  S->escaped = 0ull;
+}
+
+// One axis of the drift Eq. 2.20 on the fixed-point master position: (X, residual) is a 42-bit
+// integer in units of Q/1024; the displacement dt*v is rounded to that unit.
+__device__ __forceinline__ unsigned drift_axis(unsigned X, unsigned& res, double disp_sub) {
+  long long tot = ((long long)X << 10) + ((long long)res - 512) + __double2ll_rn(disp_sub);
+  long long Xn = (tot + 512) >> 10;
+  long long rn = tot - (Xn << 10) + 512;
+  if (Xn < 0) { Xn = 0; rn = 512; }
+  if (Xn > 4294967295ll) { Xn = 4294967295ll; rn = 512; }
+  res = (unsigned)rn;
+  return (unsigned)Xn;
+}
+
+// Predictor: density reinitialisation Eq. 2.17 / 2.18 from the sigma_i of the last pass A
+// (same positions, reading A13), first half kick Eq. 2.19, drift Eq. 2.20,
+// cell hash of the new position.  In place on (v, rho) ; the new position goes to TX.
+__global__ void __launch_bounds__(256)
+k_predict(DP p, SS* __restrict__ S, int nf, const uint4* __restrict__ X, float4* __restrict__ B,
+          const float4* __restrict__ ACC, const float* __restrict__ SIG, uint4* __restrict__ TX,
+          unsigned* __restrict__ keys, unsigned* __restrict__ vals) {
+  const int i = blockIdx.x * 256 + threadIdx.x;
+  if (i >= nf) return;
+  uint4 x = X[i];
+  float4 b = B[i];
+  const float4 a = ACC[i];
+  const int ph = phase_of(x);
+  if (p.flags & SPH_FLAG_REINIT) {
+    const float rho0 = p.rho0[ph];
+    const float ds = rho0 * SIG[i];  // rho0 sigma/sigma0 - rho0; SIG holds sigma/sigma0 - 1
+    float d = ds;
+    // Eq. 2.17 for rho* > rho_s: rho - rho0 = rho_s (rho* - rho0) / rho*  (same value as
+    // rho_s + (rho* - rho_s) rho0 / rho*, without the cancellation of two O(rho0) terms)
+    if (((p.fs_mask >> ph) & 1u) && b.w > ds) d = b.w * ((rho0 + ds) / (rho0 + b.w));
+    b.w = d;
+  }
+  const float hdt = 0.5f * S->dt;
+  b.x = fmaf(hdt, a.x, b.x); b.y = fmaf(hdt, a.y, b.y); b.z = fmaf(hdt, a.z, b.z);  // Eq. 2.19
+  const bool fin = isfinite(b.x) && isfinite(b.y) && isfinite(b.z);
+  if (fin) {
+    const double k = S->dt_d * p.sub_per_m;
+    unsigned rx = (x.w >> 22) & 1023u, ry = (x.w >> 12) & 1023u, rz = (x.w >> 2) & 1023u;
+    x.x = drift_axis(x.x, rx, k * (double)b.x);
+    x.y = drift_axis(x.y, ry, k * (double)b.y);
+    if (p.dim == 3) x.z = drift_axis(x.z, rz, k * (double)b.z);
+    x.w = (rx << 22) | (ry << 12) | (rz << 2) | (unsigned)ph;
+  } else {
+    atomicAdd(&S->nonfinite, 1ull);
+  }
+  TX[i] = x;
+  B[i] = b;
+  const float gx = fx_image(x.x, p.O[0], p.Q), gy = fx_image(x.y, p.O[1], p.Q);
+  const float gz = p.dim == 3 ? fx_image(x.z, p.O[2], p.Q) : 0.0f;
+  bool out = gx < p.dmin[0] || gx >= p.dmax[0] || gy < p.dmin[1] || gy >= p.dmax[1];
+  if (p.dim == 3) out = out || gz < p.dmin[2] || gz >= p.dmax[2];
+  if (out || !fin) atomicAdd(&S->escaped, 1ull);
+  keys[i] = cell_key(p, gx, gy, gz);
+  vals[i] = (unsigned)i;
+}
+
+// Wall normals, Eq. 2.16, once, in float64 (reading A10).
+template <int DIM>
+__global__ void k_normals(DP p, int nw, const uint4* __restrict__ WX, const unsigned* __restrict__ WK,
+                          const int* __restrict__ lbW, float4* __restrict__ WN) {
+  const int w = blockIdx.x * blockDim.x + threadIdx.x;
+  if (w >= nw) return;
+  const uint4 xi = WX[w];
+  const unsigned key = WK[w];
+  const unsigned row = key / (unsigned)p.nx;
+  const int cx = (int)(key - row * (unsigned)p.nx), cz = (int)(row / (unsigned)p.ny),
+            cy = (int)(row - (unsigned)cz * (unsigned)p.ny);
+  const double h = p.hD, rc2 = 4.0 * h * h;
+  const double PI = 3.14159265358979323846264338327950288;
+  const double alpha = DIM == 2 ? 7.0 / (4.0 * PI * h * h) : 21.0 / (16.0 * PI * h * h * h);
+  const double dpd = p.dpD;
+  const double V0 = DIM == 2 ? dpd * dpd : dpd * dpd * dpd;
+  double px = 0, py = 0, pz = 0;
+  for (int dz = (DIM == 3 ? -1 : 0); dz <= (DIM == 3 ? 1 : 0); ++dz)
+    for (int dy = -1; dy <= 1; ++dy) {
+      const int y = cy + dy, z = cz + dz;
+      if (y < 0 || y >= p.ny || z < 0 || z >= p.nz) continue;
+      const int rb = (z * p.ny + y) * p.nx;
+      const int s = lbW[rb + max(cx - 1, 0)], e = lbW[rb + min(cx + 1, p.nx - 1) + 1];
+      for (int j = s; j < e; ++j) {
+        if (j == w) continue;
+        const uint4 xj = WX[j];
+        const double dx = p.Q * (double)(int)(xi.x - xj.x), dyy = p.Q * (double)(int)(xi.y - xj.y),
+                     dzz = DIM == 3 ? p.Q * (double)(int)(xi.z - xj.z) : 0.0;
+        const double r2 = dx * dx + dyy * dyy + dzz * dzz;
+        if (!(r2 < rc2) || r2 == 0.0) continue;
+        const double r = sqrt(r2), q = r / h, t = 1.0 - 0.5 * q;
+        const double dw = -5.0 * alpha / h * q * t * t * t;
+        const double f = -V0 * dw / r;  // -(m_j/rho_j) grad_i W_ij = f * r_ij
+        px += f * dx; py += f * dyy; pz += f * dzz;
+      }
+    }
+  const double nrm = sqrt(px * px + py * py + pz * pz);
+  float4 n = make_float4(0.f, 0.f, 0.f, 0.f);
+  if (nrm * h >= 1e-3) n = make_float4((float)(px / nrm), (float)(py / nrm), (float)(pz / nrm), 0.f);
+  WN[w] = n;
+}
+
+// wnear[c] = 1 if any wall particle lies in the 27 / 9-cell stencil of cell c (static, set-up):
+// lets the fluid pair kernels skip the wall walk for warps in the bulk.
+__global__ void k_wnear(DP p, int ncell, const int* __restrict__ lbW, unsigned char* __restrict__ wnear) {
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= ncell) return;
+  const int row = c / p.nx, cx = c - row * p.nx, cz = row / p.ny, cy = row - cz * p.ny;
+  int any = 0;
+  for (int dz = (p.dim == 3 ? -1 : 0); dz <= (p.dim == 3 ? 1 : 0); ++dz)
+    for (int dy = -1; dy <= 1; ++dy) {
+      const int y = cy + dy, z = cz + dz;
+      if (y < 0 || y >= p.ny || z < 0 || z >= p.nz) continue;
+      const int rb = (z * p.ny + y) * p.nx;
+      any |= lbW[rb + min(cx + 1, p.nx - 1) + 1] > lbW[rb + max(cx - 1, 0)];
+    }
+  wnear[c] = (unsigned char)any;
+}

@@ -1,0 +1,99 @@
+// sph_common.cuh — parameter blocks and device helpers shared by the kernels of libsph.
+// Included by sph.cu only.  Citations: PAPER.md:<line>; readings Axx: DESIGN.md §3.
+//
+// Data layout.  Fluid and wall particles live in separate cell-sorted arrays:
+//   X4  uint4   fixed-point master position (X, Y, Z) in units of Q = 2^-k m from the origin O,
+//               .w = residual of each axis in units of Q/1024 (3 x 10 bits, biased by 512) << 2 | phase
+//   A4  float4  float32 image centred on the domain centre (xc, yc, zc, |xc|^2): candidate test only
+//   B4  float4  (vx, vy, vz, rho - rho0_phase); walls: (v_w, p_w)
+// Pair geometry is an exact integer subtraction of X4 followed by int->float, in units of Q.
+#pragma once
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+
+#include "sph.h"
+
+struct DP {
+  int dim, n_phases;
+  float rc2;       // (2h)^2, contract neighbour test on float32 images (reading A24)
+  float rc2m;      // candidate filter threshold on the centred images: rc2 + rounding margin
+  int exact_filter;  // 1: margin too large for the expanded form, use the difference form
+  float qh;        // Q / h: q = r_Q * qh
+  float Qf;        // Q
+  float gradcQ;    // W'(r)/r * r_ij = gradcQ * (1 - q/2)^3 * d_Q,   gradc = -5 alpha / h^2
+  float alpha, V0;
+  float rho0[SPH_MAX_PHASES], c0[SPH_MAX_PHASES], c2[SPH_MAX_PHASES], inv_c2[SPH_MAX_PHASES],
+      mass[SPH_MAX_PHASES];
+  float gamma_p, two_over_dp;  // two_over_dp holds 2 Q / dp (delta of Eq. 2.15 from Q units)
+  unsigned pen_mask, fs_mask, flags;
+  float ox, oy, oz, inv_edge;  // contract cell hash (reading A24)
+  int nx, ny, nz;
+  float dmin[3], dmax[3];
+  double O[3], C[3], Q, sub_per_m;  // fixed point: origin, image centre, quantum, 1024 / Q
+  double cmax, cfl, hD, dpD;
+  double massD[SPH_MAX_PHASES];
+  double a_over_s0;
+  double g[3], gamp[3], gperiod;
+};
+
+// Device-resident per-step state: written by k_dt, read by every other kernel, so that
+// sph_step(n) needs no host synchronisation between steps.
+struct SS {
+  double t;
+  double dt_d;
+  float dt;
+  float g[3];            // gravity at t^{n+1} (reading A28)
+  unsigned vmax2_bits;   // max |v|^2 over fluid, float bits (non-negative -> ordered as uint)
+  unsigned blocks_done;
+  long long steps;
+  unsigned long long escaped, nonfinite;
+  int dt_underflow;
+};
+
+#define FULL 0xffffffffu
+
+__device__ __forceinline__ int cell_coord(float x, float o, float inv, int n) {
+  // Integer contract (reading A24): one FP32 subtract, one FP32 multiply, no contraction.
+  float u = __fmul_rn(__fsub_rn(x, o), inv);
+  u = fminf(fmaxf(floorf(u), 0.0f), (float)(n - 1));  // NaN -> 0
+  return (int)u;
+}
+
+__device__ __forceinline__ float dist2(float dx, float dy, float dz) {
+  // reading A24: r2 = fmaf(dz,dz,fmaf(dy,dy,dx*dx)); in 2-D dz = 0 adds exactly 0.
+  return fmaf(dz, dz, fmaf(dy, dy, __fmul_rn(dx, dx)));
+}
+
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(FULL, v, o);
+  return v;
+}
+
+// ---- fixed-point master positions ---------------------------------------------------------
+__device__ __forceinline__ unsigned fx_from_double(double x, double O, double Q) {
+  double u = rint((x - O) / Q);
+  u = fmin(fmax(u, 0.0), 4294967295.0);  // saturate (escaped particles); NaN -> 0
+  return (unsigned)u;
+}
+__device__ __forceinline__ double fx_to_double(unsigned X, double O, double Q) {
+  return fma((double)X, Q, O);  // exact: Q is a power of two, O a multiple of Q
+}
+// float32 image of the master position (what sph_get_fields returns and the cell hash sees)
+__device__ __forceinline__ float fx_image(unsigned X, double O, double Q) { return (float)fx_to_double(X, O, Q); }
+
+__device__ __forceinline__ int phase_of(const uint4& x) { return (int)(x.w & 3u); }
+
+__device__ __forceinline__ float4 centred_image(const DP& p, const uint4& x) {
+  const float a = (float)(fx_to_double(x.x, p.O[0], p.Q) - p.C[0]);
+  const float b = (float)(fx_to_double(x.y, p.O[1], p.Q) - p.C[1]);
+  const float c = p.dim == 3 ? (float)(fx_to_double(x.z, p.O[2], p.Q) - p.C[2]) : 0.0f;
+  return make_float4(a, b, c, fmaf(c, c, fmaf(b, b, a * a)));
+}
+
+__device__ __forceinline__ unsigned cell_key(const DP& p, float x, float y, float z) {
+  const int cx = cell_coord(x, p.ox, p.inv_edge, p.nx), cy = cell_coord(y, p.oy, p.inv_edge, p.ny);
+  const int cz = p.dim == 3 ? cell_coord(z, p.oz, p.inv_edge, p.nz) : 0;
+  return (unsigned)((cz * p.ny + cy) * p.nx + cx);
+}

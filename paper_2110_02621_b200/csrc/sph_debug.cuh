@@ -1,0 +1,232 @@
+// sph_debug.cuh — output, integral quantities and the integer-contract debug paths (not on the
+// hot path).  Included by sph.cu only.  The contract (reading A24) is defined on the float32
+// image of the master position: these kernels work on image arrays G = (xg, yg, zg, 0).
+#pragma once
+#include "sph_common.cuh"
+
+__global__ void k_image(DP p, int n, const uint4* __restrict__ X, float4* __restrict__ G) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const uint4 x = X[i];
+  G[i] = make_float4(fx_image(x.x, p.O[0], p.Q), fx_image(x.y, p.O[1], p.Q),
+                     p.dim == 3 ? fx_image(x.z, p.O[2], p.Q) : 0.0f, 0.0f);
+}
+
+// ------------------------------------------------------------------------------------------
+// Contract-exact stencil walk (debug paths): one warp per particle, lanes over the candidates of each x-row of the
+// 27 (3-D) / 9 (2-D) cell stencil (coalesced float4 loads), hits compacted through a
+// per-warp shared-memory queue so that the expensive pair body runs with full warps.
+// ------------------------------------------------------------------------------------------
+template <typename Body>
+__device__ __forceinline__ void walk(const DP& p, const float4* __restrict__ P, const int* __restrict__ lb,
+                                     float xi, float yi, float zi, int self, unsigned* q, Body&& body) {
+  const int lane = threadIdx.x & 31;
+  const unsigned lt = (1u << lane) - 1u;
+  const int cx = cell_coord(xi, p.ox, p.inv_edge, p.nx), cy = cell_coord(yi, p.oy, p.inv_edge, p.ny);
+  const int cz = p.dim == 3 ? cell_coord(zi, p.oz, p.inv_edge, p.nz) : 0;
+  const int nrow = p.dim == 3 ? 9 : 3;
+  int rs = 0, re = 0;
+  if (lane < nrow) {
+    int y = cy + (lane % 3) - 1, z = cz + (lane / 3) - 1;
+    if (p.dim != 3) z = 0;
+    if (y >= 0 && y < p.ny && z >= 0 && z < p.nz) {
+      int rb = (z * p.ny + y) * p.nx;
+      rs = lb[rb + max(cx - 1, 0)];
+      re = lb[rb + min(cx + 1, p.nx - 1) + 1];
+    }
+  }
+  int qn = 0, qh = 0;
+  for (int r = 0; r < nrow; ++r) {
+    const int s = __shfl_sync(FULL, rs, r), e = __shfl_sync(FULL, re, r);
+    for (int j0 = s; j0 < e; j0 += 32) {
+      const int j = j0 + lane;
+      bool hit = false;
+      if (j < e) {
+        float4 pj = P[j];
+        float r2 = dist2(xi - pj.x, yi - pj.y, zi - pj.z);
+        hit = (r2 < p.rc2) && (j != self);
+      }
+      const unsigned m = __ballot_sync(FULL, hit);
+      if (m) {
+        if (hit) q[(qh + qn + __popc(m & lt)) & 63] = (unsigned)j;
+        qn += __popc(m);
+        __syncwarp();
+        if (qn >= 32) {
+          body((int)q[(qh + lane) & 63]);
+          qh = (qh + 32) & 63;
+          qn -= 32;
+          __syncwarp();
+        }
+      }
+    }
+  }
+  if (qn > 0) {
+    __syncwarp();
+    if (lane < qn) body((int)q[(qh + lane) & 63]);
+  }
+  __syncwarp();
+}
+
+constexpr int PW = 8;  // warps per block in k_neigh
+
+
+// ------------------------------------------------------------------------------------------
+// Output
+// ------------------------------------------------------------------------------------------
+__global__ void k_get(DP p, int n, int is_wall, const uint4* __restrict__ X, const float4* __restrict__ B,
+                      const float4* __restrict__ ACC, const unsigned* __restrict__ ID, float* pos,
+                      float* vel, float* rho, float* prs, float* acc) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const uint4 x = X[i];
+  const float4 b = B[i];
+  const size_t o = ID[i];
+  if (pos) {
+    pos[3 * o] = fx_image(x.x, p.O[0], p.Q);
+    pos[3 * o + 1] = fx_image(x.y, p.O[1], p.Q);
+    pos[3 * o + 2] = p.dim == 3 ? fx_image(x.z, p.O[2], p.Q) : 0.0f;
+  }
+  if (vel) { vel[3 * o] = b.x; vel[3 * o + 1] = b.y; vel[3 * o + 2] = b.z; }
+  if (is_wall) {  // B = (v_w, p_w)
+    if (acc) { acc[3 * o] = 0.f; acc[3 * o + 1] = 0.f; acc[3 * o + 2] = 0.f; }
+    if (rho) rho[o] = fmaf(b.w, p.inv_c2[0], p.rho0[0]);
+    if (prs) prs[o] = b.w;
+  } else {
+    const int ph = phase_of(x);
+    if (acc) { const float4 a = ACC[i]; acc[3 * o] = a.x; acc[3 * o + 1] = a.y; acc[3 * o + 2] = a.z; }
+    if (rho) rho[o] = p.rho0[ph] + b.w;
+    if (prs) prs[o] = p.c2[ph] * b.w;
+  }
+}
+
+__global__ void k_scatter_f(int n, const float* __restrict__ src, const unsigned* __restrict__ ID,
+                            float* dst, float scale, float shift) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) dst[ID[i]] = scale * (src[i] + shift);
+}
+
+__global__ void k_scatter_n(int n, const float4* __restrict__ src, const unsigned* __restrict__ ID,
+                            float* dst) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const float4 v = src[i];
+  const size_t o = ID[i];
+  dst[3 * o] = v.x; dst[3 * o + 1] = v.y; dst[3 * o + 2] = v.z;
+}
+
+struct StatAcc {
+  double ek;
+  unsigned long long count[SPH_MAX_PHASES];  // fluid particles per phase (mass = sum count * m_phase, exact)
+  unsigned long long pairs;
+  unsigned xfront_bits;  // ordered encoding of float
+};
+
+__device__ __forceinline__ unsigned f2ord(float f) {
+  unsigned u = __float_as_uint(f);
+  return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+
+__global__ void __launch_bounds__(256)
+k_stats(DP p, int nf, const uint4* __restrict__ X, const float4* __restrict__ B, StatAcc* out) {
+  double ek = 0;
+  unsigned cnt[SPH_MAX_PHASES] = {0, 0, 0, 0};
+  float xf = -INFINITY;
+  const int up = p.dim - 1;
+  const float zlim = p.dmin[up] + 6.0f * (float)p.dpD;
+  for (int i = blockIdx.x * 256 + threadIdx.x; i < nf; i += gridDim.x * 256) {
+    const uint4 x = X[i];
+    const float4 v = B[i];
+    const int ph = phase_of(x);
+    ek += 0.5 * p.massD[ph] * ((double)v.x * v.x + (double)v.y * v.y + (double)v.z * v.z);
+#pragma unroll
+    for (int k = 0; k < SPH_MAX_PHASES; ++k) cnt[k] += (ph == k);
+    const float zz = up == 2 ? fx_image(x.z, p.O[2], p.Q) : fx_image(x.y, p.O[1], p.Q);
+    if (ph == 0 && zz < zlim) xf = fmaxf(xf, fx_image(x.x, p.O[0], p.Q));
+  }
+  for (int o = 16; o > 0; o >>= 1) {
+    ek += __shfl_xor_sync(FULL, ek, o);
+#pragma unroll
+    for (int k = 0; k < SPH_MAX_PHASES; ++k) cnt[k] += __shfl_xor_sync(FULL, cnt[k], o);
+    xf = fmaxf(xf, __shfl_xor_sync(FULL, xf, o));
+  }
+  if ((threadIdx.x & 31) == 0) {
+    atomicAdd(&out->ek, ek);
+#pragma unroll
+    for (int k = 0; k < SPH_MAX_PHASES; ++k)
+      if (cnt[k]) atomicAdd(&out->count[k], (unsigned long long)cnt[k]);
+    atomicMax(&out->xfront_bits, f2ord(xf));
+  }
+}
+// Hit counting / listing for sph_get_stats (n_pairs) and sph_debug_neighbours.
+// mode 0: count into cnt[caller id] (and total pairs); mode 1: fill ids at off[caller id].
+__global__ void __launch_bounds__(PW * 32)
+k_neigh(DP p, int n, int is_wall, int mode, const float4* __restrict__ Pself, const unsigned* __restrict__ IDself,
+        const float4* __restrict__ P, const unsigned* __restrict__ ID, const int* __restrict__ lbF,
+        const float4* __restrict__ WP, const unsigned* __restrict__ WID, const int* __restrict__ lbW,
+        int* __restrict__ cnt, const long long* __restrict__ off, int* __restrict__ ids, long long cap,
+        unsigned long long* total) {
+  __shared__ unsigned qs[PW][64];
+  const int i = blockIdx.x * PW + (threadIdx.x >> 5);
+  if (i >= n) return;
+  const int lane = threadIdx.x & 31;
+  unsigned* q = qs[threadIdx.x >> 5];
+  const float4 pi = Pself[i];
+  const unsigned me = IDself[i];
+  const long long base = mode ? off[me] : 0;
+  // the body runs with full warps except in the tail; tot is re-broadcast from lane 0 after
+  int tot = 0;
+  walk(p, P, lbF, pi.x, pi.y, pi.z, is_wall ? -1 : i, q, [&](int j) {
+    unsigned act = __activemask();
+    int k = __popc(act & ((1u << lane) - 1u));
+    if (mode && base + tot + k < cap) ids[base + tot + k] = (int)ID[j];
+    tot += __popc(act);
+  });
+  tot = __shfl_sync(FULL, tot, 0);
+  if (!is_wall) {
+    walk(p, WP, lbW, pi.x, pi.y, pi.z, -1, q, [&](int j) {
+      unsigned act = __activemask();
+      int k = __popc(act & ((1u << lane) - 1u));
+      if (mode && base + tot + k < cap) ids[base + tot + k] = (int)WID[j];
+      tot += __popc(act);
+    });
+    tot = __shfl_sync(FULL, tot, 0);
+  }
+  __syncwarp();
+  if (lane == 0) {
+    if (!mode) {
+      if (cnt) cnt[me] = tot;
+      if (total) atomicAdd(total, (unsigned long long)tot);
+    } else {
+      // ascending caller ids within the row (insertion sort; debug path, rows of ~20-100)
+      long long m = tot;
+      if (base + m > cap) m = cap > base ? cap - base : 0;
+      __threadfence_block();
+      for (long long a = 1; a < m; ++a) {
+        int x = ids[base + a];
+        long long b = a - 1;
+        while (b >= 0 && ids[base + b] > x) { ids[base + b + 1] = ids[base + b]; --b; }
+        ids[base + b + 1] = x;
+      }
+    }
+  }
+}
+
+__global__ void k_dbg_cells(DP p, int n, const float4* __restrict__ P, const unsigned* __restrict__ ID,
+                            int* cell_id, int* perm, int perm_base) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const float4 r = P[i];
+  const int cx = cell_coord(r.x, p.ox, p.inv_edge, p.nx), cy = cell_coord(r.y, p.oy, p.inv_edge, p.ny);
+  const int cz = p.dim == 3 ? cell_coord(r.z, p.oz, p.inv_edge, p.nz) : 0;
+  if (cell_id) cell_id[ID[i]] = (cz * p.ny + cy) * p.nx + cx;
+  if (perm) perm[perm_base + i] = (int)ID[i];
+}
+
+__global__ void k_dbg_ranges(int ncell, const int* __restrict__ lb, int* cs, int* ce) {
+  int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= ncell) return;
+  int s = lb[c], e = lb[c + 1];
+  if (s == e) s = e = 0;
+  cs[c] = s;
+  ce[c] = e;
+}

@@ -1,0 +1,317 @@
+// sph_pair.cuh — the neighbour walk and the three pair kernels (wall extrapolation, pass A, pass B).
+// Included by sph.cu only.  DESIGN.md §5 describes the scheme:
+//   one thread per particle i (cell-sorted order, so a warp covers ~2 cells);
+//   phase 1  each lane walks the 9 (3-D) / 3 (2-D) x-rows of its own 27 / 9-cell stencil, every
+//            row one contiguous index range; the candidate float4 (centred image, |x|^2) is the
+//            same address for all lanes of a cell (one L1 wavefront per cell present in the warp);
+//            filter r^2 = |xj|^2 - 2 xi.xj + |xi|^2 < rc^2 + margin: 3 FFMA + 1 FSETP;
+//            survivors are appended to the lane's private shared-memory queue q[k][tid];
+//   phase 2  when any lane's queue is nearly full (and at the end) every lane drains its own queue:
+//            exact geometry from the fixed-point positions (integer subtract + I2F), then the
+//            pair physics.  Filter false positives (margin) have r >= 2h and add exactly zero.
+#pragma once
+#include "sph_common.cuh"
+
+constexpr int PB = 128;   // threads per block in the pair kernels
+constexpr int QCAP = 64;  // queue entries per lane (32 KB of shared memory per block)
+constexpr int CH = 8;     // candidates per lane between two queue-occupancy votes
+
+template <int DIM, bool EXACT, class Body>
+__device__ __forceinline__ void walk_q(const DP& p, const float4* __restrict__ A, const int* __restrict__ lb,
+                                       const bool act, const float4 ai, const int cx, const int cy,
+                                       const int cz, unsigned* __restrict__ q, Body&& body) {
+  const float m2x = -2.0f * ai.x, m2y = -2.0f * ai.y, m2z = -2.0f * ai.z;
+  const float thr = EXACT ? p.rc2m : p.rc2m - ai.w;
+  int qn = 0;
+  auto drain = [&]() {
+    const int nm = __reduce_max_sync(FULL, qn);
+#pragma unroll 2
+    for (int k = 0; k < nm; ++k)
+      if (k < qn) body(q[k * PB]);
+    qn = 0;
+  };
+  constexpr int NR = DIM == 3 ? 9 : 3;
+  int ry = -1, rz = DIM == 3 ? -1 : 0;
+#pragma unroll 1
+  for (int r = 0; r < NR; ++r) {
+    int s = 0, e = 0;
+    const int y = cy + ry, z = cz + rz;
+    if (act && y >= 0 && y < p.ny && z >= 0 && z < p.nz) {
+      const int rb = (z * p.ny + y) * p.nx;
+      s = __ldg(lb + rb + max(cx - 1, 0));
+      e = __ldg(lb + rb + min(cx + 1, p.nx - 1) + 1);
+    }
+    if (++ry > 1) { ry = -1; ++rz; }
+    const int nmax = __reduce_max_sync(FULL, e - s);
+#pragma unroll 1
+    for (int k0 = 0; k0 < nmax; k0 += CH) {
+#pragma unroll
+      for (int u = 0; u < CH; ++u) {
+        const int j = s + k0 + u;
+        if (j < e) {
+          const float4 pj = __ldg(A + j);
+          float t;
+          if (EXACT) t = dist2(ai.x - pj.x, ai.y - pj.y, DIM == 3 ? ai.z - pj.z : 0.0f);
+          else if (DIM == 3) t = fmaf(m2x, pj.x, fmaf(m2y, pj.y, fmaf(m2z, pj.z, pj.w)));
+          else t = fmaf(m2x, pj.x, fmaf(m2y, pj.y, pj.w));
+          if (t < thr) {
+            q[qn * PB] = (unsigned)j;
+            ++qn;
+          }
+        }
+      }
+      if (__any_sync(FULL, qn > QCAP - CH)) drain();
+    }
+  }
+  drain();
+}
+
+// Exact pair geometry in units of Q from the fixed-point positions: d = X_i - X_j (wrapping
+// integer subtract, exact), r^2, 1/r (r = 0 -> r = 0 with a finite 1/r), q = r/h and the
+// Wendland C2 factors (reading A1): w = (1 - q/2)^4 (1 + 2q) = W / alpha_d,  f = (1 - q/2)^3.
+struct Geo {
+  float dx, dy, dz, r, rinv, w, f;
+};
+template <int DIM>
+__device__ __forceinline__ Geo geometry(const DP& p, const uint4& xi, const uint4& xj) {
+  Geo g;
+  g.dx = (float)(int)(xi.x - xj.x);
+  g.dy = (float)(int)(xi.y - xj.y);
+  g.dz = DIM == 3 ? (float)(int)(xi.z - xj.z) : 0.0f;
+  const float r2 = DIM == 3 ? fmaf(g.dz, g.dz, fmaf(g.dy, g.dy, g.dx * g.dx)) : fmaf(g.dy, g.dy, g.dx * g.dx);
+  g.rinv = rsqrtf(fmaxf(r2, 0.5f));
+  g.r = r2 * g.rinv;
+  const float qq = g.r * p.qh;
+  const float t = fmaxf(fmaf(-0.5f, qq, 1.0f), 0.0f), t2 = t * t;
+  g.w = t2 * t2 * fmaf(2.0f, qq, 1.0f);
+  g.f = t2 * t;
+  return g;
+}
+
+__device__ __forceinline__ void cell_of_key(const DP& p, unsigned key, int& cx, int& cy, int& cz) {
+  const unsigned row = key / (unsigned)p.nx;
+  cx = (int)(key - row * (unsigned)p.nx);
+  cz = (int)(row / (unsigned)p.ny);
+  cy = (int)(row - (unsigned)cz * (unsigned)p.ny);
+}
+
+// ------------------------------------------------------------------------------------------
+// Wall extrapolation, Eq. 2.12 (readings A4-A7); a_w = 0, v_wall = 0.
+// One thread per wall dummy particle, summing over its fluid neighbours.  WB = (v_w, p_w).
+// ------------------------------------------------------------------------------------------
+template <int DIM, bool MULTI, bool EXACT, bool WITH_VEL>
+__global__ void __launch_bounds__(PB)
+k_wall(const DP p, const SS* __restrict__ S, const int nw, const float4* __restrict__ WA,
+       const uint4* __restrict__ WX, const unsigned* __restrict__ WK, float4* __restrict__ WB,
+       const float4* __restrict__ A, const uint4* __restrict__ X, const float4* __restrict__ B,
+       const int* __restrict__ lbF) {
+  __shared__ unsigned qs[QCAP * PB];
+  unsigned* q = qs + threadIdx.x;
+  const int w0 = blockIdx.x * PB + threadIdx.x;
+  const bool act = w0 < nw;
+  const int w = act ? w0 : nw - 1;
+  const float4 ai = WA[w];
+  const uint4 xi = WX[w];
+  int cx, cy, cz;
+  cell_of_key(p, WK[w], cx, cy, cz);
+  float sW = 0, sp = 0, sWr = 0, srx = 0, sry = 0, srz = 0, svx = 0, svy = 0, svz = 0;
+  walk_q<DIM, EXACT>(p, A, lbF, act, ai, cx, cy, cz, q, [&](const unsigned j) {
+    const uint4 xj = __ldg(X + j);
+    const float4 bj = __ldg(B + j);
+    const Geo g = geometry<DIM>(p, xi, xj);  // r_wf = r_w - r_f
+    const int ph = MULTI ? phase_of(xj) : 0;
+    const float rhof = p.rho0[ph] + bj.w, pf = p.c2[ph] * bj.w;
+    sW += g.w;
+    if (MULTI) {
+      const float ir = __fdividef(g.w, rhof);
+      sp = fmaf(pf, ir, sp);
+      sWr += ir;
+      srx = fmaf(g.dx, g.w, srx); sry = fmaf(g.dy, g.w, sry); srz = fmaf(g.dz, g.w, srz);
+    } else {
+      sp = fmaf(pf, g.w, sp);
+      const float rw = rhof * g.w;
+      srx = fmaf(g.dx, rw, srx); sry = fmaf(g.dy, rw, sry); srz = fmaf(g.dz, rw, srz);
+    }
+    if (WITH_VEL) { svx = fmaf(bj.x, g.w, svx); svy = fmaf(bj.y, g.w, svy); svz = fmaf(bj.z, g.w, svz); }
+  });
+  if (!act) return;
+  float pwall = 0.f, vx = 0.f, vy = 0.f, vz = 0.f;
+  if (sW > 0.f) {
+    const float lever = p.Qf * (S->g[0] * srx + S->g[1] * sry + S->g[2] * srz);
+    pwall = (sp + lever) / (MULTI ? sWr : sW);
+    if (WITH_VEL && (p.flags & SPH_FLAG_WALL_VEL_MIRROR)) {
+      const float is = 1.0f / sW;
+      vx = -svx * is; vy = -svy * is; vz = -svz * is;
+    }
+  }
+  if (WITH_VEL) WB[w] = make_float4(vx, vy, vz, pwall);
+  else WB[w].w = pwall;
+}
+
+// ------------------------------------------------------------------------------------------
+// Pair pass A: sigma_i + Riemann continuity Eq. 2.9 with Eq. 2.8
+// in the scalar form (v_i - v*).grad W = (U* - U_L) W', then the density update
+// Eq. 2.21 / summation Eq. 2.4 in the normalised form of Eq. 2.18 (readings A3, A5, A15).
+// The self pair is a candidate like any other: it adds W(0) to sigma (reading A14) and, with
+// r = 0 and v_ij = 0, nothing to the continuity sum.
+// ------------------------------------------------------------------------------------------
+template <int DIM, bool MULTI, bool EXACT>
+__global__ void __launch_bounds__(PB)
+k_pass_a(const DP p, const SS* __restrict__ S, const int nf, const int init,
+         const float4* __restrict__ A, const uint4* __restrict__ X, const float4* __restrict__ B,
+         const unsigned* __restrict__ K, const int* __restrict__ lbF,
+         const float4* __restrict__ WA, const uint4* __restrict__ WX, const float4* __restrict__ WB,
+         const int* __restrict__ lbW, const unsigned char* __restrict__ wnear,
+         float4* __restrict__ Bout, float* __restrict__ SIG, float* __restrict__ DRHO) {
+  __shared__ unsigned qs[QCAP * PB];
+  unsigned* q = qs + threadIdx.x;
+  const int i0 = blockIdx.x * PB + threadIdx.x;
+  const bool act = i0 < nf;
+  const int i = act ? i0 : nf - 1;
+  const float4 ai = A[i];
+  const uint4 xi = X[i];
+  const float4 bi = B[i];
+  const unsigned key = K[i];
+  int cx, cy, cz;
+  cell_of_key(p, key, cx, cy, cz);
+  const int phi = MULTI ? phase_of(xi) : 0;
+  const float rho0i = p.rho0[phi], c2i = p.c2[phi], ci = p.c0[phi];
+  const float rhoi = rho0i + bi.w, prsi = c2i * bi.w, ZL = rhoi * ci;
+  float sg = 0.f, sc = 0.f;  // compensated sum of W/alpha (DESIGN.md §4 "precision")
+  float acc = 0.f;
+  walk_q<DIM, EXACT>(p, A, lbF, act, ai, cx, cy, cz, q, [&](const unsigned j) {
+    const uint4 xj = __ldg(X + j);
+    const float4 bj = __ldg(B + j);
+    const Geo g = geometry<DIM>(p, xi, xj);
+    { const float y = g.w - sc, t = sg + y; sc = (t - sg) - y; sg = t; }
+    const float vd = fmaf(bi.z - bj.z, g.dz, fmaf(bi.y - bj.y, g.dy, (bi.x - bj.x) * g.dx));
+    if (!MULTI) {
+      // equal c: (U* - U_L)(Z_L + Z_R) = c (rho_j v_ij.e + c (rho_i - rho_j)) with p = c^2 (rho - rho0)
+      const float rhoj = rho0i + bj.w;
+      const float num = fmaf(rhoj, vd, (ci * (bi.w - bj.w)) * g.r);
+      acc = fmaf(g.f, __fdividef(num, rhoj * (rhoi + rhoj)), acc);
+    } else {
+      const int phj = phase_of(xj);
+      const float rhoj = p.rho0[phj] + bj.w, ZR = rhoj * p.c0[phj];
+      const float dpr = phj == phi ? c2i * (bi.w - bj.w) : prsi - p.c2[phj] * bj.w;
+      const float num = fmaf(ZR, vd, dpr * g.r);  // (U* - U_L) W' (Z_L + Z_R) / (W'/r), units of Q
+      acc = fmaf(p.mass[phj] * g.f, __fdividef(num, rhoj * (ZL + ZR)), acc);
+    }
+  });
+  float accw = 0.f;
+  if (__any_sync(FULL, act && wnear[key])) {
+    walk_q<DIM, EXACT>(p, WA, lbW, act, ai, cx, cy, cz, q, [&](const unsigned j) {
+      const uint4 xj = __ldg(WX + j);
+      const float4 bj = __ldg(WB + j);  // (v_w, p_w)
+      const Geo g = geometry<DIM>(p, xi, xj);
+      { const float y = g.w - sc, t = sg + y; sc = (t - sg) - y; sg = t; }
+      const float rhow = fmaf(bj.w, p.inv_c2[phi], rho0i);  // reading A5
+      const float ZR = rhow * ci;
+      const float vd = fmaf(bi.z - bj.z, g.dz, fmaf(bi.y - bj.y, g.dy, (bi.x - bj.x) * g.dx));
+      const float num = fmaf(ZR, vd, (prsi - bj.w) * g.r);
+      accw = fmaf(g.f, __fdividef(num, ZL + ZR), accw);
+    });
+  }
+  if (!act) return;
+  // sigma_i / sigma0 - 1 in float64 from the compensated sum, stored as float32: the density of
+  // Eq. 2.17 / 2.18 is rho0 (1 + dev), so the deviation carries the precision.
+  const float dev = (float)(p.a_over_s0 * ((double)sg - (double)sc) - 1.0);
+  const float accf = MULTI ? acc : p.mass[0] * acc;
+  const float drho = 2.0f * rhoi * p.gradcQ * fmaf(p.V0, accw, accf);  // Eq. 2.9
+  float d = bi.w;
+  if (!init) {
+    if ((p.fs_mask >> phi) & 1u) d = fmaf(S->dt, drho, d);  // Eq. 2.21
+    else d = rho0i * dev;                                   // Eq. 2.4 / 2.18
+  }
+  Bout[i] = make_float4(bi.x, bi.y, bi.z, d);
+  SIG[i] = dev;
+  DRHO[i] = drho;
+}
+
+// ------------------------------------------------------------------------------------------
+// Pair pass B: momentum Eq. 2.10 with p* of Eq. 2.8 (fluid j) / Eq. 2.11 (wall j), penalty
+// Eq. 2.13-2.15 (readings A8, A9, A11), gravity, then the second half kick Eq. 2.22.
+// ------------------------------------------------------------------------------------------
+template <int DIM, bool MULTI, bool EXACT>
+__global__ void __launch_bounds__(PB)
+k_pass_b(const DP p, const SS* __restrict__ S, const int nf,
+         const float4* __restrict__ A, const uint4* __restrict__ X, const float4* __restrict__ B,
+         const unsigned* __restrict__ K, const int* __restrict__ lbF,
+         const float4* __restrict__ WA, const uint4* __restrict__ WX, const float4* __restrict__ WB,
+         const float4* __restrict__ WN, const int* __restrict__ lbW,
+         const unsigned char* __restrict__ wnear, float4* __restrict__ Bout, float4* __restrict__ ACC) {
+  __shared__ unsigned qs[QCAP * PB];
+  unsigned* q = qs + threadIdx.x;
+  const int i0 = blockIdx.x * PB + threadIdx.x;
+  const bool act = i0 < nf;
+  const int i = act ? i0 : nf - 1;
+  const float4 ai = A[i];
+  const uint4 xi = X[i];
+  const float4 bi = B[i];
+  const unsigned key = K[i];
+  int cx, cy, cz;
+  cell_of_key(p, key, cx, cy, cz);
+  const int phi = MULTI ? phase_of(xi) : 0;
+  const float rho0i = p.rho0[phi], c2i = p.c2[phi], ci = p.c0[phi];
+  const float rhoi = rho0i + bi.w, prsi = c2i * bi.w, ZL = rhoi * ci;
+  float ax = 0.f, ay = 0.f, az = 0.f;
+  walk_q<DIM, EXACT>(p, A, lbF, act, ai, cx, cy, cz, q, [&](const unsigned j) {
+    const uint4 xj = __ldg(X + j);
+    const float4 bj = __ldg(B + j);
+    const Geo g = geometry<DIM>(p, xi, xj);
+    const float vd = fmaf(bi.z - bj.z, g.dz, fmaf(bi.y - bj.y, g.dy, (bi.x - bj.x) * g.dx));
+    const float dU = -vd * g.rinv;  // U_L - U_R
+    float coef;
+    if (!MULTI) {
+      // equal c: p*/rho_j = (rho_i p_j + rho_j p_i + rho_i rho_j beta dU) / ((rho_i + rho_j) rho_j)
+      const float rhoj = rho0i + bj.w, prsj = c2i * bj.w;
+      const float beta = fminf(3.0f * fmaxf(dU, 0.f), ci);
+      const float num = fmaf(rhoi * rhoj, beta * dU, fmaf(rhoi, prsj, rhoj * prsi));
+      coef = g.f * __fdividef(num, (rhoi + rhoj) * rhoj);
+    } else {
+      const int phj = phase_of(xj);
+      const float rhoj = p.rho0[phj] + bj.w, prsj = p.c2[phj] * bj.w, ZR = rhoj * p.c0[phj];
+      const float izs = __fdividef(1.0f, ZL + ZR);
+      const float ctil = (ZL + ZR) * __fdividef(1.0f, rhoi + rhoj);
+      const float beta = fminf(3.0f * fmaxf(dU, 0.f), ctil);
+      const float pstar = fmaf(ZL, prsj, ZR * prsi) * izs + ZL * ZR * izs * __fdividef(beta, ctil) * dU;
+      coef = g.f * __fdividef(p.mass[phj] * pstar, rhoj);
+    }
+    ax = fmaf(coef, g.dx, ax); ay = fmaf(coef, g.dy, ay); az = fmaf(coef, g.dz, az);
+  });
+  float wx = 0.f, wy = 0.f, wz = 0.f;
+  if (__any_sync(FULL, act && wnear[key])) {
+    const bool pen = (p.pen_mask >> phi) & 1u;
+    walk_q<DIM, EXACT>(p, WA, lbW, act, ai, cx, cy, cz, q, [&](const unsigned j) {
+      const uint4 xj = __ldg(WX + j);
+      const float pw = __ldg(&WB[j].w);
+      const Geo g = geometry<DIM>(p, xi, xj);
+      const float rhow = fmaf(pw, p.inv_c2[phi], rho0i);
+      const float pstar = __fdividef(fmaf(rhoi, pw, rhow * prsi), rhoi + rhow);  // Eq. 2.11
+      const float coef = g.f * pstar;
+      wx = fmaf(coef, g.dx, wx); wy = fmaf(coef, g.dy, wy); wz = fmaf(coef, g.dz, wz);
+      if (pen) {
+        const float4 n = __ldg(WN + j);
+        if (n.x != 0.f || n.y != 0.f || n.z != 0.f) {
+          const float nd = n.x * g.dx + n.y * g.dy + n.z * g.dz;  // n_w . (r_i - r_w) / Q
+          const float delta = nd * p.two_over_dp;                  // Eq. 2.15 (reading A9); two_over_dp holds 2 Q / dp
+          if (delta < 1.0f && delta > -1.0f) {
+            const float lam = (1.0f - delta) * (1.0f - delta);     // Eq. 2.14 (reading A8)
+            const float Pn = p.gamma_p * lam * fabsf(prsi * nd * g.rinv);
+            const float c = Pn * g.f * g.r;                        // Eq. 2.13, W' = (W'/r) r
+            wx = fmaf(c, n.x, wx); wy = fmaf(c, n.y, wy); wz = fmaf(c, n.z, wz);
+          }
+        }
+      }
+    });
+  }
+  if (!act) return;
+  const float sf = -2.0f * p.gradcQ / rhoi * (MULTI ? 1.0f : p.mass[0]);  // Eq. 2.10
+  const float sw = -2.0f * p.gradcQ / rhoi * p.V0;
+  ax = fmaf(sf, ax, fmaf(sw, wx, S->g[0]));
+  ay = fmaf(sf, ay, fmaf(sw, wy, S->g[1]));
+  az = DIM == 3 ? fmaf(sf, az, fmaf(sw, wz, S->g[2])) : 0.f;
+  ACC[i] = make_float4(ax, ay, az, 0.f);
+  const float hdt = 0.5f * S->dt;
+  Bout[i] = make_float4(fmaf(hdt, ax, bi.x), fmaf(hdt, ay, bi.y), fmaf(hdt, az, bi.z), bi.w);  // Eq. 2.22
+}

@@ -1,0 +1,151 @@
+// sph_sort.cuh — device radix sort of (cell id, index) and cell lower bounds.  Included by sph.cu.
+#pragma once
+// ------------------------------------------------------------------------------------------
+// Device radix sort (stable LSD, 8-bit digits) of (cell id, index).  BASELINE.json north_star
+// "cell hash, device radix sort"; the paper only names the step.
+// Per pass: tile histograms -> row sums -> scan -> stable scatter with warp match ranking.
+// ------------------------------------------------------------------------------------------
+constexpr int RS_THREADS = 256, RS_ITEMS = 16, RS_TILE = RS_THREADS * RS_ITEMS, RS_WARPS = 8;
+
+__global__ void __launch_bounds__(RS_THREADS)
+k_radix_hist(const unsigned* __restrict__ keys, int n, int shift, unsigned* __restrict__ hist,
+             int nblk) {
+  __shared__ unsigned h[256];
+  h[threadIdx.x] = 0;
+  __syncthreads();
+  const int lane = threadIdx.x & 31;
+  const int base = blockIdx.x * RS_TILE;
+#pragma unroll 4
+  for (int it = 0; it < RS_ITEMS; ++it) {
+    int idx = base + it * RS_THREADS + threadIdx.x;
+    bool ok = idx < n;
+    unsigned d = ok ? ((keys[idx] >> shift) & 255u) : 256u;
+    unsigned peers = __match_any_sync(FULL, d);
+    if (ok && lane == __ffs(peers) - 1) atomicAdd(&h[d], (unsigned)__popc(peers));
+  }
+  __syncthreads();
+  hist[threadIdx.x * nblk + blockIdx.x] = h[threadIdx.x];
+}
+
+__global__ void __launch_bounds__(256)
+k_scan_rowsum(const unsigned* __restrict__ hist, int nblk, unsigned* __restrict__ rowsum) {
+  __shared__ unsigned sm[8];
+  unsigned s = 0;
+  const unsigned* row = hist + (size_t)blockIdx.x * nblk;
+  for (int i = threadIdx.x; i < nblk; i += 256) s += row[i];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(FULL, s, o);
+  if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = s;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    unsigned t = 0;
+    for (int w = 0; w < 8; ++w) t += sm[w];
+    rowsum[blockIdx.x] = t;
+  }
+}
+
+// Exclusive scan of hist in (digit-major, block-minor) order, in place.
+__global__ void __launch_bounds__(256)
+k_scan_apply(unsigned* __restrict__ hist, int nblk, const unsigned* __restrict__ rowsum) {
+  __shared__ unsigned sm[8];
+  __shared__ unsigned carry_s;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  // base = sum of rowsum[d'] for d' < digit
+  unsigned b = (threadIdx.x < blockIdx.x) ? rowsum[threadIdx.x] : 0u;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) b += __shfl_xor_sync(FULL, b, o);
+  if (lane == 0) sm[wid] = b;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    unsigned t = 0;
+    for (int w = 0; w < 8; ++w) t += sm[w];
+    carry_s = t;
+  }
+  __syncthreads();
+  unsigned* row = hist + (size_t)blockIdx.x * nblk;
+  for (int i0 = 0; i0 < nblk; i0 += 256) {
+    int i = i0 + threadIdx.x;
+    unsigned v = i < nblk ? row[i] : 0u;
+    unsigned x = v;  // inclusive warp scan
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      unsigned y = __shfl_up_sync(FULL, x, o);
+      if (lane >= o) x += y;
+    }
+    __syncthreads();  // previous iteration's readers of sm / carry_s are done
+    if (lane == 31) sm[wid] = x;
+    __syncthreads();
+    unsigned woff = 0;
+    for (int w = 0; w < wid; ++w) woff += sm[w];
+    unsigned carry = carry_s;
+    if (i < nblk) row[i] = carry + woff + x - v;
+    __syncthreads();
+    if (threadIdx.x == 255) carry_s = carry + woff + x;
+  }
+}
+
+__global__ void __launch_bounds__(RS_THREADS)
+k_radix_scatter(const unsigned* __restrict__ keys, const unsigned* __restrict__ vals, int n, int shift,
+                const unsigned* __restrict__ hist, int nblk, unsigned* __restrict__ keys_out,
+                unsigned* __restrict__ vals_out) {
+  __shared__ unsigned wc[RS_WARPS][256];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  for (int i = threadIdx.x; i < RS_WARPS * 256; i += RS_THREADS) (&wc[0][0])[i] = 0;
+  __syncthreads();
+  const int base = blockIdx.x * RS_TILE + wid * (RS_ITEMS * 32);
+  unsigned k[RS_ITEMS], rank[RS_ITEMS];
+  const unsigned lt = (1u << lane) - 1u;
+#pragma unroll
+  for (int it = 0; it < RS_ITEMS; ++it) {
+    int idx = base + it * 32 + lane;  // warp-contiguous order keeps the sort stable
+    bool ok = idx < n;
+    k[it] = ok ? keys[idx] : 0xffffffffu;
+    unsigned d = ok ? ((k[it] >> shift) & 255u) : 256u;
+    unsigned peers = __match_any_sync(FULL, d);
+    int leader = __ffs(peers) - 1;
+    unsigned old = 0;
+    if (ok && lane == leader) {
+      old = wc[wid][d];
+      wc[wid][d] = old + __popc(peers);
+    }
+    old = __shfl_sync(FULL, old, leader);
+    rank[it] = old + __popc(peers & lt);
+    __syncwarp();
+  }
+  __syncthreads();
+  {  // exclusive prefix over warps per digit, plus the scanned global base of this tile
+    unsigned d = threadIdx.x, run = hist[d * nblk + blockIdx.x];
+#pragma unroll
+    for (int w = 0; w < RS_WARPS; ++w) {
+      unsigned t = wc[w][d];
+      wc[w][d] = run;
+      run += t;
+    }
+  }
+  __syncthreads();
+#pragma unroll
+  for (int it = 0; it < RS_ITEMS; ++it) {
+    int idx = base + it * 32 + lane;
+    if (idx < n) {
+      unsigned d = (k[it] >> shift) & 255u;
+      unsigned dst = wc[wid][d] + rank[it];
+      keys_out[dst] = k[it];
+      vals_out[dst] = vals[idx];
+    }
+  }
+}
+
+// lb[c] = number of sorted particles with key < c, c = 0..ncell (dense lower bounds: the three
+// cells of an x-row of the stencil are one contiguous range [lb[c0], lb[c1+1])).  One thread per
+// cell, binary search in the sorted keys (the tank may be mostly dry: no serial gap filling).
+__global__ void __launch_bounds__(256)
+k_cell_bounds(const unsigned* __restrict__ keys, int n, int ncell, int* __restrict__ lb) {
+  const int c = blockIdx.x * 256 + threadIdx.x;
+  if (c > ncell) return;
+  int lo = 0, hi = n;
+  while (lo < hi) {
+    const int mid = (lo + hi) >> 1;
+    if (keys[mid] < (unsigned)c) lo = mid + 1; else hi = mid;
+  }
+  lb[c] = lo;
+}
