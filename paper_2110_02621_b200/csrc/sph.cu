@@ -419,6 +419,7 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
     rc = radix_sort(c, st, nw, c->keyA, c->valA, c->keyB, c->valB, &ks, &vs);
     if (rc) { cudaFree(idx); return rc; }
     LAUNCH(k_reorder, cdiv(nw, 256), 256, st, c->dp, nw, vs, c->TX, c->TB, c->ID0, c->WX, c->WB, c->WA, c->WID);
+    LAUNCH(k_wall_selfidx, cdiv(nw, 256), 256, st, nw, c->WX);
     CK(cudaMemcpyAsync(c->WK, ks, sizeof(unsigned) * nw, cudaMemcpyDeviceToDevice, st));
     LAUNCH(k_image, cdiv(nw, 256), 256, st, c->dp, nw, c->WX, c->WG);
     LAUNCH(k_cell_bounds, cdiv(c->ncell + 1, 256), 256, st, ks, nw, (int)c->ncell, c->lbW);

@@ -217,3 +217,10 @@ __global__ void k_wnear(DP p, int ncell, const int* __restrict__ lbW, unsigned c
     }
   wnear[c] = (unsigned char)any;
 }
+
+// Walls are static and single-"phase": their X4.w carries the particle's own sorted index instead
+// (lets a pair body reach per-wall data such as the normal from the gathered position alone).
+__global__ void k_wall_selfidx(int nw, uint4* __restrict__ WX) {
+  const int w = blockIdx.x * blockDim.x + threadIdx.x;
+  if (w < nw) WX[w].w = (unsigned)w;
+}

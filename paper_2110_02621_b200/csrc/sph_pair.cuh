@@ -12,24 +12,49 @@
 #pragma once
 #include "sph_common.cuh"
 
-constexpr int PB = 128;   // threads per block in the pair kernels
-constexpr int QCAP = 64;  // queue entries per lane (32 KB of shared memory per block)
-constexpr int CH = 8;     // candidates per lane between two queue-occupancy votes
+#ifndef SPH_PB
+#define SPH_PB 128
+#endif
+#ifndef SPH_QCAP
+#define SPH_QCAP 32
+#endif
+#ifndef SPH_CH
+#define SPH_CH 4
+#endif
+#ifndef SPH_DU
+#define SPH_DU 2
+#endif
+constexpr int PB = SPH_PB;     // threads per block in the pair kernels
+constexpr int QCAP = SPH_QCAP; // queue entries per lane (QCAP * PB * 4 bytes of shared memory per block)
+constexpr int CH = SPH_CH;     // candidates per lane between two queue-occupancy votes (loads issued together)
+constexpr int DU = SPH_DU;     // queue entries drained together (their gathers issued together)
 
+// Body = struct with  Ld load(unsigned j) const  and  void apply(const Ld&)  so that the drain can
+// issue the gathers of DU queue entries before the arithmetic of the first one.
 template <int DIM, bool EXACT, class Body>
 __device__ __forceinline__ void walk_q(const DP& p, const float4* __restrict__ A, const int* __restrict__ lb,
                                        const bool act, const float4 ai, const int cx, const int cy,
-                                       const int cz, unsigned* __restrict__ q, Body&& body) {
+                                       const int cz, unsigned* __restrict__ q, Body& body) {
   const float m2x = -2.0f * ai.x, m2y = -2.0f * ai.y, m2z = -2.0f * ai.z;
   const float thr = EXACT ? p.rc2m : p.rc2m - ai.w;
   int qn = 0;
   auto drain = [&]() {
     const int nm = __reduce_max_sync(FULL, qn);
-#pragma unroll 2
-    for (int k = 0; k < nm; ++k)
-      if (k < qn) body(q[k * PB]);
+#pragma unroll 1
+    for (int k = 0; k < nm; k += DU) {
+      unsigned j[DU];
+#pragma unroll
+      for (int u = 0; u < DU; ++u) j[u] = q[(k + u < qn ? k + u : 0) * PB];  // slot 0 always holds a valid index
+      decltype(body.load(0u)) ld[DU];
+#pragma unroll
+      for (int u = 0; u < DU; ++u) ld[u] = body.load(j[u]);
+#pragma unroll
+      for (int u = 0; u < DU; ++u)
+        if (k + u < qn) body.apply(ld[u]);
+    }
     qn = 0;
   };
+  q[0] = 0u;  // a lane that never queues anything still reads slot 0 in the drain
   constexpr int NR = DIM == 3 ? 9 : 3;
   int ry = -1, rz = DIM == 3 ? -1 : 0;
 #pragma unroll 1
@@ -43,21 +68,22 @@ __device__ __forceinline__ void walk_q(const DP& p, const float4* __restrict__ A
     }
     if (++ry > 1) { ry = -1; ++rz; }
     const int nmax = __reduce_max_sync(FULL, e - s);
+    const int last = e > s ? e - 1 : 0;  // clamp for the unconditional loads (index 0 is valid)
 #pragma unroll 1
     for (int k0 = 0; k0 < nmax; k0 += CH) {
+      float4 pj[CH];
+#pragma unroll
+      for (int u = 0; u < CH; ++u) pj[u] = __ldg(A + min(s + k0 + u, last));
 #pragma unroll
       for (int u = 0; u < CH; ++u) {
         const int j = s + k0 + u;
-        if (j < e) {
-          const float4 pj = __ldg(A + j);
-          float t;
-          if (EXACT) t = dist2(ai.x - pj.x, ai.y - pj.y, DIM == 3 ? ai.z - pj.z : 0.0f);
-          else if (DIM == 3) t = fmaf(m2x, pj.x, fmaf(m2y, pj.y, fmaf(m2z, pj.z, pj.w)));
-          else t = fmaf(m2x, pj.x, fmaf(m2y, pj.y, pj.w));
-          if (t < thr) {
-            q[qn * PB] = (unsigned)j;
-            ++qn;
-          }
+        float t;
+        if (EXACT) t = dist2(ai.x - pj[u].x, ai.y - pj[u].y, DIM == 3 ? ai.z - pj[u].z : 0.0f);
+        else if (DIM == 3) t = fmaf(m2x, pj[u].x, fmaf(m2y, pj[u].y, fmaf(m2z, pj[u].z, pj[u].w)));
+        else t = fmaf(m2x, pj[u].x, fmaf(m2y, pj[u].y, pj[u].w));
+        if (j < e && t < thr) {
+          q[qn * PB] = (unsigned)j;
+          ++qn;
         }
       }
       if (__any_sync(FULL, qn > QCAP - CH)) drain();
@@ -88,6 +114,22 @@ __device__ __forceinline__ Geo geometry(const DP& p, const uint4& xi, const uint
   return g;
 }
 
+// Queue-entry payload of the pair bodies: the neighbour's fixed-point position and (v, rho - rho0).
+struct LdXB {
+  uint4 x;
+  float4 b;
+};
+template <class F>
+struct BodyXB {
+  const uint4* __restrict__ X;
+  const float4* __restrict__ B;
+  F f;
+  __device__ __forceinline__ LdXB load(const unsigned j) const { return LdXB{__ldg(X + j), __ldg(B + j)}; }
+  __device__ __forceinline__ void apply(const LdXB& l) { f(l.x, l.b); }
+};
+template <class F>
+__device__ __forceinline__ BodyXB<F> make_body(const uint4* X, const float4* B, F f) { return BodyXB<F>{X, B, f}; }
+
 __device__ __forceinline__ void cell_of_key(const DP& p, unsigned key, int& cx, int& cy, int& cz) {
   const unsigned row = key / (unsigned)p.nx;
   cx = (int)(key - row * (unsigned)p.nx);
@@ -115,9 +157,8 @@ k_wall(const DP p, const SS* __restrict__ S, const int nw, const float4* __restr
   int cx, cy, cz;
   cell_of_key(p, WK[w], cx, cy, cz);
   float sW = 0, sp = 0, sWr = 0, srx = 0, sry = 0, srz = 0, svx = 0, svy = 0, svz = 0;
-  walk_q<DIM, EXACT>(p, A, lbF, act, ai, cx, cy, cz, q, [&](const unsigned j) {
-    const uint4 xj = __ldg(X + j);
-    const float4 bj = __ldg(B + j);
+  {
+    auto body = make_body(X, B, [&](const uint4& xj, const float4& bj) {
     const Geo g = geometry<DIM>(p, xi, xj);  // r_wf = r_w - r_f
     const int ph = MULTI ? phase_of(xj) : 0;
     const float rhof = p.rho0[ph] + bj.w, pf = p.c2[ph] * bj.w;
@@ -133,7 +174,9 @@ k_wall(const DP p, const SS* __restrict__ S, const int nw, const float4* __restr
       srx = fmaf(g.dx, rw, srx); sry = fmaf(g.dy, rw, sry); srz = fmaf(g.dz, rw, srz);
     }
     if (WITH_VEL) { svx = fmaf(bj.x, g.w, svx); svy = fmaf(bj.y, g.w, svy); svz = fmaf(bj.z, g.w, svz); }
-  });
+    });
+    walk_q<DIM, EXACT>(p, A, lbF, act, ai, cx, cy, cz, q, body);
+  }
   if (!act) return;
   float pwall = 0.f, vx = 0.f, vy = 0.f, vz = 0.f;
   if (sW > 0.f) {
@@ -179,9 +222,8 @@ k_pass_a(const DP p, const SS* __restrict__ S, const int nf, const int init,
   const float rhoi = rho0i + bi.w, prsi = c2i * bi.w, ZL = rhoi * ci;
   float sg = 0.f, sc = 0.f;  // compensated sum of W/alpha (DESIGN.md §4 "precision")
   float acc = 0.f;
-  walk_q<DIM, EXACT>(p, A, lbF, act, ai, cx, cy, cz, q, [&](const unsigned j) {
-    const uint4 xj = __ldg(X + j);
-    const float4 bj = __ldg(B + j);
+  {
+    auto body = make_body(X, B, [&](const uint4& xj, const float4& bj) {
     const Geo g = geometry<DIM>(p, xi, xj);
     { const float y = g.w - sc, t = sg + y; sc = (t - sg) - y; sg = t; }
     const float vd = fmaf(bi.z - bj.z, g.dz, fmaf(bi.y - bj.y, g.dy, (bi.x - bj.x) * g.dx));
@@ -197,12 +239,13 @@ k_pass_a(const DP p, const SS* __restrict__ S, const int nf, const int init,
       const float num = fmaf(ZR, vd, dpr * g.r);  // (U* - U_L) W' (Z_L + Z_R) / (W'/r), units of Q
       acc = fmaf(p.mass[phj] * g.f, __fdividef(num, rhoj * (ZL + ZR)), acc);
     }
-  });
+    });
+    walk_q<DIM, EXACT>(p, A, lbF, act, ai, cx, cy, cz, q, body);
+  }
   float accw = 0.f;
   if (__any_sync(FULL, act && wnear[key])) {
-    walk_q<DIM, EXACT>(p, WA, lbW, act, ai, cx, cy, cz, q, [&](const unsigned j) {
-      const uint4 xj = __ldg(WX + j);
-      const float4 bj = __ldg(WB + j);  // (v_w, p_w)
+    {
+      auto body = make_body(WX, WB, [&](const uint4& xj, const float4& bj) {  // (v_w, p_w)
       const Geo g = geometry<DIM>(p, xi, xj);
       { const float y = g.w - sc, t = sg + y; sc = (t - sg) - y; sg = t; }
       const float rhow = fmaf(bj.w, p.inv_c2[phi], rho0i);  // reading A5
@@ -210,7 +253,9 @@ k_pass_a(const DP p, const SS* __restrict__ S, const int nf, const int init,
       const float vd = fmaf(bi.z - bj.z, g.dz, fmaf(bi.y - bj.y, g.dy, (bi.x - bj.x) * g.dx));
       const float num = fmaf(ZR, vd, (prsi - bj.w) * g.r);
       accw = fmaf(g.f, __fdividef(num, ZL + ZR), accw);
-    });
+      });
+      walk_q<DIM, EXACT>(p, WA, lbW, act, ai, cx, cy, cz, q, body);
+    }
   }
   if (!act) return;
   // sigma_i / sigma0 - 1 in float64 from the compensated sum, stored as float32: the density of
@@ -255,9 +300,8 @@ k_pass_b(const DP p, const SS* __restrict__ S, const int nf,
   const float rho0i = p.rho0[phi], c2i = p.c2[phi], ci = p.c0[phi];
   const float rhoi = rho0i + bi.w, prsi = c2i * bi.w, ZL = rhoi * ci;
   float ax = 0.f, ay = 0.f, az = 0.f;
-  walk_q<DIM, EXACT>(p, A, lbF, act, ai, cx, cy, cz, q, [&](const unsigned j) {
-    const uint4 xj = __ldg(X + j);
-    const float4 bj = __ldg(B + j);
+  {
+    auto body = make_body(X, B, [&](const uint4& xj, const float4& bj) {
     const Geo g = geometry<DIM>(p, xi, xj);
     const float vd = fmaf(bi.z - bj.z, g.dz, fmaf(bi.y - bj.y, g.dy, (bi.x - bj.x) * g.dx));
     const float dU = -vd * g.rinv;  // U_L - U_R
@@ -278,20 +322,22 @@ k_pass_b(const DP p, const SS* __restrict__ S, const int nf,
       coef = g.f * __fdividef(p.mass[phj] * pstar, rhoj);
     }
     ax = fmaf(coef, g.dx, ax); ay = fmaf(coef, g.dy, ay); az = fmaf(coef, g.dz, az);
-  });
+    });
+    walk_q<DIM, EXACT>(p, A, lbF, act, ai, cx, cy, cz, q, body);
+  }
   float wx = 0.f, wy = 0.f, wz = 0.f;
   if (__any_sync(FULL, act && wnear[key])) {
     const bool pen = (p.pen_mask >> phi) & 1u;
-    walk_q<DIM, EXACT>(p, WA, lbW, act, ai, cx, cy, cz, q, [&](const unsigned j) {
-      const uint4 xj = __ldg(WX + j);
-      const float pw = __ldg(&WB[j].w);
+    {
+      auto body = make_body(WX, WB, [&](const uint4& xj, const float4& bj) {
+      const float pw = bj.w;
       const Geo g = geometry<DIM>(p, xi, xj);
       const float rhow = fmaf(pw, p.inv_c2[phi], rho0i);
       const float pstar = __fdividef(fmaf(rhoi, pw, rhow * prsi), rhoi + rhow);  // Eq. 2.11
       const float coef = g.f * pstar;
       wx = fmaf(coef, g.dx, wx); wy = fmaf(coef, g.dy, wy); wz = fmaf(coef, g.dz, wz);
       if (pen) {
-        const float4 n = __ldg(WN + j);
+        const float4 n = __ldg(WN + xj.w);  // wall X4.w holds the wall particle's own sorted index
         if (n.x != 0.f || n.y != 0.f || n.z != 0.f) {
           const float nd = n.x * g.dx + n.y * g.dy + n.z * g.dz;  // n_w . (r_i - r_w) / Q
           const float delta = nd * p.two_over_dp;                  // Eq. 2.15 (reading A9); two_over_dp holds 2 Q / dp
@@ -303,7 +349,9 @@ k_pass_b(const DP p, const SS* __restrict__ S, const int nf,
           }
         }
       }
-    });
+      });
+      walk_q<DIM, EXACT>(p, WA, lbW, act, ai, cx, cy, cz, q, body);
+    }
   }
   if (!act) return;
   const float sf = -2.0f * p.gradcQ / rhoi * (MULTI ? 1.0f : p.mass[0]);  // Eq. 2.10
