@@ -40,8 +40,10 @@ struct sph_ctx {
   int64_t launches = 0;
   float sigma0 = 0.f;
   // fluid (cell-sorted): master position, filter image, (v, rho - rho0) x3, acceleration
-  uint4 *X = nullptr, *TX = nullptr;
-  float4 *A = nullptr, *B0 = nullptr, *B1 = nullptr, *TB = nullptr, *ACC = nullptr;
+  // R0: records after the reorder, R1: after pass A (density updated); TB: (v, rho - rho0) after pass B
+  XB *R0 = nullptr, *R1 = nullptr;
+  uint4* TX = nullptr;
+  float4 *A = nullptr, *TB = nullptr, *ACC = nullptr;
   float *SIG = nullptr, *DRHO = nullptr;
   unsigned *ID0 = nullptr, *ID1 = nullptr, *IDcur = nullptr, *IDnext = nullptr;
   unsigned *keyA = nullptr, *valA = nullptr, *keyB = nullptr, *valB = nullptr, *hist = nullptr,
@@ -49,8 +51,8 @@ struct sph_ctx {
   const unsigned* K = nullptr;  // sorted cell keys of the current fluid order (one of keyA / keyB)
   int *lbF = nullptr, *lbW = nullptr;
   // wall (static)
-  uint4* WX = nullptr;
-  float4 *WA = nullptr, *WB = nullptr, *WN = nullptr, *WG = nullptr;
+  XB* WR = nullptr;
+  float4 *WA = nullptr, *WN = nullptr, *WG = nullptr;
   unsigned *WK = nullptr, *WID = nullptr;
   unsigned char* wnear = nullptr;
   SS* S = nullptr;
@@ -118,9 +120,9 @@ int dalloc(sph_ctx* c, T** p, size_t count) {
 }
 
 void free_all(sph_ctx* c) {
-  void* ptrs[] = {c->X, c->TX, c->A, c->B0, c->B1, c->TB, c->ACC, c->SIG, c->DRHO, c->ID0, c->ID1,
-                  c->keyA, c->valA, c->keyB, c->valB, c->hist, c->rowsum, c->lbF, c->lbW, c->WX,
-                  c->WA, c->WB, c->WN, c->WG, c->WK, c->WID, c->wnear, c->S, c->dt_seq, c->stat};
+  void* ptrs[] = {c->R0, c->R1, c->TX, c->A, c->TB, c->ACC, c->SIG, c->DRHO, c->ID0, c->ID1,
+                  c->keyA, c->valA, c->keyB, c->valB, c->hist, c->rowsum, c->lbF, c->lbW, c->WR,
+                  c->WA, c->WN, c->WG, c->WK, c->WID, c->wnear, c->S, c->dt_seq, c->stat};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   for (auto e : c->ev) cudaEventDestroy(e);
@@ -166,13 +168,13 @@ struct Prof {
 };
 
 // wall extrapolation launcher (B = the fluid (v, rho - rho0) array the pressures are read from)
-void launch_wall(sph_ctx* c, cudaStream_t st, bool with_vel, const float4* B) {
+void launch_wall(sph_ctx* c, cudaStream_t st, bool with_vel, const XB* R) {
   if (c->nw == 0 || c->nf == 0) return;
   const int grid = cdiv(c->nw, PB), nw = (int)c->nw;
   if (with_vel) {
-    WALL_DISPATCH(true, grid, st, c->dp, c->S, nw, c->WA, c->WX, c->WK, c->WB, c->A, c->X, B, c->lbF);
+    WALL_DISPATCH(true, grid, st, c->dp, c->S, nw, c->WA, c->WR, c->WK, c->A, R, c->lbF);
   } else {
-    WALL_DISPATCH(false, grid, st, c->dp, c->S, nw, c->WA, c->WX, c->WK, c->WB, c->A, c->X, B, c->lbF);
+    WALL_DISPATCH(false, grid, st, c->dp, c->S, nw, c->WA, c->WR, c->WK, c->A, R, c->lbF);
   }
 }
 
@@ -185,22 +187,22 @@ int pipeline_after_hash(sph_ctx* c, cudaStream_t st, int init, Prof& pf) {
   c->K = ks;
   pf.mark();  // end sort
   if (nf > 0) {
-    LAUNCH(k_reorder, cdiv(nf, 256), 256, st, c->dp, nf, vs, c->TX, c->TB, c->IDcur, c->X, c->B0, c->A, c->IDnext);
+    LAUNCH(k_reorder, cdiv(nf, 256), 256, st, c->dp, nf, vs, c->TX, c->TB, c->IDcur, c->R0, c->A, c->IDnext);
     std::swap(c->IDcur, c->IDnext);
   }
   LAUNCH(k_cell_bounds, cdiv(c->ncell + 1, 256), 256, st, ks, nf, (int)c->ncell, c->lbF);
   pf.mark();  // end reorder
-  launch_wall(c, st, true, c->B0);
+  launch_wall(c, st, true, c->R0);
   pf.mark();  // end wall 1
   if (nf > 0) {
-    PAIR_DISPATCH(k_pass_a, cdiv(nf, PB), st, c->dp, c->S, nf, init, c->A, c->X, c->B0, c->K, c->lbF, c->WA, c->WX,
-                  c->WB, c->lbW, c->wnear, c->B1, c->SIG, c->DRHO);
+    PAIR_DISPATCH(k_pass_a, cdiv(nf, PB), st, c->dp, c->S, nf, init, c->A, c->R0, c->K, c->lbF, c->WA, c->WR,
+                  c->lbW, c->wnear, c->R1, c->SIG, c->DRHO);
   }
   pf.mark();  // end pass A
-  launch_wall(c, st, false, c->B1);
+  launch_wall(c, st, false, c->R1);
   pf.mark();  // end wall 2
   if (nf > 0) {
-    PAIR_DISPATCH(k_pass_b, cdiv(nf, PB), st, c->dp, c->S, nf, c->A, c->X, c->B1, c->K, c->lbF, c->WA, c->WX, c->WB,
+    PAIR_DISPATCH(k_pass_b, cdiv(nf, PB), st, c->dp, c->S, nf, c->A, c->R1, c->K, c->lbF, c->WA, c->WR,
                   c->WN, c->lbW, c->wnear, c->TB, c->ACC);
   }
   pf.mark();  // end pass B
@@ -227,7 +229,7 @@ int do_steps(sph_ctx* c, int32_t n_steps, const double* dt_host, cudaStream_t st
     pf.mark();  // start
     LAUNCH(k_dt, dt_grid, 256, st, c->dp, c->S, nf, c->TB, dt_host ? c->dt_seq : nullptr, s);
     if (nf > 0)
-      LAUNCH(k_predict, cdiv(nf, 256), 256, st, c->dp, c->S, nf, c->X, c->TB, c->ACC, c->SIG, c->TX, c->keyA, c->valA);
+      LAUNCH(k_predict, cdiv(nf, 256), 256, st, c->dp, c->S, nf, c->R1, c->TB, c->ACC, c->SIG, c->TX, c->keyA, c->valA);
     pf.mark();  // end predict
     int rc = pipeline_after_hash(c, st, 0, pf);
     if (rc) return rc;
@@ -239,7 +241,7 @@ int do_steps(sph_ctx* c, int32_t n_steps, const double* dt_host, cudaStream_t st
 // float32 images of the current fluid positions for the contract-exact debug walks (scratch: TX)
 float4* fluid_images(sph_ctx* c, cudaStream_t st) {
   float4* G = reinterpret_cast<float4*>(c->TX);
-  if (c->nf) LAUNCH(k_image, cdiv(c->nf, 256), 256, st, c->dp, (int)c->nf, c->X, G);
+  if (c->nf) LAUNCH(k_image, cdiv(c->nf, 256), 256, st, c->dp, (int)c->nf, c->R1, G);
   return G;
 }
 
@@ -387,8 +389,8 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
   const int nf = (int)c->nf, nw = (int)c->nw;
   const size_t cap = (size_t)std::max(nf, nw);
   int rc = 0;
-  rc |= dalloc(c, &c->X, nf); rc |= dalloc(c, &c->TX, cap); rc |= dalloc(c, &c->A, nf);
-  rc |= dalloc(c, &c->B0, nf); rc |= dalloc(c, &c->B1, nf); rc |= dalloc(c, &c->TB, cap);
+  rc |= dalloc(c, &c->R0, nf); rc |= dalloc(c, &c->R1, nf); rc |= dalloc(c, &c->TX, cap); rc |= dalloc(c, &c->A, (size_t)nf + 16);
+  rc |= dalloc(c, &c->TB, cap);
   rc |= dalloc(c, &c->ACC, nf); rc |= dalloc(c, &c->SIG, nf); rc |= dalloc(c, &c->DRHO, nf);
   rc |= dalloc(c, &c->ID0, cap); rc |= dalloc(c, &c->ID1, cap);
   rc |= dalloc(c, &c->keyA, cap); rc |= dalloc(c, &c->valA, cap); rc |= dalloc(c, &c->keyB, cap);
@@ -397,13 +399,15 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
   rc |= dalloc(c, &c->rowsum, 256);
   rc |= dalloc(c, &c->lbF, c->ncell + 1); rc |= dalloc(c, &c->lbW, c->ncell + 1);
   rc |= dalloc(c, &c->wnear, c->ncell);
-  rc |= dalloc(c, &c->WX, nw); rc |= dalloc(c, &c->WA, nw); rc |= dalloc(c, &c->WB, nw);
+  rc |= dalloc(c, &c->WR, nw); rc |= dalloc(c, &c->WA, (size_t)nw + 16);
   rc |= dalloc(c, &c->WN, nw); rc |= dalloc(c, &c->WG, nw); rc |= dalloc(c, &c->WK, nw);
   rc |= dalloc(c, &c->WID, nw);
   rc |= dalloc(c, &c->S, 1); rc |= dalloc(c, &c->stat, 1);
   if (rc) return c->err.find("out of memory") != std::string::npos ? SPH_ENOMEM : SPH_ECUDA;
   c->IDcur = c->ID0; c->IDnext = c->ID1;
   CK(cudaMemsetAsync(c->S, 0, sizeof(SS), st));
+  CK(cudaMemsetAsync(c->A + nf, 0, 16 * sizeof(float4), st));   // padding read by the chunked candidate loads
+  CK(cudaMemsetAsync(c->WA + nw, 0, 16 * sizeof(float4), st));
   CK(cudaMemsetAsync(c->ACC, 0, sizeof(float4) * std::max(nf, 1), st));
   {  // gravity at t = 0 (sin(0) = 0)
     float g0[3] = {(float)c->prm.g[0], (float)c->prm.g[1], (float)c->prm.g[2]};
@@ -418,13 +422,13 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
     unsigned *ks, *vs;
     rc = radix_sort(c, st, nw, c->keyA, c->valA, c->keyB, c->valB, &ks, &vs);
     if (rc) { cudaFree(idx); return rc; }
-    LAUNCH(k_reorder, cdiv(nw, 256), 256, st, c->dp, nw, vs, c->TX, c->TB, c->ID0, c->WX, c->WB, c->WA, c->WID);
-    LAUNCH(k_wall_selfidx, cdiv(nw, 256), 256, st, nw, c->WX);
+    LAUNCH(k_reorder, cdiv(nw, 256), 256, st, c->dp, nw, vs, c->TX, c->TB, c->ID0, c->WR, c->WA, c->WID);
+    LAUNCH(k_wall_selfidx, cdiv(nw, 256), 256, st, nw, c->WR);
     CK(cudaMemcpyAsync(c->WK, ks, sizeof(unsigned) * nw, cudaMemcpyDeviceToDevice, st));
-    LAUNCH(k_image, cdiv(nw, 256), 256, st, c->dp, nw, c->WX, c->WG);
+    LAUNCH(k_image, cdiv(nw, 256), 256, st, c->dp, nw, c->WR, c->WG);
     LAUNCH(k_cell_bounds, cdiv(c->ncell + 1, 256), 256, st, ks, nw, (int)c->ncell, c->lbW);
-    if (c->prm.dim == 3) LAUNCH(k_normals<3>, cdiv(nw, 128), 128, st, c->dp, nw, c->WX, c->WK, c->lbW, c->WN);
-    else LAUNCH(k_normals<2>, cdiv(nw, 128), 128, st, c->dp, nw, c->WX, c->WK, c->lbW, c->WN);
+    if (c->prm.dim == 3) LAUNCH(k_normals<3>, cdiv(nw, 128), 128, st, c->dp, nw, c->WR, c->WK, c->lbW, c->WN);
+    else LAUNCH(k_normals<2>, cdiv(nw, 128), 128, st, c->dp, nw, c->WR, c->WK, c->lbW, c->WN);
   } else {
     LAUNCH(k_cell_bounds, cdiv(c->ncell + 1, 256), 256, st, c->keyA, 0, (int)c->ncell, c->lbW);
   }
@@ -487,8 +491,8 @@ int sph_get_fields(sph_ctx* c, float* pos, float* vel, float* rho, float* p, flo
   if (!c) return SPH_EINVAL;
   if (!c->loaded) { c->err = "no particles"; return SPH_EINVAL; }
   cudaStream_t st = (cudaStream_t)stream;
-  if (c->nf) LAUNCH(k_get, cdiv(c->nf, 256), 256, st, c->dp, (int)c->nf, 0, c->X, c->TB, c->ACC, c->IDcur, pos, vel, rho, p, acc);
-  if (c->nw) LAUNCH(k_get, cdiv(c->nw, 256), 256, st, c->dp, (int)c->nw, 1, c->WX, c->WB, (const float4*)nullptr, c->WID, pos, vel, rho, p, acc);
+  if (c->nf) LAUNCH(k_get, cdiv(c->nf, 256), 256, st, c->dp, (int)c->nf, 0, c->R1, c->TB, c->ACC, c->IDcur, pos, vel, rho, p, acc);
+  if (c->nw) LAUNCH(k_get, cdiv(c->nw, 256), 256, st, c->dp, (int)c->nw, 1, c->WR, (const float4*)nullptr, (const float4*)nullptr, c->WID, pos, vel, rho, p, acc);
   CK(cudaGetLastError());
   return SPH_OK;
 }
@@ -530,7 +534,7 @@ int sph_get_stats(sph_ctx* c, sph_stats* out, void* stream) {
   CK(cudaMemcpyAsync(c->stat, &z, sizeof(z), cudaMemcpyHostToDevice, st));
   const int nf = (int)c->nf;
   if (nf) {
-    LAUNCH(k_stats, std::min(cdiv(nf, 256), 1184), 256, st, c->dp, nf, c->X, c->TB, c->stat);
+    LAUNCH(k_stats, std::min(cdiv(nf, 256), 1184), 256, st, c->dp, nf, c->R1, c->TB, c->stat);
     const float4* G = fluid_images(c, st);
     LAUNCH(k_neigh, cdiv(nf, PW), PW * 32, st, c->dp, nf, 0, 0, G, c->IDcur, G, c->IDcur, c->lbF, c->WG,
            c->WID, c->lbW, (int*)nullptr, (const long long*)nullptr, (int*)nullptr, 0ll, &c->stat->pairs);

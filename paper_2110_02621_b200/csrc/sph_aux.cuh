@@ -37,14 +37,13 @@ __global__ void k_load(DP p, int n, int is_wall, const int* __restrict__ idx, co
 // Gather into cell-sorted order and derive the centred float32 image used by the candidate filter.
 __global__ void __launch_bounds__(256)
 k_reorder(DP p, int n, const unsigned* __restrict__ vals, const uint4* __restrict__ TX,
-          const float4* __restrict__ TB, const unsigned* __restrict__ IDin, uint4* __restrict__ X,
-          float4* __restrict__ B, float4* __restrict__ A, unsigned* __restrict__ IDout) {
+          const float4* __restrict__ TB, const unsigned* __restrict__ IDin, XB* __restrict__ R,
+          float4* __restrict__ A, unsigned* __restrict__ IDout) {
   const int s = blockIdx.x * 256 + threadIdx.x;
   if (s >= n) return;
   const unsigned v = vals[s];
   const uint4 x = TX[v];
-  X[s] = x;
-  B[s] = TB[v];
+  R[s] = XB{x, TB[v]};
   A[s] = centred_image(p, x);
   IDout[s] = IDin[v];
 }
@@ -117,12 +116,12 @@ __device__ __forceinline__ unsigned drift_axis(unsigned X, unsigned& res, double
 // (same positions, reading A13), first half kick Eq. 2.19, drift Eq. 2.20,
 // cell hash of the new position.  In place on (v, rho) ; the new position goes to TX.
 __global__ void __launch_bounds__(256)
-k_predict(DP p, SS* __restrict__ S, int nf, const uint4* __restrict__ X, float4* __restrict__ B,
+k_predict(DP p, SS* __restrict__ S, int nf, const XB* __restrict__ R, float4* __restrict__ B,
           const float4* __restrict__ ACC, const float* __restrict__ SIG, uint4* __restrict__ TX,
           unsigned* __restrict__ keys, unsigned* __restrict__ vals) {
   const int i = blockIdx.x * 256 + threadIdx.x;
   if (i >= nf) return;
-  uint4 x = X[i];
+  uint4 x = R[i].x;
   float4 b = B[i];
   const float4 a = ACC[i];
   const int ph = phase_of(x);
@@ -161,11 +160,11 @@ k_predict(DP p, SS* __restrict__ S, int nf, const uint4* __restrict__ X, float4*
 
 // Wall normals, Eq. 2.16, once, in float64 (reading A10).
 template <int DIM>
-__global__ void k_normals(DP p, int nw, const uint4* __restrict__ WX, const unsigned* __restrict__ WK,
+__global__ void k_normals(DP p, int nw, const XB* __restrict__ WR, const unsigned* __restrict__ WK,
                           const int* __restrict__ lbW, float4* __restrict__ WN) {
   const int w = blockIdx.x * blockDim.x + threadIdx.x;
   if (w >= nw) return;
-  const uint4 xi = WX[w];
+  const uint4 xi = WR[w].x;
   const unsigned key = WK[w];
   const unsigned row = key / (unsigned)p.nx;
   const int cx = (int)(key - row * (unsigned)p.nx), cz = (int)(row / (unsigned)p.ny),
@@ -184,7 +183,7 @@ __global__ void k_normals(DP p, int nw, const uint4* __restrict__ WX, const unsi
       const int s = lbW[rb + max(cx - 1, 0)], e = lbW[rb + min(cx + 1, p.nx - 1) + 1];
       for (int j = s; j < e; ++j) {
         if (j == w) continue;
-        const uint4 xj = WX[j];
+        const uint4 xj = WR[j].x;
         const double dx = p.Q * (double)(int)(xi.x - xj.x), dyy = p.Q * (double)(int)(xi.y - xj.y),
                      dzz = DIM == 3 ? p.Q * (double)(int)(xi.z - xj.z) : 0.0;
         const double r2 = dx * dx + dyy * dyy + dzz * dzz;
@@ -220,7 +219,7 @@ __global__ void k_wnear(DP p, int ncell, const int* __restrict__ lbW, unsigned c
 
 // Walls are static and single-"phase": their X4.w carries the particle's own sorted index instead
 // (lets a pair body reach per-wall data such as the normal from the gathered position alone).
-__global__ void k_wall_selfidx(int nw, uint4* __restrict__ WX) {
+__global__ void k_wall_selfidx(int nw, XB* __restrict__ WR) {
   const int w = blockIdx.x * blockDim.x + threadIdx.x;
-  if (w < nw) WX[w].w = (unsigned)w;
+  if (w < nw) WR[w].x.w = (unsigned)w;
 }

@@ -2,6 +2,7 @@
 // Included by sph.cu only.  Citations: PAPER.md:<line>; readings Axx: DESIGN.md §3.
 //
 // Data layout.  Fluid and wall particles live in separate cell-sorted arrays:
+//   (X4 and B4 are interleaved in one 32-byte record XB per particle)
 //   X4  uint4   fixed-point master position (X, Y, Z) in units of Q = 2^-k m from the origin O,
 //               .w = residual of each axis in units of Q/1024 (3 x 10 bits, biased by 512) << 2 | phase
 //   A4  float4  float32 image centred on the domain centre (xc, yc, zc, |xc|^2): candidate test only
@@ -36,6 +37,19 @@ struct DP {
   double a_over_s0;
   double g[3], gamp[3], gperiod;
 };
+
+// Per-particle record gathered by the pair bodies: one 32-byte sector, one 256-bit load.
+struct __align__(32) XB {
+  uint4 x;   // fixed-point master position (+ residual / phase, or the wall's own index)
+  float4 b;  // (vx, vy, vz, rho - rho0_phase); walls: (v_w, p_w)
+};
+__device__ __forceinline__ XB ldg256(const XB* p) {  // LDG.E.256 (sm_100+): the whole record in one request
+  XB r;
+  asm("ld.global.nc.v8.u32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+      : "=r"(r.x.x), "=r"(r.x.y), "=r"(r.x.z), "=r"(r.x.w), "=f"(r.b.x), "=f"(r.b.y), "=f"(r.b.z), "=f"(r.b.w)
+      : "l"(p));
+  return r;
+}
 
 // Device-resident per-step state: written by k_dt, read by every other kernel, so that
 // sph_step(n) needs no host synchronisation between steps.

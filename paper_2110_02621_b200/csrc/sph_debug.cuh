@@ -4,10 +4,10 @@
 #pragma once
 #include "sph_common.cuh"
 
-__global__ void k_image(DP p, int n, const uint4* __restrict__ X, float4* __restrict__ G) {
+__global__ void k_image(DP p, int n, const XB* __restrict__ R, float4* __restrict__ G) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
-  const uint4 x = X[i];
+  const uint4 x = R[i].x;
   G[i] = make_float4(fx_image(x.x, p.O[0], p.Q), fx_image(x.y, p.O[1], p.Q),
                      p.dim == 3 ? fx_image(x.z, p.O[2], p.Q) : 0.0f, 0.0f);
 }
@@ -73,13 +73,13 @@ constexpr int PW = 8;  // warps per block in k_neigh
 // ------------------------------------------------------------------------------------------
 // Output
 // ------------------------------------------------------------------------------------------
-__global__ void k_get(DP p, int n, int is_wall, const uint4* __restrict__ X, const float4* __restrict__ B,
+__global__ void k_get(DP p, int n, int is_wall, const XB* __restrict__ R, const float4* __restrict__ B,
                       const float4* __restrict__ ACC, const unsigned* __restrict__ ID, float* pos,
                       float* vel, float* rho, float* prs, float* acc) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
-  const uint4 x = X[i];
-  const float4 b = B[i];
+  const uint4 x = R[i].x;
+  const float4 b = B ? B[i] : R[i].b;
   const size_t o = ID[i];
   if (pos) {
     pos[3 * o] = fx_image(x.x, p.O[0], p.Q);
@@ -127,14 +127,14 @@ __device__ __forceinline__ unsigned f2ord(float f) {
 }
 
 __global__ void __launch_bounds__(256)
-k_stats(DP p, int nf, const uint4* __restrict__ X, const float4* __restrict__ B, StatAcc* out) {
+k_stats(DP p, int nf, const XB* __restrict__ R, const float4* __restrict__ B, StatAcc* out) {
   double ek = 0;
   unsigned cnt[SPH_MAX_PHASES] = {0, 0, 0, 0};
   float xf = -INFINITY;
   const int up = p.dim - 1;
   const float zlim = p.dmin[up] + 6.0f * (float)p.dpD;
   for (int i = blockIdx.x * 256 + threadIdx.x; i < nf; i += gridDim.x * 256) {
-    const uint4 x = X[i];
+    const uint4 x = R[i].x;
     const float4 v = B[i];
     const int ph = phase_of(x);
     ek += 0.5 * p.massD[ph] * ((double)v.x * v.x + (double)v.y * v.y + (double)v.z * v.z);

@@ -37,24 +37,24 @@ __device__ __forceinline__ void walk_q(const DP& p, const float4* __restrict__ A
                                        const int cz, unsigned* __restrict__ q, Body& body) {
   const float m2x = -2.0f * ai.x, m2y = -2.0f * ai.y, m2z = -2.0f * ai.z;
   const float thr = EXACT ? p.rc2m : p.rc2m - ai.w;
-  int qn = 0;
+  // next free slot of this lane's queue q[k * PB], k = 0..QCAP-1, as a 32-bit shared-memory address
+  const unsigned qa0 = (unsigned)__cvta_generic_to_shared(q);
+  unsigned qa = qa0;
   auto drain = [&]() {
+    const int qn = (int)(qa - qa0) / (PB * 4);
     const int nm = __reduce_max_sync(FULL, qn);
 #pragma unroll 1
     for (int k = 0; k < nm; k += DU) {
-      unsigned j[DU];
-#pragma unroll
-      for (int u = 0; u < DU; ++u) j[u] = q[(k + u < qn ? k + u : 0) * PB];  // slot 0 always holds a valid index
       decltype(body.load(0u)) ld[DU];
 #pragma unroll
-      for (int u = 0; u < DU; ++u) ld[u] = body.load(j[u]);
+      for (int u = 0; u < DU; ++u)
+        if (k + u < qn) ld[u] = body.load(q[(k + u) * PB]);
 #pragma unroll
       for (int u = 0; u < DU; ++u)
         if (k + u < qn) body.apply(ld[u]);
     }
-    qn = 0;
+    qa = qa0;
   };
-  q[0] = 0u;  // a lane that never queues anything still reads slot 0 in the drain
   constexpr int NR = DIM == 3 ? 9 : 3;
   int ry = -1, rz = DIM == 3 ? -1 : 0;
 #pragma unroll 1
@@ -67,26 +67,28 @@ __device__ __forceinline__ void walk_q(const DP& p, const float4* __restrict__ A
       e = __ldg(lb + rb + min(cx + 1, p.nx - 1) + 1);
     }
     if (++ry > 1) { ry = -1; ++rz; }
-    const int nmax = __reduce_max_sync(FULL, e - s);
-    const int last = e > s ? e - 1 : 0;  // clamp for the unconditional loads (index 0 is valid)
+    const int len = e - s;
+    const int nmax = __reduce_max_sync(FULL, len);
+    const int last = len > 0 ? e - 1 : 0;  // clamp of the chunk base (index 0 is valid; arrays are padded by CH)
 #pragma unroll 1
     for (int k0 = 0; k0 < nmax; k0 += CH) {
+      const int jb = s + k0, rem = len - k0;
+      const float4* __restrict__ ap = A + min(jb, last);
       float4 pj[CH];
 #pragma unroll
-      for (int u = 0; u < CH; ++u) pj[u] = __ldg(A + min(s + k0 + u, last));
+      for (int u = 0; u < CH; ++u) pj[u] = __ldg(ap + u);
 #pragma unroll
       for (int u = 0; u < CH; ++u) {
-        const int j = s + k0 + u;
         float t;
         if (EXACT) t = dist2(ai.x - pj[u].x, ai.y - pj[u].y, DIM == 3 ? ai.z - pj[u].z : 0.0f);
         else if (DIM == 3) t = fmaf(m2x, pj[u].x, fmaf(m2y, pj[u].y, fmaf(m2z, pj[u].z, pj[u].w)));
         else t = fmaf(m2x, pj[u].x, fmaf(m2y, pj[u].y, pj[u].w));
-        if (j < e && t < thr) {
-          q[qn * PB] = (unsigned)j;
-          ++qn;
+        if (u < rem && t < thr) {
+          asm volatile("st.shared.u32 [%0], %1;" ::"r"(qa), "r"(jb + u) : "memory");
+          qa += PB * 4;
         }
       }
-      if (__any_sync(FULL, qn > QCAP - CH)) drain();
+      if (__any_sync(FULL, qa > qa0 + (QCAP - CH) * PB * 4)) drain();
     }
   }
   drain();
@@ -95,6 +97,16 @@ __device__ __forceinline__ void walk_q(const DP& p, const float4* __restrict__ A
 // Exact pair geometry in units of Q from the fixed-point positions: d = X_i - X_j (wrapping
 // integer subtract, exact), r^2, 1/r (r = 0 -> r = 0 with a finite 1/r), q = r/h and the
 // Wendland C2 factors (reading A1): w = (1 - q/2)^4 (1 + 2q) = W / alpha_d,  f = (1 - q/2)^3.
+__device__ __forceinline__ float rsqrt_fast(float x) {  // MUFU.RSQ, no denormal fix-up (x >= 0.5 here)
+  float y;
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ float div_fast(float a, float b) {  // a * MUFU.RCP(b), b normal and finite here
+  float y;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(b));
+  return a * y;
+}
 struct Geo {
   float dx, dy, dz, r, rinv, w, f;
 };
@@ -105,7 +117,7 @@ __device__ __forceinline__ Geo geometry(const DP& p, const uint4& xi, const uint
   g.dy = (float)(int)(xi.y - xj.y);
   g.dz = DIM == 3 ? (float)(int)(xi.z - xj.z) : 0.0f;
   const float r2 = DIM == 3 ? fmaf(g.dz, g.dz, fmaf(g.dy, g.dy, g.dx * g.dx)) : fmaf(g.dy, g.dy, g.dx * g.dx);
-  g.rinv = rsqrtf(fmaxf(r2, 0.5f));
+  g.rinv = rsqrt_fast(fmaxf(r2, 0.5f));
   g.r = r2 * g.rinv;
   const float qq = g.r * p.qh;
   const float t = fmaxf(fmaf(-0.5f, qq, 1.0f), 0.0f), t2 = t * t;
@@ -114,21 +126,16 @@ __device__ __forceinline__ Geo geometry(const DP& p, const uint4& xi, const uint
   return g;
 }
 
-// Queue-entry payload of the pair bodies: the neighbour's fixed-point position and (v, rho - rho0).
-struct LdXB {
-  uint4 x;
-  float4 b;
-};
+// Pair body = the neighbour's record (one 256-bit gather) + the arithmetic on it.
 template <class F>
 struct BodyXB {
-  const uint4* __restrict__ X;
-  const float4* __restrict__ B;
+  const XB* __restrict__ R;
   F f;
-  __device__ __forceinline__ LdXB load(const unsigned j) const { return LdXB{__ldg(X + j), __ldg(B + j)}; }
-  __device__ __forceinline__ void apply(const LdXB& l) { f(l.x, l.b); }
+  __device__ __forceinline__ XB load(const unsigned j) const { return ldg256(R + j); }
+  __device__ __forceinline__ void apply(const XB& l) { f(l.x, l.b); }
 };
 template <class F>
-__device__ __forceinline__ BodyXB<F> make_body(const uint4* X, const float4* B, F f) { return BodyXB<F>{X, B, f}; }
+__device__ __forceinline__ BodyXB<F> make_body(const XB* R, F f) { return BodyXB<F>{R, f}; }
 
 __device__ __forceinline__ void cell_of_key(const DP& p, unsigned key, int& cx, int& cy, int& cz) {
   const unsigned row = key / (unsigned)p.nx;
@@ -144,27 +151,26 @@ __device__ __forceinline__ void cell_of_key(const DP& p, unsigned key, int& cx, 
 template <int DIM, bool MULTI, bool EXACT, bool WITH_VEL>
 __global__ void __launch_bounds__(PB)
 k_wall(const DP p, const SS* __restrict__ S, const int nw, const float4* __restrict__ WA,
-       const uint4* __restrict__ WX, const unsigned* __restrict__ WK, float4* __restrict__ WB,
-       const float4* __restrict__ A, const uint4* __restrict__ X, const float4* __restrict__ B,
-       const int* __restrict__ lbF) {
+       XB* __restrict__ WR, const unsigned* __restrict__ WK,
+       const float4* __restrict__ A, const XB* __restrict__ R, const int* __restrict__ lbF) {
   __shared__ unsigned qs[QCAP * PB];
   unsigned* q = qs + threadIdx.x;
   const int w0 = blockIdx.x * PB + threadIdx.x;
   const bool act = w0 < nw;
   const int w = act ? w0 : nw - 1;
   const float4 ai = WA[w];
-  const uint4 xi = WX[w];
+  const uint4 xi = WR[w].x;
   int cx, cy, cz;
   cell_of_key(p, WK[w], cx, cy, cz);
   float sW = 0, sp = 0, sWr = 0, srx = 0, sry = 0, srz = 0, svx = 0, svy = 0, svz = 0;
   {
-    auto body = make_body(X, B, [&](const uint4& xj, const float4& bj) {
+    auto body = make_body(R, [&](const uint4& xj, const float4& bj) {
     const Geo g = geometry<DIM>(p, xi, xj);  // r_wf = r_w - r_f
     const int ph = MULTI ? phase_of(xj) : 0;
     const float rhof = p.rho0[ph] + bj.w, pf = p.c2[ph] * bj.w;
     sW += g.w;
     if (MULTI) {
-      const float ir = __fdividef(g.w, rhof);
+      const float ir = div_fast(g.w, rhof);
       sp = fmaf(pf, ir, sp);
       sWr += ir;
       srx = fmaf(g.dx, g.w, srx); sry = fmaf(g.dy, g.w, sry); srz = fmaf(g.dz, g.w, srz);
@@ -187,8 +193,8 @@ k_wall(const DP p, const SS* __restrict__ S, const int nw, const float4* __restr
       vx = -svx * is; vy = -svy * is; vz = -svz * is;
     }
   }
-  if (WITH_VEL) WB[w] = make_float4(vx, vy, vz, pwall);
-  else WB[w].w = pwall;
+  if (WITH_VEL) WR[w].b = make_float4(vx, vy, vz, pwall);
+  else WR[w].b.w = pwall;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -201,19 +207,19 @@ k_wall(const DP p, const SS* __restrict__ S, const int nw, const float4* __restr
 template <int DIM, bool MULTI, bool EXACT>
 __global__ void __launch_bounds__(PB)
 k_pass_a(const DP p, const SS* __restrict__ S, const int nf, const int init,
-         const float4* __restrict__ A, const uint4* __restrict__ X, const float4* __restrict__ B,
+         const float4* __restrict__ A, const XB* __restrict__ R,
          const unsigned* __restrict__ K, const int* __restrict__ lbF,
-         const float4* __restrict__ WA, const uint4* __restrict__ WX, const float4* __restrict__ WB,
+         const float4* __restrict__ WA, const XB* __restrict__ WR,
          const int* __restrict__ lbW, const unsigned char* __restrict__ wnear,
-         float4* __restrict__ Bout, float* __restrict__ SIG, float* __restrict__ DRHO) {
+         XB* __restrict__ Rout, float* __restrict__ SIG, float* __restrict__ DRHO) {
   __shared__ unsigned qs[QCAP * PB];
   unsigned* q = qs + threadIdx.x;
   const int i0 = blockIdx.x * PB + threadIdx.x;
   const bool act = i0 < nf;
   const int i = act ? i0 : nf - 1;
   const float4 ai = A[i];
-  const uint4 xi = X[i];
-  const float4 bi = B[i];
+  const uint4 xi = R[i].x;
+  const float4 bi = R[i].b;
   const unsigned key = K[i];
   int cx, cy, cz;
   cell_of_key(p, key, cx, cy, cz);
@@ -223,7 +229,7 @@ k_pass_a(const DP p, const SS* __restrict__ S, const int nf, const int init,
   float sg = 0.f, sc = 0.f;  // compensated sum of W/alpha (DESIGN.md §4 "precision")
   float acc = 0.f;
   {
-    auto body = make_body(X, B, [&](const uint4& xj, const float4& bj) {
+    auto body = make_body(R, [&](const uint4& xj, const float4& bj) {
     const Geo g = geometry<DIM>(p, xi, xj);
     { const float y = g.w - sc, t = sg + y; sc = (t - sg) - y; sg = t; }
     const float vd = fmaf(bi.z - bj.z, g.dz, fmaf(bi.y - bj.y, g.dy, (bi.x - bj.x) * g.dx));
@@ -231,13 +237,13 @@ k_pass_a(const DP p, const SS* __restrict__ S, const int nf, const int init,
       // equal c: (U* - U_L)(Z_L + Z_R) = c (rho_j v_ij.e + c (rho_i - rho_j)) with p = c^2 (rho - rho0)
       const float rhoj = rho0i + bj.w;
       const float num = fmaf(rhoj, vd, (ci * (bi.w - bj.w)) * g.r);
-      acc = fmaf(g.f, __fdividef(num, rhoj * (rhoi + rhoj)), acc);
+      acc = fmaf(g.f, div_fast(num, rhoj * (rhoi + rhoj)), acc);
     } else {
       const int phj = phase_of(xj);
       const float rhoj = p.rho0[phj] + bj.w, ZR = rhoj * p.c0[phj];
       const float dpr = phj == phi ? c2i * (bi.w - bj.w) : prsi - p.c2[phj] * bj.w;
       const float num = fmaf(ZR, vd, dpr * g.r);  // (U* - U_L) W' (Z_L + Z_R) / (W'/r), units of Q
-      acc = fmaf(p.mass[phj] * g.f, __fdividef(num, rhoj * (ZL + ZR)), acc);
+      acc = fmaf(p.mass[phj] * g.f, div_fast(num, rhoj * (ZL + ZR)), acc);
     }
     });
     walk_q<DIM, EXACT>(p, A, lbF, act, ai, cx, cy, cz, q, body);
@@ -245,14 +251,14 @@ k_pass_a(const DP p, const SS* __restrict__ S, const int nf, const int init,
   float accw = 0.f;
   if (__any_sync(FULL, act && wnear[key])) {
     {
-      auto body = make_body(WX, WB, [&](const uint4& xj, const float4& bj) {  // (v_w, p_w)
+      auto body = make_body(WR, [&](const uint4& xj, const float4& bj) {  // (v_w, p_w)
       const Geo g = geometry<DIM>(p, xi, xj);
       { const float y = g.w - sc, t = sg + y; sc = (t - sg) - y; sg = t; }
       const float rhow = fmaf(bj.w, p.inv_c2[phi], rho0i);  // reading A5
       const float ZR = rhow * ci;
       const float vd = fmaf(bi.z - bj.z, g.dz, fmaf(bi.y - bj.y, g.dy, (bi.x - bj.x) * g.dx));
       const float num = fmaf(ZR, vd, (prsi - bj.w) * g.r);
-      accw = fmaf(g.f, __fdividef(num, ZL + ZR), accw);
+      accw = fmaf(g.f, div_fast(num, ZL + ZR), accw);
       });
       walk_q<DIM, EXACT>(p, WA, lbW, act, ai, cx, cy, cz, q, body);
     }
@@ -268,7 +274,7 @@ k_pass_a(const DP p, const SS* __restrict__ S, const int nf, const int init,
     if ((p.fs_mask >> phi) & 1u) d = fmaf(S->dt, drho, d);  // Eq. 2.21
     else d = rho0i * dev;                                   // Eq. 2.4 / 2.18
   }
-  Bout[i] = make_float4(bi.x, bi.y, bi.z, d);
+  Rout[i] = XB{xi, make_float4(bi.x, bi.y, bi.z, d)};
   SIG[i] = dev;
   DRHO[i] = drho;
 }
@@ -280,9 +286,9 @@ k_pass_a(const DP p, const SS* __restrict__ S, const int nf, const int init,
 template <int DIM, bool MULTI, bool EXACT>
 __global__ void __launch_bounds__(PB)
 k_pass_b(const DP p, const SS* __restrict__ S, const int nf,
-         const float4* __restrict__ A, const uint4* __restrict__ X, const float4* __restrict__ B,
+         const float4* __restrict__ A, const XB* __restrict__ R,
          const unsigned* __restrict__ K, const int* __restrict__ lbF,
-         const float4* __restrict__ WA, const uint4* __restrict__ WX, const float4* __restrict__ WB,
+         const float4* __restrict__ WA, const XB* __restrict__ WR,
          const float4* __restrict__ WN, const int* __restrict__ lbW,
          const unsigned char* __restrict__ wnear, float4* __restrict__ Bout, float4* __restrict__ ACC) {
   __shared__ unsigned qs[QCAP * PB];
@@ -291,8 +297,8 @@ k_pass_b(const DP p, const SS* __restrict__ S, const int nf,
   const bool act = i0 < nf;
   const int i = act ? i0 : nf - 1;
   const float4 ai = A[i];
-  const uint4 xi = X[i];
-  const float4 bi = B[i];
+  const uint4 xi = R[i].x;
+  const float4 bi = R[i].b;
   const unsigned key = K[i];
   int cx, cy, cz;
   cell_of_key(p, key, cx, cy, cz);
@@ -301,7 +307,7 @@ k_pass_b(const DP p, const SS* __restrict__ S, const int nf,
   const float rhoi = rho0i + bi.w, prsi = c2i * bi.w, ZL = rhoi * ci;
   float ax = 0.f, ay = 0.f, az = 0.f;
   {
-    auto body = make_body(X, B, [&](const uint4& xj, const float4& bj) {
+    auto body = make_body(R, [&](const uint4& xj, const float4& bj) {
     const Geo g = geometry<DIM>(p, xi, xj);
     const float vd = fmaf(bi.z - bj.z, g.dz, fmaf(bi.y - bj.y, g.dy, (bi.x - bj.x) * g.dx));
     const float dU = -vd * g.rinv;  // U_L - U_R
@@ -311,15 +317,15 @@ k_pass_b(const DP p, const SS* __restrict__ S, const int nf,
       const float rhoj = rho0i + bj.w, prsj = c2i * bj.w;
       const float beta = fminf(3.0f * fmaxf(dU, 0.f), ci);
       const float num = fmaf(rhoi * rhoj, beta * dU, fmaf(rhoi, prsj, rhoj * prsi));
-      coef = g.f * __fdividef(num, (rhoi + rhoj) * rhoj);
+      coef = g.f * div_fast(num, (rhoi + rhoj) * rhoj);
     } else {
       const int phj = phase_of(xj);
       const float rhoj = p.rho0[phj] + bj.w, prsj = p.c2[phj] * bj.w, ZR = rhoj * p.c0[phj];
-      const float izs = __fdividef(1.0f, ZL + ZR);
-      const float ctil = (ZL + ZR) * __fdividef(1.0f, rhoi + rhoj);
+      const float izs = div_fast(1.0f, ZL + ZR);
+      const float ctil = (ZL + ZR) * div_fast(1.0f, rhoi + rhoj);
       const float beta = fminf(3.0f * fmaxf(dU, 0.f), ctil);
-      const float pstar = fmaf(ZL, prsj, ZR * prsi) * izs + ZL * ZR * izs * __fdividef(beta, ctil) * dU;
-      coef = g.f * __fdividef(p.mass[phj] * pstar, rhoj);
+      const float pstar = fmaf(ZL, prsj, ZR * prsi) * izs + ZL * ZR * izs * div_fast(beta, ctil) * dU;
+      coef = g.f * div_fast(p.mass[phj] * pstar, rhoj);
     }
     ax = fmaf(coef, g.dx, ax); ay = fmaf(coef, g.dy, ay); az = fmaf(coef, g.dz, az);
     });
@@ -329,11 +335,11 @@ k_pass_b(const DP p, const SS* __restrict__ S, const int nf,
   if (__any_sync(FULL, act && wnear[key])) {
     const bool pen = (p.pen_mask >> phi) & 1u;
     {
-      auto body = make_body(WX, WB, [&](const uint4& xj, const float4& bj) {
+      auto body = make_body(WR, [&](const uint4& xj, const float4& bj) {
       const float pw = bj.w;
       const Geo g = geometry<DIM>(p, xi, xj);
       const float rhow = fmaf(pw, p.inv_c2[phi], rho0i);
-      const float pstar = __fdividef(fmaf(rhoi, pw, rhow * prsi), rhoi + rhow);  // Eq. 2.11
+      const float pstar = div_fast(fmaf(rhoi, pw, rhow * prsi), rhoi + rhow);  // Eq. 2.11
       const float coef = g.f * pstar;
       wx = fmaf(coef, g.dx, wx); wy = fmaf(coef, g.dy, wy); wz = fmaf(coef, g.dz, wz);
       if (pen) {
