@@ -288,7 +288,7 @@ def run_gpu(args):
                       "frac_with_candidates": (fl + CAND_FLOPS * cands) / t / 1e12 / peak}
     # HBM-bound stages: algorithmic bytes per fluid particle
     hbm = _peaks().get("hbm_gbs", 6650.0)
-    bytes_pp = {"predict": 148.0, "sort": 16.0 * 2 * g_sort_passes(g), "reorder": 156.0}
+    bytes_pp = {"predict": 108.0, "sort": (16.0 + 4.0) * g_sort_passes(g), "reorder": 92.0}
     for name, b in bytes_pp.items():
         t = stage_ms[name] * 1e-3
         if t > 0:
@@ -296,7 +296,7 @@ def run_gpu(args):
     dom = max(("pass_a", "pass_b"), key=lambda k: stage_ms[k])
     roofline = {"bound": "alu", "kernel": "k_" + dom, "achieved": kern[dom]["tflops_hit_only"],
                 "peak": peak, "unit": "TFLOP/s", "frac": kern[dom]["frac_hit_only"], "traffic": None,
-                "peak_source": "148 SM x 128 FP32 lanes x 2 x clocks.max.sm (DESIGN.md §7), not measured",
+                "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 flop x clocks.max.sm (DESIGN.md §7); MEASURED_PEAKS.json holds no non-tensor FP32 peak",
                 "achieved_with_candidates": kern[dom]["tflops_with_candidates"],
                 "frac_with_candidates": kern[dom]["frac_with_candidates"],
                 "flops_per_hit": FLOPS_HIT[dom], "flops_per_candidate": CAND_FLOPS}
