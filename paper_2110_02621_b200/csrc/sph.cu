@@ -320,7 +320,7 @@ int sph_create(const sph_params* prm, sph_ctx** out) {
       }
     }
     d.sub_per_m = 1024.0 / d.Q;
-    d.Qf = (float)d.Q; d.qh = (float)(d.Q / h);
+    d.Qf = (float)d.Q; d.qh = (float)(d.Q / h); d.qhD = d.Q / h;
     d.gradcQ = (float)(-5.0 * alpha / (h * h) * d.Q);
     d.two_over_dp = (float)(2.0 * d.Q / dp);
     // candidate filter margin: rounding of the expanded form |xj|^2 - 2 xi.xj + |xi|^2 on images
@@ -423,7 +423,6 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
     rc = radix_sort(c, st, nw, c->keyA, c->valA, c->keyB, c->valB, &ks, &vs);
     if (rc) { cudaFree(idx); return rc; }
     LAUNCH(k_reorder, cdiv(nw, 256), 256, st, c->dp, nw, vs, c->TX, c->TB, c->ID0, c->WR, c->WA, c->WID);
-    LAUNCH(k_wall_selfidx, cdiv(nw, 256), 256, st, nw, c->WR);
     CK(cudaMemcpyAsync(c->WK, ks, sizeof(unsigned) * nw, cudaMemcpyDeviceToDevice, st));
     LAUNCH(k_image, cdiv(nw, 256), 256, st, c->dp, nw, c->WR, c->WG);
     LAUNCH(k_cell_bounds, cdiv(c->ncell + 1, 256), 256, st, ks, nw, (int)c->ncell, c->lbW);

@@ -17,10 +17,11 @@ __global__ void k_load(DP p, int n, int is_wall, const int* __restrict__ idx, co
   const int o = idx[i];
   const int ph = is_wall ? 0 : tag[o];
   uint4 x;
-  x.x = fx_from_double((double)pos[3 * o], p.O[0], p.Q);
-  x.y = fx_from_double((double)pos[3 * o + 1], p.O[1], p.Q);
-  x.z = p.dim == 3 ? fx_from_double((double)pos[3 * o + 2], p.O[2], p.Q) : 0u;
-  x.w = RES_MID | (unsigned)ph;
+  unsigned rx, ry, rz = 512u;
+  x.x = fx_from_double((double)pos[3 * o], p.O[0], p.Q, rx);
+  x.y = fx_from_double((double)pos[3 * o + 1], p.O[1], p.Q, ry);
+  x.z = p.dim == 3 ? fx_from_double((double)pos[3 * o + 2], p.O[2], p.Q, rz) : 0u;
+  x.w = (rx << 22) | (ry << 12) | (rz << 2) | (unsigned)ph;
   TX[i] = x;
   if (is_wall) {
     TB[i] = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -215,11 +216,4 @@ __global__ void k_wnear(DP p, int ncell, const int* __restrict__ lbW, unsigned c
       any |= lbW[rb + min(cx + 1, p.nx - 1) + 1] > lbW[rb + max(cx - 1, 0)];
     }
   wnear[c] = (unsigned char)any;
-}
-
-// Walls are static and single-"phase": their X4.w carries the particle's own sorted index instead
-// (lets a pair body reach per-wall data such as the normal from the gathered position alone).
-__global__ void k_wall_selfidx(int nw, XB* __restrict__ WR) {
-  const int w = blockIdx.x * blockDim.x + threadIdx.x;
-  if (w < nw) WR[w].x.w = (unsigned)w;
 }

@@ -32,7 +32,7 @@ struct DP {
   int nx, ny, nz;
   float dmin[3], dmax[3];
   double O[3], C[3], Q, sub_per_m;  // fixed point: origin, image centre, quantum, 1024 / Q
-  double cmax, cfl, hD, dpD;
+  double cmax, cfl, hD, dpD, qhD;  // qhD = Q / h
   double massD[SPH_MAX_PHASES];
   double a_over_s0;
   double g[3], gamp[3], gperiod;
@@ -86,10 +86,17 @@ __device__ __forceinline__ float warp_sum(float v) {
 }
 
 // ---- fixed-point master positions ---------------------------------------------------------
-__device__ __forceinline__ unsigned fx_from_double(double x, double O, double Q) {
-  double u = rint((x - O) / Q);
-  u = fmin(fmax(u, 0.0), 4294967295.0);  // saturate (escaped particles); NaN -> 0
-  return (unsigned)u;
+// x -> (X, residual): the position in units of Q/1024 rounded to an integer, split into the 32-bit
+// fixed-point word and the 10-bit residual (biased by 512).  Saturates outside the span; NaN -> 0.
+__device__ __forceinline__ unsigned fx_from_double(double x, double O, double Q, unsigned& res) {
+  double u = rint((x - O) / Q * 1024.0);
+  u = fmin(fmax(u, 0.0), 4294967295.0 * 1024.0);
+  const long long tot = (long long)u;
+  long long X = (tot + 512) >> 10;
+  if (X > 4294967295ll) X = 4294967295ll;
+  res = (unsigned)(tot - (X << 10) + 512);
+  if (res > 1023u) res = 512u;
+  return (unsigned)X;
 }
 __device__ __forceinline__ double fx_to_double(unsigned X, double O, double Q) {
   return fma((double)X, Q, O);  // exact: Q is a power of two, O a multiple of Q

@@ -97,16 +97,34 @@ __device__ __forceinline__ void walk_q(const DP& p, const float4* __restrict__ A
 // Exact pair geometry in units of Q from the fixed-point positions: d = X_i - X_j (wrapping
 // integer subtract, exact), r^2, 1/r (r = 0 -> r = 0 with a finite 1/r), q = r/h and the
 // Wendland C2 factors (reading A1): w = (1 - q/2)^4 (1 + 2q) = W / alpha_d,  f = (1 - q/2)^3.
-__device__ __forceinline__ float rsqrt_fast(float x) {  // MUFU.RSQ, no denormal fix-up (x >= 0.5 here)
+// MUFU.RSQ / MUFU.RCP are accurate to about 2^-22 and their error is a smooth function of the
+// operand, i.e. of the neighbour's distance and density: in the momentum sum, whose terms cancel to
+// 1e-3 of their size, that is a systematic bias of 1e-4 g at H / dp = 100 (measured against the oracle).
+// One Newton step each makes the error rounding-sized and random.
+__device__ __forceinline__ float rsqrt_fast(float x) {  // x >= 0.5 here: no denormal fix-up needed
   float y;
   asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-  return y;
+  const float e = fmaf(-x * y, y, 1.0f);
+  return fmaf(0.5f * y, e, y);
 }
-__device__ __forceinline__ float div_fast(float a, float b) {  // a * MUFU.RCP(b), b normal and finite here
+__device__ __forceinline__ float div_fast(float a, float b) {  // b normal and finite here
   float y;
   asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(b));
+  y = fmaf(y, fmaf(-b, y, 1.0f), y);
   return a * y;
 }
+// Compensated (Kahan) float32 accumulator.  The momentum sum cancels to O(g) from terms whose
+// partial sums reach O(g H / h): plain float32 accumulation loses 1e-4 g at H / dp = 100
+// (measured against the oracle); sigma needs 5e-7 relative for the same reason.
+struct KSum {
+  float s = 0.f, c = 0.f;
+  __device__ __forceinline__ void add(const float x) {
+    const float y = x - c, t = s + y;
+    c = (t - s) - y;
+    s = t;
+  }
+  __device__ __forceinline__ float value() const { return s - c; }
+};
 struct Geo {
   float dx, dy, dz, r, rinv, w, f;
 };
@@ -126,13 +144,47 @@ __device__ __forceinline__ Geo geometry(const DP& p, const uint4& xi, const uint
   return g;
 }
 
+// W / alpha_d in float64 from the exact integer separation (reading A1), for the number density
+// sigma_i only.  p = c0^2 rho0 (sigma/sigma0 - 1) with c0^2 = 200 g H amplifies a relative error of
+// sigma by 200, and the momentum sum amplifies a pressure error by another H / h: float32 terms
+// (2e-7 each) leave 3e-5 of rho0 g H in p and 2.5e-4 g in a at H / dp = 100 (measured against the
+// oracle).  r^2 is an exact 64-bit integer; 1/sqrt by MUFU.RSQ64H + one Newton step (1e-12).
+template <int DIM, bool SUBQ>
+__device__ __forceinline__ double w64(const DP& p, const uint4& xi, const uint4& xj) {
+  const long long dx = (int)(xi.x - xj.x), dy = (int)(xi.y - xj.y), dz = DIM == 3 ? (int)(xi.z - xj.z) : 0;
+  double r2, qs;
+  if (SUBQ) {
+    // multi-phase: include the 10-bit residuals (units of Q/1024).  For a light phase with its own
+    // large c0 (config 2b: c_air^2 = 1000 c_w^2) sigma must be good to 1e-11, i.e. positions to 1e-12 m.
+    const double ex = (double)((dx << 10) + (int)((xi.w >> 22) & 1023u) - (int)((xj.w >> 22) & 1023u));
+    const double ey = (double)((dy << 10) + (int)((xi.w >> 12) & 1023u) - (int)((xj.w >> 12) & 1023u));
+    const double ez = DIM == 3 ? (double)((dz << 10) + (int)((xi.w >> 2) & 1023u) - (int)((xj.w >> 2) & 1023u)) : 0.0;
+    r2 = fma(ez, ez, fma(ey, ey, ex * ex));
+    qs = p.qhD * (1.0 / 1024.0);
+  } else {
+    r2 = (double)(dx * dx + dy * dy + dz * dz);
+    qs = p.qhD;
+  }
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(r2));
+  const double e = fma(-r2 * y, y, 1.0);
+  y = fma(0.5 * y, e, y);
+  const double q = r2 > 0.0 ? r2 * y * qs : 0.0;
+  const double t = fmax(fma(-0.5, q, 1.0), 0.0), t2 = t * t;
+  return t2 * t2 * fma(2.0, q, 1.0);
+}
+
 // Pair body = the neighbour's record (one 256-bit gather) + the arithmetic on it.
+struct LdXB {
+  XB r;
+  unsigned j;
+};
 template <class F>
 struct BodyXB {
   const XB* __restrict__ R;
   F f;
-  __device__ __forceinline__ XB load(const unsigned j) const { return ldg256(R + j); }
-  __device__ __forceinline__ void apply(const XB& l) { f(l.x, l.b); }
+  __device__ __forceinline__ LdXB load(const unsigned j) const { return LdXB{ldg256(R + j), j}; }
+  __device__ __forceinline__ void apply(const LdXB& l) { f(l.r.x, l.r.b, l.j); }
 };
 template <class F>
 __device__ __forceinline__ BodyXB<F> make_body(const XB* R, F f) { return BodyXB<F>{R, f}; }
@@ -164,7 +216,7 @@ k_wall(const DP p, const SS* __restrict__ S, const int nw, const float4* __restr
   cell_of_key(p, WK[w], cx, cy, cz);
   float sW = 0, sp = 0, sWr = 0, srx = 0, sry = 0, srz = 0, svx = 0, svy = 0, svz = 0;
   {
-    auto body = make_body(R, [&](const uint4& xj, const float4& bj) {
+    auto body = make_body(R, [&](const uint4& xj, const float4& bj, const unsigned j) {
     const Geo g = geometry<DIM>(p, xi, xj);  // r_wf = r_w - r_f
     const int ph = MULTI ? phase_of(xj) : 0;
     const float rhof = p.rho0[ph] + bj.w, pf = p.c2[ph] * bj.w;
@@ -226,12 +278,12 @@ k_pass_a(const DP p, const SS* __restrict__ S, const int nf, const int init,
   const int phi = MULTI ? phase_of(xi) : 0;
   const float rho0i = p.rho0[phi], c2i = p.c2[phi], ci = p.c0[phi];
   const float rhoi = rho0i + bi.w, prsi = c2i * bi.w, ZL = rhoi * ci;
-  float sg = 0.f, sc = 0.f;  // compensated sum of W/alpha (DESIGN.md §4 "precision")
+  double sig = 0.0;  // sum of W/alpha in float64 (DESIGN.md §4 "precision")
   float acc = 0.f;
   {
-    auto body = make_body(R, [&](const uint4& xj, const float4& bj) {
+    auto body = make_body(R, [&](const uint4& xj, const float4& bj, const unsigned j) {
     const Geo g = geometry<DIM>(p, xi, xj);
-    { const float y = g.w - sc, t = sg + y; sc = (t - sg) - y; sg = t; }
+    sig += w64<DIM, MULTI>(p, xi, xj);
     const float vd = fmaf(bi.z - bj.z, g.dz, fmaf(bi.y - bj.y, g.dy, (bi.x - bj.x) * g.dx));
     if (!MULTI) {
       // equal c: (U* - U_L)(Z_L + Z_R) = c (rho_j v_ij.e + c (rho_i - rho_j)) with p = c^2 (rho - rho0)
@@ -251,9 +303,9 @@ k_pass_a(const DP p, const SS* __restrict__ S, const int nf, const int init,
   float accw = 0.f;
   if (__any_sync(FULL, act && wnear[key])) {
     {
-      auto body = make_body(WR, [&](const uint4& xj, const float4& bj) {  // (v_w, p_w)
+      auto body = make_body(WR, [&](const uint4& xj, const float4& bj, const unsigned j) {  // (v_w, p_w)
       const Geo g = geometry<DIM>(p, xi, xj);
-      { const float y = g.w - sc, t = sg + y; sc = (t - sg) - y; sg = t; }
+      sig += w64<DIM, MULTI>(p, xi, xj);
       const float rhow = fmaf(bj.w, p.inv_c2[phi], rho0i);  // reading A5
       const float ZR = rhow * ci;
       const float vd = fmaf(bi.z - bj.z, g.dz, fmaf(bi.y - bj.y, g.dy, (bi.x - bj.x) * g.dx));
@@ -264,9 +316,9 @@ k_pass_a(const DP p, const SS* __restrict__ S, const int nf, const int init,
     }
   }
   if (!act) return;
-  // sigma_i / sigma0 - 1 in float64 from the compensated sum, stored as float32: the density of
+  // sigma_i / sigma0 - 1 in float64, stored as float32: the density of
   // Eq. 2.17 / 2.18 is rho0 (1 + dev), so the deviation carries the precision.
-  const float dev = (float)(p.a_over_s0 * ((double)sg - (double)sc) - 1.0);
+  const float dev = (float)(p.a_over_s0 * sig - 1.0);
   const float accf = MULTI ? acc : p.mass[0] * acc;
   const float drho = 2.0f * rhoi * p.gradcQ * fmaf(p.V0, accw, accf);  // Eq. 2.9
   float d = bi.w;
@@ -305,9 +357,9 @@ k_pass_b(const DP p, const SS* __restrict__ S, const int nf,
   const int phi = MULTI ? phase_of(xi) : 0;
   const float rho0i = p.rho0[phi], c2i = p.c2[phi], ci = p.c0[phi];
   const float rhoi = rho0i + bi.w, prsi = c2i * bi.w, ZL = rhoi * ci;
-  float ax = 0.f, ay = 0.f, az = 0.f;
+  KSum ax, ay, az;
   {
-    auto body = make_body(R, [&](const uint4& xj, const float4& bj) {
+    auto body = make_body(R, [&](const uint4& xj, const float4& bj, const unsigned j) {
     const Geo g = geometry<DIM>(p, xi, xj);
     const float vd = fmaf(bi.z - bj.z, g.dz, fmaf(bi.y - bj.y, g.dy, (bi.x - bj.x) * g.dx));
     const float dU = -vd * g.rinv;  // U_L - U_R
@@ -327,23 +379,25 @@ k_pass_b(const DP p, const SS* __restrict__ S, const int nf,
       const float pstar = fmaf(ZL, prsj, ZR * prsi) * izs + ZL * ZR * izs * div_fast(beta, ctil) * dU;
       coef = g.f * div_fast(p.mass[phj] * pstar, rhoj);
     }
-    ax = fmaf(coef, g.dx, ax); ay = fmaf(coef, g.dy, ay); az = fmaf(coef, g.dz, az);
+    ax.add(coef * g.dx); ay.add(coef * g.dy);
+    if (DIM == 3) az.add(coef * g.dz);
     });
     walk_q<DIM, EXACT>(p, A, lbF, act, ai, cx, cy, cz, q, body);
   }
-  float wx = 0.f, wy = 0.f, wz = 0.f;
+  KSum wx, wy, wz;
   if (__any_sync(FULL, act && wnear[key])) {
     const bool pen = (p.pen_mask >> phi) & 1u;
     {
-      auto body = make_body(WR, [&](const uint4& xj, const float4& bj) {
+      auto body = make_body(WR, [&](const uint4& xj, const float4& bj, const unsigned j) {
       const float pw = bj.w;
       const Geo g = geometry<DIM>(p, xi, xj);
       const float rhow = fmaf(pw, p.inv_c2[phi], rho0i);
       const float pstar = div_fast(fmaf(rhoi, pw, rhow * prsi), rhoi + rhow);  // Eq. 2.11
       const float coef = g.f * pstar;
-      wx = fmaf(coef, g.dx, wx); wy = fmaf(coef, g.dy, wy); wz = fmaf(coef, g.dz, wz);
+      wx.add(coef * g.dx); wy.add(coef * g.dy);
+      if (DIM == 3) wz.add(coef * g.dz);
       if (pen) {
-        const float4 n = __ldg(WN + xj.w);  // wall X4.w holds the wall particle's own sorted index
+        const float4 n = __ldg(WN + j);
         if (n.x != 0.f || n.y != 0.f || n.z != 0.f) {
           const float nd = n.x * g.dx + n.y * g.dy + n.z * g.dz;  // n_w . (r_i - r_w) / Q
           const float delta = nd * p.two_over_dp;                  // Eq. 2.15 (reading A9); two_over_dp holds 2 Q / dp
@@ -351,7 +405,8 @@ k_pass_b(const DP p, const SS* __restrict__ S, const int nf,
             const float lam = (1.0f - delta) * (1.0f - delta);     // Eq. 2.14 (reading A8)
             const float Pn = p.gamma_p * lam * fabsf(prsi * nd * g.rinv);
             const float c = Pn * g.f * g.r;                        // Eq. 2.13, W' = (W'/r) r
-            wx = fmaf(c, n.x, wx); wy = fmaf(c, n.y, wy); wz = fmaf(c, n.z, wz);
+            wx.add(c * n.x); wy.add(c * n.y);
+            if (DIM == 3) wz.add(c * n.z);
           }
         }
       }
@@ -362,10 +417,13 @@ k_pass_b(const DP p, const SS* __restrict__ S, const int nf,
   if (!act) return;
   const float sf = -2.0f * p.gradcQ / rhoi * (MULTI ? 1.0f : p.mass[0]);  // Eq. 2.10
   const float sw = -2.0f * p.gradcQ / rhoi * p.V0;
-  ax = fmaf(sf, ax, fmaf(sw, wx, S->g[0]));
-  ay = fmaf(sf, ay, fmaf(sw, wy, S->g[1]));
-  az = DIM == 3 ? fmaf(sf, az, fmaf(sw, wz, S->g[2])) : 0.f;
-  ACC[i] = make_float4(ax, ay, az, 0.f);
+  // a = g + sf * fluid sum + sw * wall sum, combined in float64 once per particle (the two sums
+  // nearly cancel against g in a resting column)
+  const double sfd = (double)sf, swd = (double)sw;
+  const float fx = (float)((double)S->g[0] + sfd * ((double)ax.s - (double)ax.c) + swd * ((double)wx.s - (double)wx.c));
+  const float fy = (float)((double)S->g[1] + sfd * ((double)ay.s - (double)ay.c) + swd * ((double)wy.s - (double)wy.c));
+  const float fz = DIM == 3 ? (float)((double)S->g[2] + sfd * ((double)az.s - (double)az.c) + swd * ((double)wz.s - (double)wz.c)) : 0.f;
+  ACC[i] = make_float4(fx, fy, fz, 0.f);
   const float hdt = 0.5f * S->dt;
-  Bout[i] = make_float4(fmaf(hdt, ax, bi.x), fmaf(hdt, ay, bi.y), fmaf(hdt, az, bi.z), bi.w);  // Eq. 2.22
+  Bout[i] = make_float4(fmaf(hdt, fx, bi.x), fmaf(hdt, fy, bi.y), fmaf(hdt, fz, bi.z), bi.w);  // Eq. 2.22
 }
