@@ -248,14 +248,11 @@ def run_gpu(args):
     launches = g.launch_count() - l0
     clocks = sampler.stop()
     ms = float(sum(a.elapsed_time(b) for a, b in ev))
-    if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, "cuda")
     st = g.get_stats()
     if st["escaped"] or st["nonfinite"]:
         raise SystemExit("bench run went bad: %r" % (st,))
-    value = world * nfl * K / (ms * 1e-3)
+    value = whole_job_rate(nfl * K, world, ms * 1e-3)
     pairs_s = world * st["npairs"] * K / (ms * 1e-3)
 
     # ---- per-stage times (CUDA events recorded by the library on the same stream) ---------------
@@ -320,10 +317,7 @@ def run_gpu(args):
     g2.get_fields_into_host(pos=out["pos"].numpy(), vel=out["vel"].numpy(), rho=out["rho"].numpy())
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = max_over_ranks(e2e_s, "cuda")
     h2d = (n * (12 + 12 + 4 + 4)) / KE
     d2h = (n * 4 + n * (12 + 12 + 4)) / KE + 88      # tag read-back + fields, + sph_stats per step
     e2e = {"value": world * nfl * KE / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d,
@@ -355,6 +349,23 @@ def run_gpu(args):
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
+
+
+def max_over_ranks(value, device=None):
+    """Replicas-only multi-GPU timing rule: every rank times its own replica, the job time is the
+    max over ranks (torch.distributed all_reduce MAX; backend nccl on GPUs, gloo in the CPU test)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(value)
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device or "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_rate(units_per_rank, world, seconds):
+    """value of the JSON line: units processed by all replicas / max-over-ranks time."""
+    return world * units_per_rank / seconds
 
 
 def _neighbour_counts(g):
