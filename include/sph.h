@@ -130,6 +130,9 @@ int sph_get_fields_host(sph_ctx* ctx, float* pos_host, float* vel_host, float* r
 /* Integral quantities; runs small reduction kernels and synchronises.  Returns SPH_ENONFINITE /
  * SPH_EDTUNDERFLOW (with *out filled) if the run has gone bad. */
 int sph_get_stats(sph_ctx* ctx, sph_stats* out, void* stream);
+/* Same; with_pairs = 0 skips the contract-exact pair count (a full stencil walk, as expensive as a
+ * pair pass) and returns n_pairs = -1: the per-step monitoring call (t, dt, E_k, mass, x_front). */
+int sph_get_stats_ex(sph_ctx* ctx, sph_stats* out, int32_t with_pairs, void* stream);
 
 /* Per-stage device times.  With profiling on, sph_step brackets every stage with CUDA events
  * on the caller's stream; sph_get_timings synchronises and returns the accumulated milliseconds

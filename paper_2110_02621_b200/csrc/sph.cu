@@ -524,7 +524,9 @@ int sph_get_fields_host(sph_ctx* c, float* pos, float* vel, float* rho, float* p
   return SPH_OK;
 }
 
-int sph_get_stats(sph_ctx* c, sph_stats* out, void* stream) {
+int sph_get_stats(sph_ctx* c, sph_stats* out, void* stream) { return sph_get_stats_ex(c, out, 1, stream); }
+
+int sph_get_stats_ex(sph_ctx* c, sph_stats* out, int32_t with_pairs, void* stream) {
   if (!c || !out) return SPH_EINVAL;
   if (!c->loaded) { c->err = "no particles"; return SPH_EINVAL; }
   cudaStream_t st = (cudaStream_t)stream;
@@ -534,16 +536,18 @@ int sph_get_stats(sph_ctx* c, sph_stats* out, void* stream) {
   const int nf = (int)c->nf;
   if (nf) {
     LAUNCH(k_stats, std::min(cdiv(nf, 256), 1184), 256, st, c->dp, nf, c->R1, c->TB, c->stat);
-    const float4* G = fluid_images(c, st);
-    LAUNCH(k_neigh, cdiv(nf, PW), PW * 32, st, c->dp, nf, 0, 0, G, c->IDcur, G, c->IDcur, c->lbF, c->WG,
-           c->WID, c->lbW, (int*)nullptr, (const long long*)nullptr, (int*)nullptr, 0ll, &c->stat->pairs);
+    if (with_pairs) {
+      const float4* G = fluid_images(c, st);
+      LAUNCH(k_neigh, cdiv(nf, PW), PW * 32, st, c->dp, nf, 0, 0, G, c->IDcur, G, c->IDcur, c->lbF, c->WG,
+             c->WID, c->lbW, (int*)nullptr, (const long long*)nullptr, (int*)nullptr, 0ll, &c->stat->pairs);
+    }
   }
   SS hs;
   CK(cudaMemcpyAsync(&z, c->stat, sizeof(z), cudaMemcpyDeviceToHost, st));
   CK(cudaMemcpyAsync(&hs, c->S, sizeof(hs), cudaMemcpyDeviceToHost, st));
   CK(cudaStreamSynchronize(st));
   out->t = hs.t; out->dt = hs.dt_d; out->steps = hs.steps; out->n_fluid = c->nf; out->n_wall = c->nw;
-  out->n_pairs = (int64_t)z.pairs; out->e_kin = z.ek;
+  out->n_pairs = with_pairs ? (int64_t)z.pairs : -1; out->e_kin = z.ek;
   out->mass = 0.0;
   for (int k = 0; k < SPH_MAX_PHASES; ++k) out->mass += (double)z.count[k] * c->dp.massD[k];
   {

@@ -46,7 +46,7 @@ class SphStats(C.Structure):
 
 EXPORTS = (
     "sph_create", "sph_destroy", "sph_set_particles", "sph_set_particles_host", "sph_step",
-    "sph_step_dt", "sph_get_fields", "sph_get_fields_host", "sph_get_stats", "sph_set_profiling",
+    "sph_step_dt", "sph_get_fields", "sph_get_fields_host", "sph_get_stats", "sph_get_stats_ex", "sph_set_profiling",
     "sph_get_timings", "sph_num_cells", "sph_debug_cells", "sph_debug_neighbours",
     "sph_debug_normals", "sph_debug_sigma", "sph_launch_count", "sph_last_error",
 )
@@ -73,6 +73,7 @@ def load():
     for name in ("sph_get_fields", "sph_get_fields_host"):
         f = getattr(L, name); f.restype = C.c_int; f.argtypes = [vp] * 7
     L.sph_get_stats.restype = C.c_int; L.sph_get_stats.argtypes = [vp, C.POINTER(SphStats), vp]
+    L.sph_get_stats_ex.restype = C.c_int; L.sph_get_stats_ex.argtypes = [vp, C.POINTER(SphStats), i32, vp]
     L.sph_set_profiling.restype = C.c_int; L.sph_set_profiling.argtypes = [vp, i32]
     L.sph_get_timings.restype = C.c_int; L.sph_get_timings.argtypes = [vp, vp, vp]
     L.sph_num_cells.restype = i64; L.sph_num_cells.argtypes = [vp]
@@ -191,9 +192,9 @@ class Sph:
         self._ck(self.L.sph_get_fields_host(self.ctx, _hp(pos), _hp(vel), _hp(rho), _hp(p), _hp(acc), self._st()))
 
     # -- sph_get_stats ---------------------------------------------------------------------------
-    def get_stats(self, check=True):
+    def get_stats(self, check=True, with_pairs=True):
         s = SphStats()
-        rc = self.L.sph_get_stats(self.ctx, C.byref(s), self._st())
+        rc = self.L.sph_get_stats_ex(self.ctx, C.byref(s), 1 if with_pairs else 0, self._st())
         if check:
             self._ck(rc)
         return dict(t=s.t, dt=s.dt, steps=s.steps, n_fluid=s.n_fluid, n_wall=s.n_wall, npairs=s.n_pairs,
