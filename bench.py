@@ -41,6 +41,14 @@ UNIT = "fluid particle-steps/s"
 # separately (CAND_FLOPS each) because they are overhead of the 27-cell walk, not of the method.
 FLOPS_HIT = {"pass_a": 40.0, "pass_b": 50.0, "wall": 30.0}
 CAND_FLOPS = 8.0
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from `ncu --set full` captures of these
+# exact workloads (profiles/r01b_README.md); other workloads report traffic = null.
+NCU_TRAFFIC_BYTES = {
+    ("cfg1_dam_break_3d_box", "k_pass_a"): 40.48e6 + 3.13e6,
+    ("cfg1_dam_break_3d_box", "k_pass_b"): 42.09e6 + 3.08e6,
+    ("cfg4_box_160", "k_pass_a"): 237.4e6 + 140.3e6,
+    ("cfg4_box_160", "k_pass_b"): 244.0e6 + 110.4e6,
+}
 FP32_LANES_PER_SM = 128
 N_SM = 148
 
@@ -292,7 +300,8 @@ def run_gpu(args):
             kern[name] = {"ms": 1e3 * t, "gbs": b * nfl / t / 1e9, "frac_hbm": b * nfl / t / 1e9 / hbm}
     dom = max(("pass_a", "pass_b"), key=lambda k: stage_ms[k])
     roofline = {"bound": "alu", "kernel": "k_" + dom, "achieved": kern[dom]["tflops_hit_only"],
-                "peak": peak, "unit": "TFLOP/s", "frac": kern[dom]["frac_hit_only"], "traffic": None,
+                "peak": peak, "unit": "TFLOP/s", "frac": kern[dom]["frac_hit_only"],
+                "traffic": NCU_TRAFFIC_BYTES.get((cfg["name"], "k_" + dom)),
                 "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 flop x clocks.max.sm (DESIGN.md §7); MEASURED_PEAKS.json holds no non-tensor FP32 peak",
                 "achieved_with_candidates": kern[dom]["tflops_with_candidates"],
                 "frac_with_candidates": kern[dom]["frac_with_candidates"],
