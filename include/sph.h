@@ -45,7 +45,9 @@ enum sph_error {
   SPH_ENOMEM = -2,      /* device or host allocation failed */
   SPH_ECUDA = -3,       /* CUDA runtime error (no device, launch failure, ...) */
   SPH_ENONFINITE = -4,  /* a non-finite position or velocity was seen (reported by sph_get_stats) */
-  SPH_EDTUNDERFLOW = -5 /* the time step fell below 1e-12 (reported by sph_get_stats) */
+  SPH_EDTUNDERFLOW = -5, /* the time step fell below 1e-12 (reported by sph_get_stats) */
+  SPH_ENEIGHBOURS = -6   /* a particle had more neighbours than max_neighbours (reported by sph_get_stats);
+                            the step results are then incomplete */
 };
 
 /* Physical and numerical parameters: the paper's statement of the problem. */
@@ -65,7 +67,7 @@ typedef struct {
   uint32_t free_surface_mask;    /* bit k: phase k uses continuity Eq. 2.9/2.21 + reinit Eq. 2.17;
                                     otherwise summation Eq. 2.4 + reinit Eq. 2.18 (reading A13, A15) */
   uint32_t flags;                /* sph_flags */
-  uint32_t reserved;
+  uint32_t max_neighbours;       /* capacity of the per-particle neighbour lists; 0 = default (160 in 3-D, 64 in 2-D) */
   double domain_min[3];          /* box of the cell grid; particles outside are binned in the edge */
   double domain_max[3];          /* cells and counted as escaped (reading A23)                      */
 } sph_params;
@@ -92,7 +94,8 @@ enum sph_stage {
   SPH_STAGE_WALL = 3,      /* wall extrapolation Eq. 2.12 (both calls of a step) */
   SPH_STAGE_PASS_A = 4,    /* sigma + continuity Eq. 2.9 + density update Eq. 2.21 / 2.4 + EOS */
   SPH_STAGE_PASS_B = 5,    /* momentum Eq. 2.10/2.11 + penalty Eq. 2.13 + second kick Eq. 2.22 */
-  SPH_STAGE_COUNT = 6
+  SPH_STAGE_BUILD = 6,     /* neighbour-list build: the 27 / 9-cell candidate walk, once per step */
+  SPH_STAGE_COUNT = 7
 };
 
 /* Create a context.  Validates the parameters (SPH_EINVAL), selects the current CUDA device. */

@@ -45,6 +45,10 @@ struct sph_ctx {
   uint4* TX = nullptr;
   float4 *A = nullptr, *TB = nullptr, *ACC = nullptr;
   float *SIG = nullptr, *DRHO = nullptr;
+  unsigned* NL = nullptr;  // neighbour lists, slot-major per warp: [npad / 32][caps][32]
+  int* NC = nullptr;       // neighbours per fluid particle
+  int caps = 0;
+  size_t npad = 0;
   unsigned *ID0 = nullptr, *ID1 = nullptr, *IDcur = nullptr, *IDnext = nullptr;
   unsigned *keyA = nullptr, *valA = nullptr, *keyB = nullptr, *valB = nullptr, *hist = nullptr,
            *rowsum = nullptr;
@@ -120,7 +124,7 @@ int dalloc(sph_ctx* c, T** p, size_t count) {
 }
 
 void free_all(sph_ctx* c) {
-  void* ptrs[] = {c->R0, c->R1, c->TX, c->A, c->TB, c->ACC, c->SIG, c->DRHO, c->ID0, c->ID1,
+  void* ptrs[] = {c->R0, c->R1, c->TX, c->A, c->TB, c->ACC, c->SIG, c->DRHO, c->NL, c->NC, c->ID0, c->ID1,
                   c->keyA, c->valA, c->keyB, c->valB, c->hist, c->rowsum, c->lbF, c->lbW, c->WR,
                   c->WA, c->WN, c->WG, c->WK, c->WID, c->wnear, c->S, c->dt_seq, c->stat};
   for (void* p : ptrs)
@@ -195,15 +199,24 @@ int pipeline_after_hash(sph_ctx* c, cudaStream_t st, int init, Prof& pf) {
   launch_wall(c, st, true, c->R0);
   pf.mark();  // end wall 1
   if (nf > 0) {
+    switch (PAIR_SEL(c) & 5) {  // DIM x EXACT
+      case 0: LAUNCH((k_build<2, false>), cdiv(nf, PB), PB, st, c->dp, c->S, nf, c->A, c->K, c->lbF, c->NL, c->NC, c->caps); break;
+      case 1: LAUNCH((k_build<2, true>), cdiv(nf, PB), PB, st, c->dp, c->S, nf, c->A, c->K, c->lbF, c->NL, c->NC, c->caps); break;
+      case 4: LAUNCH((k_build<3, false>), cdiv(nf, PB), PB, st, c->dp, c->S, nf, c->A, c->K, c->lbF, c->NL, c->NC, c->caps); break;
+      default: LAUNCH((k_build<3, true>), cdiv(nf, PB), PB, st, c->dp, c->S, nf, c->A, c->K, c->lbF, c->NL, c->NC, c->caps); break;
+    }
+  }
+  pf.mark();  // end list build
+  if (nf > 0) {
     PAIR_DISPATCH(k_pass_a, cdiv(nf, PB), st, c->dp, c->S, nf, init, c->A, c->R0, c->K, c->lbF, c->WA, c->WR,
-                  c->lbW, c->wnear, c->R1, c->SIG, c->DRHO);
+                  c->lbW, c->wnear, c->R1, c->SIG, c->DRHO, c->NL, c->NC, c->caps);
   }
   pf.mark();  // end pass A
   launch_wall(c, st, false, c->R1);
   pf.mark();  // end wall 2
   if (nf > 0) {
     PAIR_DISPATCH(k_pass_b, cdiv(nf, PB), st, c->dp, c->S, nf, c->A, c->R1, c->K, c->lbF, c->WA, c->WR,
-                  c->WN, c->lbW, c->wnear, c->TB, c->ACC);
+                  c->WN, c->lbW, c->wnear, c->TB, c->ACC, c->NL, c->NC, c->caps);
   }
   pf.mark();  // end pass B
   CK(cudaGetLastError());
@@ -392,6 +405,9 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
   rc |= dalloc(c, &c->R0, nf); rc |= dalloc(c, &c->R1, nf); rc |= dalloc(c, &c->TX, cap); rc |= dalloc(c, &c->A, (size_t)nf + 16);
   rc |= dalloc(c, &c->TB, cap);
   rc |= dalloc(c, &c->ACC, nf); rc |= dalloc(c, &c->SIG, nf); rc |= dalloc(c, &c->DRHO, nf);
+  c->npad = ((size_t)nf + PB - 1) / PB * PB;
+  c->caps = c->prm.max_neighbours ? (int)c->prm.max_neighbours : (c->prm.dim == 3 ? 160 : 64);
+  rc |= dalloc(c, &c->NL, c->npad * (size_t)c->caps); rc |= dalloc(c, &c->NC, nf);
   rc |= dalloc(c, &c->ID0, cap); rc |= dalloc(c, &c->ID1, cap);
   rc |= dalloc(c, &c->keyA, cap); rc |= dalloc(c, &c->valA, cap); rc |= dalloc(c, &c->keyB, cap);
   rc |= dalloc(c, &c->valB, cap);
@@ -559,6 +575,11 @@ int sph_get_stats_ex(sph_ctx* c, sph_stats* out, int32_t with_pairs, void* strea
   }
   out->escaped = (int64_t)hs.escaped; out->nonfinite = (int64_t)hs.nonfinite;
   if (hs.nonfinite) { c->err = "non-finite particle state"; return SPH_ENONFINITE; }
+  if (hs.list_overflow) {
+    c->err = "a particle has " + std::to_string(hs.list_overflow) + " neighbours, the lists hold " +
+             std::to_string(c->caps) + ": set sph_params.max_neighbours";
+    return SPH_ENEIGHBOURS;
+  }
   if (hs.dt_underflow) { c->err = "time step underflow"; return SPH_EDTUNDERFLOW; }
   return SPH_OK;
 }
@@ -579,12 +600,12 @@ int sph_get_timings(sph_ctx* c, float* ms, int32_t* n_steps) {
   for (int k = 0; k < SPH_STAGE_COUNT; ++k) ms[k] = 0.f;
   *n_steps = c->ev_steps;
   if (c->ev_steps == 0) return SPH_OK;
-  CK(cudaEventSynchronize(c->ev[(c->ev_steps - 1) * sph_ctx::EV_PER_STEP + 7]));
-  // marks per step: 0 start, 1 predict, 2 sort, 3 reorder, 4 wall1, 5 passA, 6 wall2, 7 passB
-  static const int stage_of[7] = {SPH_STAGE_PREDICT, SPH_STAGE_SORT, SPH_STAGE_REORDER, SPH_STAGE_WALL,
+  CK(cudaEventSynchronize(c->ev[(c->ev_steps - 1) * sph_ctx::EV_PER_STEP + 8]));
+  // marks per step: 0 start, 1 predict, 2 sort, 3 reorder, 4 wall1, 5 list build, 6 passA, 7 wall2, 8 passB
+  static const int stage_of[8] = {SPH_STAGE_PREDICT, SPH_STAGE_SORT, SPH_STAGE_REORDER, SPH_STAGE_WALL, SPH_STAGE_BUILD,
                                   SPH_STAGE_PASS_A, SPH_STAGE_WALL, SPH_STAGE_PASS_B};
   for (int s = 0; s < c->ev_steps; ++s)
-    for (int k = 0; k < 7; ++k) {
+    for (int k = 0; k < 8; ++k) {
       float t = 0.f;
       CK(cudaEventElapsedTime(&t, c->ev[s * sph_ctx::EV_PER_STEP + k], c->ev[s * sph_ctx::EV_PER_STEP + k + 1]));
       ms[stage_of[k]] += t;

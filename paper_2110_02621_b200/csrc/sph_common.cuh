@@ -63,6 +63,7 @@ struct SS {
   long long steps;
   unsigned long long escaped, nonfinite;
   int dt_underflow;
+  int list_overflow;     // largest neighbour count seen above the list capacity (0 = none); sticky
 };
 
 #define FULL 0xffffffffu

@@ -22,25 +22,35 @@
 #define SPH_CH 4
 #endif
 #ifndef SPH_DU
-#define SPH_DU 2
+#define SPH_DU 4
 #endif
 constexpr int PB = SPH_PB;     // threads per block in the pair kernels
 constexpr int QCAP = SPH_QCAP; // queue entries per lane (QCAP * PB * 4 bytes of shared memory per block)
 constexpr int CH = SPH_CH;     // candidates per lane between two queue-occupancy votes (loads issued together)
 constexpr int DU = SPH_DU;     // queue entries drained together (their gathers issued together)
 
-// Body = struct with  Ld load(unsigned j) const  and  void apply(const Ld&)  so that the drain can
-// issue the gathers of DU queue entries before the arithmetic of the first one.
-template <int DIM, bool EXACT, class Body>
-__device__ __forceinline__ void walk_q(const DP& p, const float4* __restrict__ A, const int* __restrict__ lb,
-                                       const bool act, const float4 ai, const int cx, const int cy,
-                                       const int cz, unsigned* __restrict__ q, Body& body) {
-  const float m2x = -2.0f * ai.x, m2y = -2.0f * ai.y, m2z = -2.0f * ai.z;
-  const float thr = EXACT ? p.rc2m : p.rc2m - ai.w;
-  // next free slot of this lane's queue q[k * PB], k = 0..QCAP-1, as a 32-bit shared-memory address
-  const unsigned qa0 = (unsigned)__cvta_generic_to_shared(q);
-  unsigned qa = qa0;
-  auto drain = [&]() {
+// Body = struct with  Ld load(unsigned j) const  and  void apply(const Ld&)  so that the gathers of
+// DU entries are issued before the arithmetic of the first one.
+//
+// Sinks of the filter walk (what happens to a candidate that passes the filter):
+//   QueueSink  the lane's private shared-memory queue q[k * PB], drained by the whole warp when any
+//              lane is nearly full and at the end (used for the wall walks and by k_wall);
+//   ListSink   the per-warp neighbour list in global memory, slot-major: NL[(warp * caps + slot) * 32 + lane]
+//              (used by k_build; the fluid pair passes then read it with coalesced loads).
+template <class Body>
+struct QueueSink {
+  unsigned* q;
+  unsigned qa0, qa;
+  Body& body;
+  __device__ __forceinline__ QueueSink(unsigned* q_, Body& b) : q(q_), body(b) {
+    qa0 = (unsigned)__cvta_generic_to_shared(q_);
+    qa = qa0;
+  }
+  __device__ __forceinline__ void push(const unsigned j) {
+    asm volatile("st.shared.u32 [%0], %1;" ::"r"(qa), "r"(j) : "memory");
+    qa += PB * 4;
+  }
+  __device__ __forceinline__ void drain() {  // all lanes of the warp together
     const int qn = (int)(qa - qa0) / (PB * 4);
     const int nm = __reduce_max_sync(FULL, qn);
 #pragma unroll 1
@@ -54,7 +64,30 @@ __device__ __forceinline__ void walk_q(const DP& p, const float4* __restrict__ A
         if (k + u < qn) body.apply(ld[u]);
     }
     qa = qa0;
-  };
+  }
+  __device__ __forceinline__ void after_chunk() {
+    if (__any_sync(FULL, qa > qa0 + (QCAP - CH) * PB * 4)) drain();
+  }
+  __device__ __forceinline__ void finish() { drain(); }
+};
+
+struct ListSink {
+  unsigned* __restrict__ nl;  // this lane's column of the warp's list: nl[slot * 32]
+  int n, caps;
+  __device__ __forceinline__ void push(const unsigned j) {
+    if (n < caps) nl[n * 32] = j;
+    ++n;  // counts past caps too: the overflow is reported, never silently dropped
+  }
+  __device__ __forceinline__ void after_chunk() {}
+  __device__ __forceinline__ void finish() {}
+};
+
+template <int DIM, bool EXACT, class Sink>
+__device__ __forceinline__ void walk_f(const DP& p, const float4* __restrict__ A, const int* __restrict__ lb,
+                                       const bool act, const float4 ai, const int cx, const int cy,
+                                       const int cz, Sink& sink) {
+  const float m2x = -2.0f * ai.x, m2y = -2.0f * ai.y, m2z = -2.0f * ai.z;
+  const float thr = EXACT ? p.rc2m : p.rc2m - ai.w;
   constexpr int NR = DIM == 3 ? 9 : 3;
   int ry = -1, rz = DIM == 3 ? -1 : 0;
 #pragma unroll 1
@@ -83,15 +116,38 @@ __device__ __forceinline__ void walk_q(const DP& p, const float4* __restrict__ A
         if (EXACT) t = dist2(ai.x - pj[u].x, ai.y - pj[u].y, DIM == 3 ? ai.z - pj[u].z : 0.0f);
         else if (DIM == 3) t = fmaf(m2x, pj[u].x, fmaf(m2y, pj[u].y, fmaf(m2z, pj[u].z, pj[u].w)));
         else t = fmaf(m2x, pj[u].x, fmaf(m2y, pj[u].y, pj[u].w));
-        if (u < rem && t < thr) {
-          asm volatile("st.shared.u32 [%0], %1;" ::"r"(qa), "r"(jb + u) : "memory");
-          qa += PB * 4;
-        }
+        if (u < rem && t < thr) sink.push((unsigned)(jb + u));
       }
-      if (__any_sync(FULL, qa > qa0 + (QCAP - CH) * PB * 4)) drain();
+      sink.after_chunk();
     }
   }
-  drain();
+  sink.finish();
+}
+
+// Queue walk = filter walk into the shared-memory queue (wall walks, k_wall).
+template <int DIM, bool EXACT, class Body>
+__device__ __forceinline__ void walk_q(const DP& p, const float4* __restrict__ A, const int* __restrict__ lb,
+                                       const bool act, const float4 ai, const int cx, const int cy,
+                                       const int cz, unsigned* __restrict__ q, Body& body) {
+  QueueSink<Body> sink(q, body);
+  walk_f<DIM, EXACT>(p, A, lb, act, ai, cx, cy, cz, sink);
+}
+
+// List walk: every lane runs over its own column of the warp's neighbour list; the slot loop is
+// warp-uniform (to the largest count in the warp), the index load is one coalesced 128-byte line.
+template <class Body>
+__device__ __forceinline__ void walk_l(const unsigned* __restrict__ nl, const int cnt, Body& body) {
+  const int nm = __reduce_max_sync(FULL, cnt);
+#pragma unroll 1
+  for (int k = 0; k < nm; k += DU) {
+    decltype(body.load(0u)) ld[DU];
+#pragma unroll
+    for (int u = 0; u < DU; ++u)
+      if (k + u < cnt) ld[u] = body.load(__ldg(nl + (k + u) * 32));
+#pragma unroll
+    for (int u = 0; u < DU; ++u)
+      if (k + u < cnt) body.apply(ld[u]);
+  }
 }
 
 // Exact pair geometry in units of Q from the fixed-point positions: d = X_i - X_j (wrapping
@@ -197,6 +253,30 @@ __device__ __forceinline__ void cell_of_key(const DP& p, unsigned key, int& cx, 
 }
 
 // ------------------------------------------------------------------------------------------
+// Neighbour list build (once per step, after the reorder): the filter walk of every fluid particle
+// over the fluid arrays, survivors written to the warp's slot-major list.  Both fluid pair passes
+// of the step read it, so the 27-cell candidate walk is done once per step, not once per pass.
+// ------------------------------------------------------------------------------------------
+template <int DIM, bool EXACT>
+__global__ void __launch_bounds__(PB)
+k_build(const DP p, SS* __restrict__ S, const int nf, const float4* __restrict__ A,
+        const unsigned* __restrict__ K, const int* __restrict__ lbF, unsigned* __restrict__ NL,
+        int* __restrict__ NC, const int caps) {
+  const int i0 = blockIdx.x * PB + threadIdx.x;
+  const bool act = i0 < nf;
+  const int i = act ? i0 : nf - 1;
+  const float4 ai = A[i];
+  int cx, cy, cz;
+  cell_of_key(p, K[i], cx, cy, cz);
+  ListSink sink{NL + (size_t)(i0 >> 5) * caps * 32 + (threadIdx.x & 31), 0, caps};
+  walk_f<DIM, EXACT>(p, A, lbF, act, ai, cx, cy, cz, sink);
+  if (act) {
+    NC[i] = min(sink.n, caps);
+    if (sink.n > caps) atomicMax(&S->list_overflow, sink.n);
+  }
+}
+
+// ------------------------------------------------------------------------------------------
 // Wall extrapolation, Eq. 2.12 (readings A4-A7); a_w = 0, v_wall = 0.
 // One thread per wall dummy particle, summing over its fluid neighbours.  WB = (v_w, p_w).
 // ------------------------------------------------------------------------------------------
@@ -263,7 +343,8 @@ k_pass_a(const DP p, const SS* __restrict__ S, const int nf, const int init,
          const unsigned* __restrict__ K, const int* __restrict__ lbF,
          const float4* __restrict__ WA, const XB* __restrict__ WR,
          const int* __restrict__ lbW, const unsigned char* __restrict__ wnear,
-         XB* __restrict__ Rout, float* __restrict__ SIG, float* __restrict__ DRHO) {
+         XB* __restrict__ Rout, float* __restrict__ SIG, float* __restrict__ DRHO,
+         const unsigned* __restrict__ NL, const int* __restrict__ NC, const int caps) {
   __shared__ unsigned qs[QCAP * PB];
   unsigned* q = qs + threadIdx.x;
   const int i0 = blockIdx.x * PB + threadIdx.x;
@@ -298,7 +379,7 @@ k_pass_a(const DP p, const SS* __restrict__ S, const int nf, const int init,
       acc = fmaf(p.mass[phj] * g.f, div_fast(num, rhoj * (ZL + ZR)), acc);
     }
     });
-    walk_q<DIM, EXACT>(p, A, lbF, act, ai, cx, cy, cz, q, body);
+    walk_l(NL + (size_t)(i0 >> 5) * caps * 32 + (threadIdx.x & 31), act ? NC[i] : 0, body);
   }
   float accw = 0.f;
   if (__any_sync(FULL, act && wnear[key])) {
@@ -342,7 +423,8 @@ k_pass_b(const DP p, const SS* __restrict__ S, const int nf,
          const unsigned* __restrict__ K, const int* __restrict__ lbF,
          const float4* __restrict__ WA, const XB* __restrict__ WR,
          const float4* __restrict__ WN, const int* __restrict__ lbW,
-         const unsigned char* __restrict__ wnear, float4* __restrict__ Bout, float4* __restrict__ ACC) {
+         const unsigned char* __restrict__ wnear, float4* __restrict__ Bout, float4* __restrict__ ACC,
+         const unsigned* __restrict__ NL, const int* __restrict__ NC, const int caps) {
   __shared__ unsigned qs[QCAP * PB];
   unsigned* q = qs + threadIdx.x;
   const int i0 = blockIdx.x * PB + threadIdx.x;
@@ -382,7 +464,7 @@ k_pass_b(const DP p, const SS* __restrict__ S, const int nf,
     ax.add(coef * g.dx); ay.add(coef * g.dy);
     if (DIM == 3) az.add(coef * g.dz);
     });
-    walk_q<DIM, EXACT>(p, A, lbF, act, ai, cx, cy, cz, q, body);
+    walk_l(NL + (size_t)(i0 >> 5) * caps * 32 + (threadIdx.x & 31), act ? NC[i] : 0, body);
   }
   KSum wx, wy, wz;
   if (__any_sync(FULL, act && wnear[key])) {

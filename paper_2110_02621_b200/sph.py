@@ -13,7 +13,7 @@ MAX_PHASES = 4
 TAG_WALL = -1
 FLAG_REINIT = 1
 FLAG_WALL_VEL_MIRROR = 2
-STAGES = ("predict", "sort", "reorder", "wall", "pass_a", "pass_b")
+STAGES = ("predict", "sort", "reorder", "wall", "pass_a", "pass_b", "build")
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libsph.so")
@@ -31,7 +31,7 @@ class SphParams(C.Structure):
         ("g", C.c_double * 3), ("g_osc_amp", C.c_double * 3), ("g_osc_period", C.c_double),
         ("cfl", C.c_double), ("penalty_strength", C.c_double),
         ("penalty_phase_mask", C.c_uint32), ("free_surface_mask", C.c_uint32),
-        ("flags", C.c_uint32), ("reserved", C.c_uint32),
+        ("flags", C.c_uint32), ("max_neighbours", C.c_uint32),
         ("domain_min", C.c_double * 3), ("domain_max", C.c_double * 3),
     ]
 
