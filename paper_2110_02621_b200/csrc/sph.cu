@@ -45,7 +45,7 @@ struct sph_ctx {
   uint4* TX = nullptr;
   float4 *A = nullptr, *TB = nullptr, *ACC = nullptr;
   float *SIG = nullptr, *DRHO = nullptr;
-  unsigned* NL = nullptr;  // neighbour lists, slot-major per warp: [npad / 32][caps][32]
+  uint4* NL = nullptr;     // neighbour lists in groups of 4, per warp: [npad / 32][caps / 4][32] (caps % 4 == 0)
   int* NC = nullptr;       // neighbours per fluid particle
   int caps = 0;
   size_t npad = 0;
@@ -406,8 +406,8 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
   rc |= dalloc(c, &c->TB, cap);
   rc |= dalloc(c, &c->ACC, nf); rc |= dalloc(c, &c->SIG, nf); rc |= dalloc(c, &c->DRHO, nf);
   c->npad = ((size_t)nf + PB - 1) / PB * PB;
-  c->caps = c->prm.max_neighbours ? (int)c->prm.max_neighbours : (c->prm.dim == 3 ? 160 : 64);
-  rc |= dalloc(c, &c->NL, c->npad * (size_t)c->caps); rc |= dalloc(c, &c->NC, nf);
+  c->caps = c->prm.max_neighbours ? (int)((c->prm.max_neighbours + 3u) & ~3u) : (c->prm.dim == 3 ? 160 : 64);
+  rc |= dalloc(c, &c->NL, c->npad * (size_t)(c->caps >> 2)); rc |= dalloc(c, &c->NC, nf);
   rc |= dalloc(c, &c->ID0, cap); rc |= dalloc(c, &c->ID1, cap);
   rc |= dalloc(c, &c->keyA, cap); rc |= dalloc(c, &c->valA, cap); rc |= dalloc(c, &c->keyB, cap);
   rc |= dalloc(c, &c->valB, cap);
