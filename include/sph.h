@@ -36,7 +36,9 @@ enum { SPH_MAX_PHASES = 4, SPH_TAG_WALL = -1 };
 
 enum sph_flags {
   SPH_FLAG_REINIT = 1,          /* density reinitialisation each step, Eq. 2.17/2.18 */
-  SPH_FLAG_WALL_VEL_MIRROR = 2  /* v_w = 2 v_wall - <v_f> (Adami-style mirror; reading A6), else v_w = v_wall */
+  SPH_FLAG_WALL_VEL_MIRROR = 2, /* v_w = 2 v_wall - <v_f> (Adami-style mirror; reading A6), else v_w = v_wall */
+  SPH_FLAG_NO_GRAPH = 4         /* sph_step issues every kernel itself instead of replaying one captured step
+                                   as a CUDA graph (same kernels, same results) */
 };
 
 enum sph_error {

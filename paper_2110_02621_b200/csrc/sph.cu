@@ -64,6 +64,10 @@ struct sph_ctx {
   int64_t dt_seq_cap = 0;
   StatAcc* stat = nullptr;
   int sort_passes = 1;
+  // one step captured as a CUDA graph (launch-bound small configurations); rebuilt after sph_set_particles
+  cudaGraphExec_t gexec = nullptr;
+  cudaStream_t cap_stream = nullptr;
+  int64_t graph_launches = 0;  // kernel launches inside the captured step
   // profiling
   bool prof = false;
   std::vector<cudaEvent_t> ev;
@@ -130,6 +134,8 @@ void free_all(sph_ctx* c) {
   for (void* p : ptrs)
     if (p) cudaFree(p);
   for (auto e : c->ev) cudaEventDestroy(e);
+  if (c->gexec) cudaGraphExecDestroy(c->gexec);
+  if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
 }
 
 // Stable radix sort of (keys, vals); result pointers returned in *ko, *vo.
@@ -192,7 +198,8 @@ int pipeline_after_hash(sph_ctx* c, cudaStream_t st, int init, Prof& pf) {
   pf.mark();  // end sort
   if (nf > 0) {
     LAUNCH(k_reorder, cdiv(nf, 256), 256, st, c->dp, nf, vs, c->TX, c->TB, c->IDcur, c->R0, c->A, c->IDnext);
-    std::swap(c->IDcur, c->IDnext);
+    // no pointer ping-pong: every step then issues the same launches with the same arguments (CUDA graph)
+    CK(cudaMemcpyAsync(c->IDcur, c->IDnext, sizeof(unsigned) * nf, cudaMemcpyDeviceToDevice, st));
   }
   LAUNCH(k_cell_bounds, cdiv(c->ncell + 1, 256), 256, st, ks, nf, (int)c->ncell, c->lbF);
   pf.mark();  // end reorder
@@ -237,14 +244,43 @@ int do_steps(sph_ctx* c, int32_t n_steps, const double* dt_host, cudaStream_t st
   }
   const int nf = (int)c->nf;
   const int dt_grid = std::max(1, std::min(cdiv(nf, 256), 148 * 4));
-  for (int s = 0; s < n_steps; ++s) {
-    Prof pf(c, st);
+  auto one_step = [&](cudaStream_t q, const double* seq, int s, Prof& pf) -> int {
     pf.mark();  // start
-    LAUNCH(k_dt, dt_grid, 256, st, c->dp, c->S, nf, c->TB, dt_host ? c->dt_seq : nullptr, s);
+    LAUNCH(k_dt, dt_grid, 256, q, c->dp, c->S, nf, c->TB, seq, s);
     if (nf > 0)
-      LAUNCH(k_predict, cdiv(nf, 256), 256, st, c->dp, c->S, nf, c->R1, c->TB, c->ACC, c->SIG, c->TX, c->keyA, c->valA);
+      LAUNCH(k_predict, cdiv(nf, 256), 256, q, c->dp, c->S, nf, c->R1, c->TB, c->ACC, c->SIG, c->TX, c->keyA, c->valA);
     pf.mark();  // end predict
-    int rc = pipeline_after_hash(c, st, 0, pf);
+    return pipeline_after_hash(c, q, 0, pf);
+  };
+  // Device-computed dt, no per-stage events: every step is the same launch sequence with the same
+  // arguments, so it is captured once (on a private stream) and replayed as a CUDA graph.
+  const bool use_graph = !dt_host && !c->prof && !(c->prm.flags & SPH_FLAG_NO_GRAPH) && n_steps > 0;
+  if (use_graph && !c->gexec) {
+    if (!c->cap_stream) CK(cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking));
+    CK(cudaStreamSynchronize(st));  // the capture stream is not ordered after st: drain st once
+    const int64_t l0 = c->launches;
+    CK(cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal));
+    Prof pf(c, c->cap_stream);
+    pf.on = false;
+    int rc = one_step(c->cap_stream, nullptr, 0, pf);
+    cudaGraph_t graph = nullptr;
+    cudaError_t e = cudaStreamEndCapture(c->cap_stream, &graph);
+    c->graph_launches = c->launches - l0;
+    c->launches = l0;
+    if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
+    if (e != cudaSuccess) { c->err = std::string("graph capture: ") + cudaGetErrorString(e); return SPH_ECUDA; }
+    e = cudaGraphInstantiate(&c->gexec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e != cudaSuccess) { c->gexec = nullptr; c->err = std::string("graph instantiate: ") + cudaGetErrorString(e); return SPH_ECUDA; }
+  }
+  for (int s = 0; s < n_steps; ++s) {
+    if (use_graph) {
+      CK(cudaGraphLaunch(c->gexec, st));
+      c->launches += c->graph_launches;
+      continue;
+    }
+    Prof pf(c, st);
+    int rc = one_step(st, dt_host ? c->dt_seq : nullptr, s, pf);
     if (rc) return rc;
     pf.done();
   }
@@ -387,6 +423,7 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
   }
   cudaStream_t st = (cudaStream_t)stream;
   c->loaded = false;
+  if (c->gexec) { cudaGraphExecDestroy(c->gexec); c->gexec = nullptr; }  // buffers are reallocated below
   // classify on the host (one-off): caller indices of fluid and wall particles, order kept
   std::vector<int32_t> htag((size_t)n);
   if (n) CK(cudaMemcpyAsync(htag.data(), tag, sizeof(int32_t) * n, cudaMemcpyDeviceToHost, st));
