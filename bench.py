@@ -4,7 +4,8 @@
 Contract (driver): `python bench.py --gpus N --steps K --warmup W` prints ONE JSON line on rank 0.
 
   step      one sph_step(1): dt reduction, reinit, kick, drift, cell hash, radix sort, reorder,
-            wall extrapolation x2, pair pass A, pair pass B (+ second kick) on one synthetic config
+            wall extrapolation x2, neighbour-list build, pair pass A, pair pass B (+ second kick)
+            on one synthetic config (replayed as a CUDA graph of the same kernels)
   workload  BASELINE.json configs[1] (3-D dam break with box obstacle, ~0.68 M fluid + ~0.47 M wall)
             unless --config says otherwise; inputs are seeded/synthetic (paper_2110_02621_b200.inputs)
   value     fluid particle-steps/s with the state resident in HBM (CUDA events on the launching
@@ -281,19 +282,26 @@ def run_gpu(args):
     sm_max = clocks.get("sm_max_mhz") or 1965.0
     peak = N_SM * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12       # TFLOP/s at max SM clock
     kern = {}
-    for name, hits, cands, per_step in (("pass_a", fluid_pairs, cand_f, 1), ("pass_b", fluid_pairs, cand_f, 1),
-                                        ("wall", wall_pairs, cand_w, 2)):
-        t = stage_ms[name] * 1e-3 / per_step
+    # Pair stages.  The 27-cell candidate walk runs once per step in k_build (fluid-fluid) and inside
+    # k_wall / the wall part of the passes (fluid-wall); the fluid pair passes read the neighbour lists.
+    # hits: flops of the paper's equations; candidates: CAND_FLOPS each, charged to the stage that tests them.
+    for name, hits, cands, per_step in (("pass_a", fluid_pairs, 0, 1), ("pass_b", fluid_pairs, 0, 1),
+                                        ("build", 0, cand_f, 1), ("wall", wall_pairs, cand_w, 2)):
+        t = stage_ms.get(name, 0.0) * 1e-3 / per_step
         if t <= 0:
             continue
-        fl = FLOPS_HIT[name] * hits
+        fl = FLOPS_HIT.get(name, 0.0) * hits
         kern[name] = {"ms": 1e3 * t, "hits": hits, "candidates": cands,
                       "tflops_hit_only": fl / t / 1e12, "frac_hit_only": fl / t / 1e12 / peak,
                       "tflops_with_candidates": (fl + CAND_FLOPS * cands) / t / 1e12,
                       "frac_with_candidates": (fl + CAND_FLOPS * cands) / t / 1e12 / peak}
+    t_pair = (stage_ms["pass_a"] + stage_ms["pass_b"] + stage_ms.get("build", 0.0)) * 1e-3
+    fl_pair = (FLOPS_HIT["pass_a"] + FLOPS_HIT["pass_b"]) * fluid_pairs
+    pair_stages = {"ms": 1e3 * t_pair, "frac_hit_only": fl_pair / t_pair / 1e12 / peak,
+                   "frac_with_candidates": (fl_pair + CAND_FLOPS * cand_f) / t_pair / 1e12 / peak}
     # HBM-bound stages: algorithmic bytes per fluid particle
     hbm = _peaks().get("hbm_gbs", 6650.0)
-    bytes_pp = {"predict": 108.0, "sort": (16.0 + 4.0) * g_sort_passes(g), "reorder": 92.0}
+    bytes_pp = {"predict": 108.0, "sort": (16.0 + 4.0) * g_sort_passes(g), "reorder": 100.0}
     for name, b in bytes_pp.items():
         t = stage_ms[name] * 1e-3
         if t > 0:
@@ -303,9 +311,9 @@ def run_gpu(args):
                 "peak": peak, "unit": "TFLOP/s", "frac": kern[dom]["frac_hit_only"],
                 "traffic": NCU_TRAFFIC_BYTES.get((cfg["name"], "k_" + dom)),
                 "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 flop x clocks.max.sm (DESIGN.md §7); MEASURED_PEAKS.json holds no non-tensor FP32 peak",
-                "achieved_with_candidates": kern[dom]["tflops_with_candidates"],
-                "frac_with_candidates": kern[dom]["frac_with_candidates"],
-                "flops_per_hit": FLOPS_HIT[dom], "flops_per_candidate": CAND_FLOPS}
+                "flops_per_hit": FLOPS_HIT[dom], "flops_per_candidate": CAND_FLOPS,
+                # list build + pass A + pass B together (the candidate walk is k_build's):
+                "pair_stages": pair_stages}
     g.close()
 
     # ---- end to end through the HOST-pointer entry points ----------------------------------------
