@@ -13,6 +13,7 @@ MAX_PHASES = 4
 TAG_WALL = -1
 FLAG_REINIT = 1
 FLAG_WALL_VEL_MIRROR = 2
+FLAG_NO_GRAPH = 4
 STAGES = ("predict", "sort", "reorder", "wall", "pass_a", "pass_b", "build")
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -105,6 +106,7 @@ def make_params(cfg: dict) -> SphParams:
     P.penalty_phase_mask = cfg.get("penalty_phase_mask", 0)
     P.free_surface_mask = cfg.get("free_surface_mask", 1)
     P.flags = cfg.get("flags", FLAG_REINIT | FLAG_WALL_VEL_MIRROR)
+    P.max_neighbours = cfg.get("max_neighbours", 0)
     return P
 
 
