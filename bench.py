@@ -417,7 +417,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="cfg1")
-    ap.add_argument("--cpu-steps", type=int, default=5, help="oracle steps of the cpu_baseline leg")
+    ap.add_argument("--cpu-steps", type=int, default=25,
+                    help="oracle steps of the cpu_baseline leg (cfg1 full size: about 0.4 s per step on 16 cores)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     args = ap.parse_args()
     if args.impl == "reference":
