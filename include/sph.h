@@ -17,8 +17,11 @@
  *    in 2-D), rho[n], tag[n].  tag = phase id 0..n_phases-1 for fluid (phase 0 the heaviest),
  *    SPH_TAG_WALL for wall dummy particles.  Results come back in the same
  *    order; the internal cell-sorted order is visible only through sph_debug_*.
- *  - Arithmetic is float32 on the device ("fully developed on single precision");
- *    density is held as the deviation rho - rho0 of the particle's phase.
+ *  - Pair arithmetic is float32 on the device ("fully developed on single precision");
+ *    density is held as the deviation rho - rho0 of the particle's phase, positions as 32-bit fixed
+ *    point (quantum Q = 2^-k m, about 1 nm for metre-sized domains) so that |x_in - x_held| <= Q/2 and
+ *    sph_get_fields returns the float32 rounding of the held position; the number density sigma_i
+ *    is summed in float64 (DESIGN.md §4 says why).
  *  - There is no CPU fallback: every call fails with SPH_ECUDA if no CUDA device is usable.
  */
 #ifndef SPH_H_
@@ -117,7 +120,9 @@ int sph_set_particles_host(sph_ctx* ctx, int64_t n, const float* pos_host, const
                            const float* rho_host, const int32_t* tag_host, void* stream);
 
 /* Advance n_steps kick-drift-kick steps (Eq. 2.19-2.24); dt is computed on
- * the device each step from Eq. 2.23-2.24 (reading A17).  Asynchronous; no host sync per step. */
+ * the device each step from Eq. 2.23-2.24 (reading A17).  Asynchronous; no host sync per step.
+ * The first call after sph_set_particles captures one step as a CUDA graph (it synchronises the
+ * stream once to do so); later steps replay it on `stream` (SPH_FLAG_NO_GRAPH: plain launches). */
 int sph_step(sph_ctx* ctx, int32_t n_steps, void* stream);
 
 /* Same, with a caller-given dt sequence (host array of n_steps doubles) so that the oracle and
