@@ -370,6 +370,7 @@ int sph_create(const sph_params* prm, sph_ctx** out) {
     }
     d.sub_per_m = 1024.0 / d.Q;
     d.Qf = (float)d.Q; d.qh = (float)(d.Q / h); d.qhD = d.Q / h;
+    d.mhqD[0] = -0.5 * d.qhD; d.mhqD[1] = d.mhqD[0] / 1024.0; d.tqD[0] = 2.0 * d.qhD; d.tqD[1] = d.tqD[0] / 1024.0;
     d.gradcQ = (float)(-5.0 * alpha / (h * h) * d.Q);
     d.two_over_dp = (float)(2.0 * d.Q / dp);
     // candidate filter margin: rounding of the expanded form |xj|^2 - 2 xi.xj + |xi|^2 on images

@@ -33,6 +33,7 @@ struct DP {
   float dmin[3], dmax[3];
   double O[3], C[3], Q, sub_per_m;  // fixed point: origin, image centre, quantum, 1024 / Q
   double cmax, cfl, hD, dpD, qhD;  // qhD = Q / h
+  double mhqD[2], tqD[2];          // -q/2 and 2q per unit of r: [0] r in Q, [1] r in Q/1024 (w64)
   double massD[SPH_MAX_PHASES];
   double a_over_s0;
   double g[3], gamp[3], gperiod;

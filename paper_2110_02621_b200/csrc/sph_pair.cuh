@@ -108,43 +108,81 @@ struct ListSink {
   __device__ __forceinline__ void finish() { flush(true); }
 };
 
-template <int DIM, bool EXACT, class Sink>
+// The candidate images of a row are staged once per warp in shared memory: the lanes of a warp sit in
+// 2-3 neighbouring cells, so their 3-cell ranges of one stencil row overlap in one index interval
+// [smin, emax) of ~4-5 cells.  The warp copies it with coalesced 16-byte loads into its tile (TW
+// candidates at a time) and every lane then walks its own sub-range out of shared memory, where the
+// lanes of one cell read the same address (a broadcast) — about one L1 wavefront per step instead
+// of the ~4.6 a warp-wide global load of 2-3 unaligned addresses costs (profiles/r01c_README.md).
+constexpr int TW = 128;  // candidates per warp tile (2 KB)
+template <int DIM, bool EXACT>
+__device__ __forceinline__ float filter_t(const float4& ai, const float m2x, const float m2y, const float m2z,
+                                          const float4& pj) {
+  if (EXACT) return dist2(ai.x - pj.x, ai.y - pj.y, DIM == 3 ? ai.z - pj.z : 0.0f);
+  if (DIM == 3) return fmaf(m2x, pj.x, fmaf(m2y, pj.y, fmaf(m2z, pj.z, pj.w)));
+  return fmaf(m2x, pj.x, fmaf(m2y, pj.y, pj.w));
+}
+template <int DIM, bool EXACT, bool STAGE, class Sink>
 __device__ __forceinline__ void walk_f(const DP& p, const float4* __restrict__ A, const int* __restrict__ lb,
                                        const bool act, const float4 ai, const int cx, const int cy,
-                                       const int cz, Sink& sink) {
+                                       const int cz, float4* __restrict__ tile, Sink& sink) {
   const float m2x = -2.0f * ai.x, m2y = -2.0f * ai.y, m2z = -2.0f * ai.z;
   const float thr = EXACT ? p.rc2m : p.rc2m - ai.w;
+  const int lane = threadIdx.x & 31;
   constexpr int NR = DIM == 3 ? 9 : 3;
   int ry = -1, rz = DIM == 3 ? -1 : 0;
 #pragma unroll 1
   for (int r = 0; r < NR; ++r) {
-    int s = 0, e = 0;
+    int s = 0x7fffffff, e = 0;
     const int y = cy + ry, z = cz + rz;
     if (act && y >= 0 && y < p.ny && z >= 0 && z < p.nz) {
       const int rb = (z * p.ny + y) * p.nx;
-      s = __ldg(lb + rb + max(cx - 1, 0));
+      const int s1 = __ldg(lb + rb + max(cx - 1, 0));
       e = __ldg(lb + rb + min(cx + 1, p.nx - 1) + 1);
+      if (e > s1) s = s1; else e = 0;
     }
     if (++ry > 1) { ry = -1; ++rz; }
-    const int len = e - s;
-    const int nmax = __reduce_max_sync(FULL, len);
-    const int last = len > 0 ? e - 1 : 0;  // clamp of the chunk base (index 0 is valid; arrays are padded by CH)
+    const int smin = STAGE ? __reduce_min_sync(FULL, s) : 0, emax = STAGE ? __reduce_max_sync(FULL, e) : 0;
+    if (STAGE && emax - smin <= TW) {  // warp-uniform; emax <= smin when no lane has a candidate in this row
+      const int t0 = smin, n = emax - smin;
+      __syncwarp();
+#pragma unroll
+      for (int k = 0; k < TW; k += 32)
+        if (k + lane < n) tile[k + lane] = __ldg(A + t0 + k + lane);
+      __syncwarp();
+      const int lo = min(s, emax) - t0;  // this lane's part of the tile: [lo, lo + len), len <= 0: none
+      const int len = e - t0 - lo;
+      const int nmax = __reduce_max_sync(FULL, len);
+      const int last = n - 1;
 #pragma unroll 1
-    for (int k0 = 0; k0 < nmax; k0 += CH) {
-      const int jb = s + k0, rem = len - k0;
-      const float4* __restrict__ ap = A + min(jb, last);
-      float4 pj[CH];
+      for (int k0 = 0; k0 < nmax; k0 += CH) {
+        const int rem = len - k0;
+        float4 pj[CH];
 #pragma unroll
-      for (int u = 0; u < CH; ++u) pj[u] = __ldg(ap + u);
+        for (int u = 0; u < CH; ++u) pj[u] = tile[min(lo + k0 + u, last)];
 #pragma unroll
-      for (int u = 0; u < CH; ++u) {
-        float t;
-        if (EXACT) t = dist2(ai.x - pj[u].x, ai.y - pj[u].y, DIM == 3 ? ai.z - pj[u].z : 0.0f);
-        else if (DIM == 3) t = fmaf(m2x, pj[u].x, fmaf(m2y, pj[u].y, fmaf(m2z, pj[u].z, pj[u].w)));
-        else t = fmaf(m2x, pj[u].x, fmaf(m2y, pj[u].y, pj[u].w));
-        if (u < rem && t < thr) sink.push((unsigned)(jb + u));
+        for (int u = 0; u < CH; ++u)
+          if (u < rem && filter_t<DIM, EXACT>(ai, m2x, m2y, m2z, pj[u]) < thr) sink.push((unsigned)(t0 + lo + k0 + u));
+        sink.after_chunk();
       }
-      sink.after_chunk();
+    } else {
+      // the lanes' ranges are far apart (a warp that straddles the end of a cell row, wall particles
+      // of a thin layer): every lane reads its own range from global memory
+      const int len = e > 0 ? e - s : 0, jb0 = e > 0 ? s : 0;
+      const int nmax = __reduce_max_sync(FULL, len);
+      const int last = len > 0 ? e - 1 : 0;
+#pragma unroll 1
+      for (int k0 = 0; k0 < nmax; k0 += CH) {
+        const int jb = jb0 + k0, rem = len - k0;
+        const float4* __restrict__ ap = A + min(jb, last);  // clamp of the chunk base (arrays are padded by CH)
+        float4 pj[CH];
+#pragma unroll
+        for (int u = 0; u < CH; ++u) pj[u] = __ldg(ap + u);
+#pragma unroll
+        for (int u = 0; u < CH; ++u)
+          if (u < rem && filter_t<DIM, EXACT>(ai, m2x, m2y, m2z, pj[u]) < thr) sink.push((unsigned)(jb + u));
+        sink.after_chunk();
+      }
     }
   }
   sink.finish();
@@ -156,7 +194,7 @@ __device__ __forceinline__ void walk_q(const DP& p, const float4* __restrict__ A
                                        const bool act, const float4 ai, const int cx, const int cy,
                                        const int cz, unsigned* __restrict__ q, Body& body) {
   QueueSink<Body> sink(q, body);
-  walk_f<DIM, EXACT>(p, A, lb, act, ai, cx, cy, cz, sink);
+  walk_f<DIM, EXACT, false>(p, A, lb, act, ai, cx, cy, cz, nullptr, sink);
 }
 
 // List walk: every lane runs over its own column of the warp's neighbour groups; the loop is
@@ -236,11 +274,11 @@ __device__ __forceinline__ Geo geometry(const DP& p, const uint4& xi, const uint
 // sigma_i only.  p = c0^2 rho0 (sigma/sigma0 - 1) with c0^2 = 200 g H amplifies a relative error of
 // sigma by 200, and the momentum sum amplifies a pressure error by another H / h: float32 terms
 // (2e-7 each) leave 3e-5 of rho0 g H in p and 2.5e-4 g in a at H / dp = 100 (measured against the
-// oracle).  r^2 is an exact 64-bit integer; 1/sqrt by MUFU.RSQ64H + one Newton step (1e-12).
+// oracle).  r^2 is an exact 64-bit integer; its root is one float64 Newton step from the float32 r.
 template <int DIM, bool SUBQ>
-__device__ __forceinline__ double w64(const DP& p, const uint4& xi, const uint4& xj) {
+__device__ __forceinline__ double w64(const DP& p, const uint4& xi, const uint4& xj, const Geo& g) {
   const long long dx = (int)(xi.x - xj.x), dy = (int)(xi.y - xj.y), dz = DIM == 3 ? (int)(xi.z - xj.z) : 0;
-  double r2, qs;
+  double r2, r0, hy;
   if (SUBQ) {
     // multi-phase: include the 10-bit residuals (units of Q/1024).  For a light phase with its own
     // large c0 (config 2b: c_air^2 = 1000 c_w^2) sigma must be good to 1e-11, i.e. positions to 1e-12 m.
@@ -248,18 +286,20 @@ __device__ __forceinline__ double w64(const DP& p, const uint4& xi, const uint4&
     const double ey = (double)((dy << 10) + (int)((xi.w >> 12) & 1023u) - (int)((xj.w >> 12) & 1023u));
     const double ez = DIM == 3 ? (double)((dz << 10) + (int)((xi.w >> 2) & 1023u) - (int)((xj.w >> 2) & 1023u)) : 0.0;
     r2 = fma(ez, ez, fma(ey, ey, ex * ex));
-    qs = p.qhD * (1.0 / 1024.0);
+    r0 = (double)(g.r * 1024.0f);
+    hy = (double)(g.rinv * (0.5f / 1024.0f));
   } else {
     r2 = (double)(dx * dx + dy * dy + dz * dz);
-    qs = p.qhD;
+    r0 = (double)g.r;
+    hy = (double)(0.5f * g.rinv);
   }
-  double y;
-  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(r2));
-  const double e = fma(-r2 * y, y, 1.0);
-  y = fma(0.5 * y, e, y);
-  const double q = r2 > 0.0 ? r2 * y * qs : 0.0;
-  const double t = fmax(fma(-0.5, q, 1.0), 0.0), t2 = t * t;
-  return t2 * t2 * fma(2.0, q, 1.0);
+  // sqrt by one Newton step in float64 from the float32 r of the geometry (relative error e <= 2e-7,
+  // with the residuals 1e-6): r = r0 + (r2 - r0^2) / (2 r0), error e^2 / 2.  r2 = 0 gives r0 = 0, r = 0.
+  const double r = fma(fma(-r0, r0, r2), hy, r0);
+  const double t = fma(r, p.mhqD[SUBQ], 1.0), u = fma(r, p.tqD[SUBQ], 1.0), t2 = t * t;
+  // outside the support (decided on the float32 q of the geometry, as for every other term) the
+  // term is exactly 0; within a rounding of q = 2 the value is below 1e-26
+  return g.f > 0.0f ? t2 * t2 * u : 0.0;
 }
 
 // Pair body = the neighbour's record (one 256-bit gather) + the arithmetic on it.
@@ -295,6 +335,7 @@ k_build(const DP p, SS* __restrict__ S, const int nf, const float4* __restrict__
         const unsigned* __restrict__ K, const int* __restrict__ lbF, uint4* __restrict__ NL,
         int* __restrict__ NC, const int caps) {
   __shared__ unsigned qs[QCAP * PB];
+  __shared__ float4 tiles[PB / 32][TW];
   const int i0 = blockIdx.x * PB + threadIdx.x;
   const bool act = i0 < nf;
   const int i = act ? i0 : nf - 1;
@@ -302,7 +343,7 @@ k_build(const DP p, SS* __restrict__ S, const int nf, const float4* __restrict__
   int cx, cy, cz;
   cell_of_key(p, K[i], cx, cy, cz);
   ListSink sink(qs + threadIdx.x, NL + (size_t)(i0 >> 5) * (caps >> 2) * 32 + (threadIdx.x & 31), caps >> 2);
-  walk_f<DIM, EXACT>(p, A, lbF, act, ai, cx, cy, cz, sink);
+  walk_f<DIM, EXACT, true>(p, A, lbF, act, ai, cx, cy, cz, tiles[threadIdx.x >> 5], sink);
   if (act) {
     NC[i] = min(sink.n, caps);
     if (sink.n > caps) atomicMax(&S->list_overflow, sink.n);
@@ -370,7 +411,7 @@ k_wall(const DP p, const SS* __restrict__ S, const int nw, const float4* __restr
 // r = 0 and v_ij = 0, nothing to the continuity sum.
 // ------------------------------------------------------------------------------------------
 template <int DIM, bool MULTI, bool EXACT>
-__global__ void __launch_bounds__(PB)
+__global__ void __launch_bounds__(PB, 6)
 k_pass_a(const DP p, const SS* __restrict__ S, const int nf, const int init,
          const float4* __restrict__ A, const XB* __restrict__ R,
          const unsigned* __restrict__ K, const int* __restrict__ lbF,
@@ -397,7 +438,7 @@ k_pass_a(const DP p, const SS* __restrict__ S, const int nf, const int init,
   {
     auto body = make_body(R, [&](const uint4& xj, const float4& bj, const unsigned j) {
     const Geo g = geometry<DIM>(p, xi, xj);
-    sig += w64<DIM, MULTI>(p, xi, xj);
+    sig += w64<DIM, MULTI>(p, xi, xj, g);
     const float vd = fmaf(bi.z - bj.z, g.dz, fmaf(bi.y - bj.y, g.dy, (bi.x - bj.x) * g.dx));
     if (!MULTI) {
       // equal c: (U* - U_L)(Z_L + Z_R) = c (rho_j v_ij.e + c (rho_i - rho_j)) with p = c^2 (rho - rho0)
@@ -419,7 +460,7 @@ k_pass_a(const DP p, const SS* __restrict__ S, const int nf, const int init,
     {
       auto body = make_body(WR, [&](const uint4& xj, const float4& bj, const unsigned j) {  // (v_w, p_w)
       const Geo g = geometry<DIM>(p, xi, xj);
-      sig += w64<DIM, MULTI>(p, xi, xj);
+      sig += w64<DIM, MULTI>(p, xi, xj, g);
       const float rhow = fmaf(bj.w, p.inv_c2[phi], rho0i);  // reading A5
       const float ZR = rhow * ci;
       const float vd = fmaf(bi.z - bj.z, g.dz, fmaf(bi.y - bj.y, g.dy, (bi.x - bj.x) * g.dx));
@@ -450,7 +491,7 @@ k_pass_a(const DP p, const SS* __restrict__ S, const int nf, const int init,
 // Eq. 2.13-2.15 (readings A8, A9, A11), gravity, then the second half kick Eq. 2.22.
 // ------------------------------------------------------------------------------------------
 template <int DIM, bool MULTI, bool EXACT>
-__global__ void __launch_bounds__(PB)
+__global__ void __launch_bounds__(PB, 6)
 k_pass_b(const DP p, const SS* __restrict__ S, const int nf,
          const float4* __restrict__ A, const XB* __restrict__ R,
          const unsigned* __restrict__ K, const int* __restrict__ lbF,
