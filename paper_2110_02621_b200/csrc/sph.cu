@@ -8,6 +8,7 @@
 // normals), sph_pair.cuh (wall extrapolation, pass A, pass B), sph_debug.cuh (output, stats,
 // integer-contract debug paths).  This file is the host side and the extern "C" entry points.
 #include <cuda_runtime.h>
+#include <cuda_fp16.h>
 #include <math.h>
 #include <stdint.h>
 #include <stdio.h>
@@ -380,6 +381,13 @@ int sph_create(const sph_params* prm, sph_ctx** out) {
     const double err_diff = 16.0 * u * R * rc;
     d.exact_filter = 2.0 * err_expanded > 0.08 * rc * rc ? 1 : 0;
     d.rc2m = (float)(rc * rc + 2.0 * (d.exact_filter ? err_diff : err_expanded));
+    {  // float16 filter of k_build (sph_pair.cuh): threshold rounded up to the next half
+      d.inv_h = (float)(1.0 / h);
+      const double thr = 4.08 + 2.0 * err_diff / (h * h);
+      __half th = __double2half(thr);
+      if ((double)__half2float(th) < thr) th = __ushort_as_half((unsigned short)(__half_as_ushort(th) + 1));
+      d.thr_h2 = (unsigned)__half_as_ushort(th) * 0x10001u;
+    }
   }
   d.gamma_p = (float)prm->penalty_strength;
   d.pen_mask = prm->penalty_phase_mask; d.fs_mask = prm->free_surface_mask; d.flags = prm->flags;

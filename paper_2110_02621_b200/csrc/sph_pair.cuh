@@ -10,6 +10,8 @@
 //            exact geometry from the fixed-point positions (integer subtract + I2F), then the
 //            pair physics.  Filter false positives (margin) have r >= 2h and add exactly zero.
 #pragma once
+#include <cuda_fp16.h>
+
 #include "sph_common.cuh"
 
 #ifndef SPH_PB
@@ -65,8 +67,8 @@ struct QueueSink {
     }
     qa = qa0;
   }
-  __device__ __forceinline__ void after_chunk() {
-    if (__any_sync(FULL, qa > qa0 + (QCAP - CH) * PB * 4)) drain();
+  __device__ __forceinline__ void after_chunk(const int ch = CH) {
+    if (__any_sync(FULL, qa > qa0 + (QCAP - ch) * PB * 4)) drain();
   }
   __device__ __forceinline__ void finish() { drain(); }
 };
@@ -87,11 +89,32 @@ struct ListSink {
   __device__ __forceinline__ void push(const unsigned j) {
     asm volatile("st.shared.u32 [%0], %1;" ::"r"(qa), "r"(j) : "memory");
     qa += PB * 4;
-    ++n;  // counts past the capacity too: the overflow is reported, never silently dropped
+  }
+  // Two candidates at once: r2 and thr are half2; candidate u (index kk + u in the lane's range of
+  // len entries, list index j0 + u) is pushed iff r2.u < thr.u and 0 <= kk + u < len.
+  __device__ __forceinline__ void push2(const unsigned r2, const unsigned thr, const int kk, const int len, const unsigned j0) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p, q;\n"
+        ".reg .u32 t;\n"
+        "setp.lt.f16x2 p|q, %1, %2;\n"
+        "setp.lt.and.u32 p, %3, %4, p;\n"
+        "add.u32 t, %3, 1;\n"
+        "setp.lt.and.u32 q, t, %4, q;\n"
+        "@p st.shared.u32 [%0], %5;\n"
+        "@p add.u32 %0, %0, %6;\n"
+        "add.u32 t, %5, 1;\n"
+        "@q st.shared.u32 [%0], t;\n"
+        "@q add.u32 %0, %0, %6;\n"
+        "}"
+        : "+r"(qa)
+        : "r"(r2), "r"(thr), "r"(kk), "r"(len), "r"(j0), "n"(PB * 4)
+        : "memory");
   }
   __device__ __forceinline__ void flush(const bool last) {
     const int qn = (int)(qa - qa0) / (PB * 4);
     const int ngr = last ? (qn + 3) >> 2 : qn >> 2;
+    if (last) n = 4 * ng + qn;  // counts past the capacity too: the overflow is reported, never silently dropped
     const int nm = __reduce_max_sync(FULL, ngr);
 #pragma unroll 1
     for (int t = 0; t < nm; ++t)
@@ -102,19 +125,58 @@ struct ListSink {
     for (int r = 0; r < rem; ++r) q[r * PB] = q[(4 * ngr + r) * PB];
     qa = qa0 + rem * PB * 4;
   }
-  __device__ __forceinline__ void after_chunk() {
-    if (__any_sync(FULL, qa > qa0 + (QCAP - CH) * PB * 4)) flush(false);
+  __device__ __forceinline__ void after_chunk(const int ch = CH) {
+    if (__any_sync(FULL, qa > qa0 + (QCAP - ch) * PB * 4)) flush(false);
   }
   __device__ __forceinline__ void finish() { flush(true); }
 };
 
-// The candidate images of a row are staged once per warp in shared memory: the lanes of a warp sit in
-// 2-3 neighbouring cells, so their 3-cell ranges of one stencil row overlap in one index interval
-// [smin, emax) of ~4-5 cells.  The warp copies it with coalesced 16-byte loads into its tile (TW
-// candidates at a time) and every lane then walks its own sub-range out of shared memory, where the
-// lanes of one cell read the same address (a broadcast) — about one L1 wavefront per step instead
-// of the ~4.6 a warp-wide global load of 2-3 unaligned addresses costs (profiles/r01c_README.md).
-constexpr int TW = 128;  // candidates per warp tile (2 KB)
+// Staged filter of k_build.  The lanes of a warp sit in 2-3 neighbouring cells, so their 3-cell
+// ranges of one stencil row overlap in one index interval [smin, emax) of ~4-5 cells.  The warp reads
+// it once with coalesced 16-byte loads and stages it in shared memory as float16 coordinates
+// relative to the warp's first particle, in units of h, two candidates per record (x0 x1 y0 y1 |
+// z0 z1); every lane then tests its own sub-range two candidates at a time with packed half
+// arithmetic (difference form).  What bounds the walk is the L1/shared data pipe, which moves 128
+// bytes per cycle whatever the address pattern: 16-byte float4 candidates cost 4 wavefronts per
+// warp-wide read (staged float32: 98 % of the pipe's peak, profiles/r01d_README.md), the 6-byte
+// float16 candidate 1.5.
+// Margin of the float16 test (units of h, r_c = 2): coordinates are below 16 in magnitude (checked
+// per row, else the row falls back to the float32 path), so each is rounded by at most 2^-8; the
+// difference by 2^-11 |d| <= 1.1e-3: 8.9e-3 per axis, 1.54e-2 in norm, 2 r |e| + |e|^2 <= 6.2e-2 on
+// r^2 at r = 2; the three roundings of the sum of squares add 3 * 2^-11 * 4 = 5.9e-3.  A true
+// neighbour therefore computes r^2 < 4.068; the threshold is 4.08 plus the float32 image margin.
+// A false positive has q >= 2 in the passes and adds exactly 0 (reading B2).
+constexpr int TW = 128;   // candidates per warp tile
+constexpr int TP = TW / 2 + 4;  // pair records per tile, padded for the chunk over-read
+constexpr int CHS = 8;    // candidates (4 pair records) per lane between two occupancy votes
+struct HCtx {          // per-lane constants of the float16 test
+  float ox, oy, oz;    // origin: centred image of the warp's first particle
+  unsigned xi, yi, zi; // this lane's coordinates, each duplicated in both halves
+  bool bad;            // a coordinate of this lane is outside the float16 working range
+};
+struct HTile {
+  uint2 xy[TP];     // (x0 x1), (y0 y1) as half2
+  unsigned z[TP];   // (z0 z1)
+};
+__device__ __forceinline__ unsigned h2(const float a, const float b) {
+  const __half2 h = __floats2half2_rn(a, b);
+  return *reinterpret_cast<const unsigned*>(&h);
+}
+__device__ __forceinline__ unsigned hsub2(const unsigned a, const unsigned b) {
+  unsigned d;
+  asm("sub.rn.f16x2 %0, %1, %2;" : "=r"(d) : "r"(a), "r"(b));
+  return d;
+}
+__device__ __forceinline__ unsigned hmul2(const unsigned a, const unsigned b) {
+  unsigned d;
+  asm("mul.rn.f16x2 %0, %1, %2;" : "=r"(d) : "r"(a), "r"(b));
+  return d;
+}
+__device__ __forceinline__ unsigned hfma2(const unsigned a, const unsigned b, const unsigned c) {
+  unsigned d;
+  asm("fma.rn.f16x2 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+  return d;
+}
 template <int DIM, bool EXACT>
 __device__ __forceinline__ float filter_t(const float4& ai, const float m2x, const float m2y, const float m2z,
                                           const float4& pj) {
@@ -125,7 +187,7 @@ __device__ __forceinline__ float filter_t(const float4& ai, const float m2x, con
 template <int DIM, bool EXACT, bool STAGE, class Sink>
 __device__ __forceinline__ void walk_f(const DP& p, const float4* __restrict__ A, const int* __restrict__ lb,
                                        const bool act, const float4 ai, const int cx, const int cy,
-                                       const int cz, float4* __restrict__ tile, Sink& sink) {
+                                       const int cz, HTile* __restrict__ tile, const HCtx& hc, Sink& sink) {
   const float m2x = -2.0f * ai.x, m2y = -2.0f * ai.y, m2z = -2.0f * ai.z;
   const float thr = EXACT ? p.rc2m : p.rc2m - ai.w;
   const int lane = threadIdx.x & 31;
@@ -143,29 +205,58 @@ __device__ __forceinline__ void walk_f(const DP& p, const float4* __restrict__ A
     }
     if (++ry > 1) { ry = -1; ++rz; }
     const int smin = STAGE ? __reduce_min_sync(FULL, s) : 0, emax = STAGE ? __reduce_max_sync(FULL, e) : 0;
-    if (STAGE && emax - smin <= TW) {  // warp-uniform; emax <= smin when no lane has a candidate in this row
+    bool staged = false;
+    if constexpr (STAGE) if (emax - smin <= TW) {  // warp-uniform; emax <= smin when no lane has a candidate in this row
       const int t0 = smin, n = emax - smin;
+      bool bad = hc.bad;
       __syncwarp();
 #pragma unroll
-      for (int k = 0; k < TW; k += 32)
-        if (k + lane < n) tile[k + lane] = __ldg(A + t0 + k + lane);
-      __syncwarp();
-      const int lo = min(s, emax) - t0;  // this lane's part of the tile: [lo, lo + len), len <= 0: none
-      const int len = e - t0 - lo;
-      const int nmax = __reduce_max_sync(FULL, len);
-      const int last = n - 1;
-#pragma unroll 1
-      for (int k0 = 0; k0 < nmax; k0 += CH) {
-        const int rem = len - k0;
-        float4 pj[CH];
-#pragma unroll
-        for (int u = 0; u < CH; ++u) pj[u] = tile[min(lo + k0 + u, last)];
-#pragma unroll
-        for (int u = 0; u < CH; ++u)
-          if (u < rem && filter_t<DIM, EXACT>(ai, m2x, m2y, m2z, pj[u]) < thr) sink.push((unsigned)(t0 + lo + k0 + u));
-        sink.after_chunk();
+      for (int k = 0; k < TW; k += 32) {
+        const int c = k + lane;
+        if (c < n) {
+          const float4 a = __ldg(A + t0 + c);
+          const float x = (a.x - hc.ox) * p.inv_h, y = (a.y - hc.oy) * p.inv_h, z = DIM == 3 ? (a.z - hc.oz) * p.inv_h : 0.0f;
+          bad |= !(fmaxf(fabsf(x), fmaxf(fabsf(y), fabsf(z))) < 15.9f);
+          __half* xy = reinterpret_cast<__half*>(tile->xy + (c >> 1)) + (c & 1);
+          xy[0] = __float2half_rn(x);
+          xy[2] = __float2half_rn(y);
+          if (DIM == 3) reinterpret_cast<__half*>(tile->z + (c >> 1))[c & 1] = __float2half_rn(z);
+        }
       }
-    } else {
+      staged = !__any_sync(FULL, bad);
+      __syncwarp();
+      if (staged) {
+        const int lo = min(s, emax) - t0;  // this lane's part of the tile: [lo, lo + len), len <= 0: none
+        const int len = max(e - t0 - lo, 0), odd = lo & 1, np = (odd + len + 1) >> 1;
+        const int npmax = __reduce_max_sync(FULL, np);
+        const int pb = lo >> 1, plast = (n + 1) >> 1;
+#pragma unroll 1
+        for (int kp = 0; kp < npmax; kp += CHS / 2) {
+          const int pi = min(pb + kp, plast);  // reads run up to 3 records past the last one: the tile is padded
+          uint2 xy[CHS / 2];
+          unsigned zz[CHS / 2];
+#pragma unroll
+          for (int u = 0; u < CHS / 2; ++u) {
+            xy[u] = tile->xy[pi + u];
+            if (DIM == 3) zz[u] = tile->z[pi + u];
+          }
+          const int kk = 2 * kp - odd;           // index of the chunk's first candidate in the lane's range
+          const unsigned j0 = (unsigned)(t0 + 2 * (pb + kp));
+#pragma unroll
+          for (int u = 0; u < CHS / 2; ++u) {
+            const unsigned dx = hsub2(hc.xi, xy[u].x), dy = hsub2(hc.yi, xy[u].y);
+            unsigned r2 = hfma2(dy, dy, hmul2(dx, dx));
+            if (DIM == 3) {
+              const unsigned dz = hsub2(hc.zi, zz[u]);
+              r2 = hfma2(dz, dz, r2);
+            }
+            sink.push2(r2, p.thr_h2, kk + 2 * u, len, j0 + 2 * u);
+          }
+          sink.after_chunk(CHS);
+        }
+      }
+    }
+    if (!staged) {
       // the lanes' ranges are far apart (a warp that straddles the end of a cell row, wall particles
       // of a thin layer): every lane reads its own range from global memory
       const int len = e > 0 ? e - s : 0, jb0 = e > 0 ? s : 0;
@@ -181,7 +272,7 @@ __device__ __forceinline__ void walk_f(const DP& p, const float4* __restrict__ A
 #pragma unroll
         for (int u = 0; u < CH; ++u)
           if (u < rem && filter_t<DIM, EXACT>(ai, m2x, m2y, m2z, pj[u]) < thr) sink.push((unsigned)(jb + u));
-        sink.after_chunk();
+        sink.after_chunk(STAGE ? CHS : CH);  // the head room the next chunk of either path needs
       }
     }
   }
@@ -194,7 +285,7 @@ __device__ __forceinline__ void walk_q(const DP& p, const float4* __restrict__ A
                                        const bool act, const float4 ai, const int cx, const int cy,
                                        const int cz, unsigned* __restrict__ q, Body& body) {
   QueueSink<Body> sink(q, body);
-  walk_f<DIM, EXACT, false>(p, A, lb, act, ai, cx, cy, cz, nullptr, sink);
+  walk_f<DIM, EXACT, false>(p, A, lb, act, ai, cx, cy, cz, nullptr, HCtx{}, sink);
 }
 
 // List walk: every lane runs over its own column of the warp's neighbour groups; the loop is
@@ -335,7 +426,7 @@ k_build(const DP p, SS* __restrict__ S, const int nf, const float4* __restrict__
         const unsigned* __restrict__ K, const int* __restrict__ lbF, uint4* __restrict__ NL,
         int* __restrict__ NC, const int caps) {
   __shared__ unsigned qs[QCAP * PB];
-  __shared__ float4 tiles[PB / 32][TW];
+  __shared__ HTile tiles[PB / 32];
   const int i0 = blockIdx.x * PB + threadIdx.x;
   const bool act = i0 < nf;
   const int i = act ? i0 : nf - 1;
@@ -343,7 +434,14 @@ k_build(const DP p, SS* __restrict__ S, const int nf, const float4* __restrict__
   int cx, cy, cz;
   cell_of_key(p, K[i], cx, cy, cz);
   ListSink sink(qs + threadIdx.x, NL + (size_t)(i0 >> 5) * (caps >> 2) * 32 + (threadIdx.x & 31), caps >> 2);
-  walk_f<DIM, EXACT, true>(p, A, lbF, act, ai, cx, cy, cz, tiles[threadIdx.x >> 5], sink);
+  HCtx hc;
+  hc.ox = __shfl_sync(FULL, ai.x, 0); hc.oy = __shfl_sync(FULL, ai.y, 0); hc.oz = DIM == 3 ? __shfl_sync(FULL, ai.z, 0) : 0.0f;
+  {
+    const float x = (ai.x - hc.ox) * p.inv_h, y = (ai.y - hc.oy) * p.inv_h, z = DIM == 3 ? (ai.z - hc.oz) * p.inv_h : 0.0f;
+    hc.bad = act && !(fmaxf(fabsf(x), fmaxf(fabsf(y), fabsf(z))) < 15.9f);
+    hc.xi = h2(x, x); hc.yi = h2(y, y); hc.zi = h2(z, z);
+  }
+  walk_f<DIM, EXACT, true>(p, A, lbF, act, ai, cx, cy, cz, tiles + (threadIdx.x >> 5), hc, sink);
   if (act) {
     NC[i] = min(sink.n, caps);
     if (sink.n > caps) atomicMax(&S->list_overflow, sink.n);
