@@ -167,6 +167,14 @@ int sph_debug_cells(sph_ctx* ctx, int32_t* cell_id_host, int32_t* perm_host,
 int sph_debug_neighbours(sph_ctx* ctx, int64_t* offsets_host, int32_t* ids_host, int64_t cap,
                          int64_t* total_host, void* stream);
 
+/* Checks the step's fluid-fluid neighbour lists (built once per step by the candidate filter,
+ * DESIGN.md section 5) against the float32 contract of reading A24 on the current positions:
+ * out3_host[0] = contract neighbours missing from a list (must be 0: the filter is conservative),
+ * out3_host[1] = list entries that are not contract neighbours (filter margin; they add exactly 0,
+ * reading B2), out3_host[2] = list entries in total (self entries included).  HOST pointer to 3
+ * values; synchronises the stream.  Errors: SPH_EINVAL without particles, SPH_ECUDA. */
+int sph_debug_list_check(sph_ctx* ctx, int64_t* out3_host, void* stream);
+
 /* Wall normals Eq. 2.16 in caller order (n*3, zero for fluid entries); HOST pointer. */
 int sph_debug_normals(sph_ctx* ctx, float* normals_host, void* stream);
 

@@ -732,6 +732,26 @@ int sph_debug_neighbours(sph_ctx* c, int64_t* offsets, int32_t* ids, int64_t cap
   return rc;
 }
 
+int sph_debug_list_check(sph_ctx* c, int64_t* out3, void* stream) {
+  if (!c || !out3) return SPH_EINVAL;
+  if (!c->loaded) { c->err = "no particles"; return SPH_EINVAL; }
+  cudaStream_t st = (cudaStream_t)stream;
+  out3[0] = out3[1] = out3[2] = 0;
+  if (!c->nf) return SPH_OK;
+  unsigned long long* d = nullptr;
+  CK(cudaMalloc((void**)&d, 24));
+  CK(cudaMemsetAsync(d, 0, 24, st));
+  const float4* G = fluid_images(c, st);
+  LAUNCH(k_list_check, cdiv(c->nf, PW), PW * 32, st, c->dp, (int)c->nf, G, c->lbF, c->NL, c->NC, c->caps, d);
+  unsigned long long h[3];
+  cudaError_t e = cudaMemcpyAsync(h, d, 24, cudaMemcpyDeviceToHost, st);
+  cudaError_t e2 = cudaStreamSynchronize(st);
+  cudaFree(d);
+  if (e != cudaSuccess || e2 != cudaSuccess) { c->err = cudaGetErrorString(e != cudaSuccess ? e : e2); return SPH_ECUDA; }
+  for (int k = 0; k < 3; ++k) out3[k] = (int64_t)h[k];
+  return SPH_OK;
+}
+
 int sph_debug_normals(sph_ctx* c, float* normals, void* stream) {
   if (!c || !normals) return SPH_EINVAL;
   if (!c->loaded) { c->err = "no particles"; return SPH_EINVAL; }

@@ -211,6 +211,37 @@ k_neigh(DP p, int n, int is_wall, int mode, const float4* __restrict__ Pself, co
   }
 }
 
+// sph_debug_list_check: every fluid neighbour of the float32 contract (reading A24) must be an entry
+// of the step's neighbour list (the float16 / float32 candidate filters of k_build are conservative);
+// out[0] += contract neighbours missing from the list, out[1] += list entries (self excluded) that
+// are not contract neighbours, out[2] += list entries in total.
+__global__ void __launch_bounds__(PW * 32)
+k_list_check(DP p, int nf, const float4* __restrict__ P, const int* __restrict__ lbF,
+             const uint4* __restrict__ NL, const int* __restrict__ NC, int caps, unsigned long long* out) {
+  __shared__ unsigned qs[PW][64];
+  const int i = blockIdx.x * PW + (threadIdx.x >> 5);
+  if (i >= nf) return;
+  const int lane = threadIdx.x & 31;
+  const float4 pi = P[i];
+  const unsigned* col = reinterpret_cast<const unsigned*>(NL + (size_t)(i >> 5) * (caps >> 2) * 32 + (i & 31));
+  const int cnt = NC[i];
+  int missing = 0, found = 0;
+  walk(p, P, lbF, pi.x, pi.y, pi.z, i, qs[threadIdx.x >> 5], [&](int j) {
+    bool in = false;
+    for (int k = 0; k < cnt && !in; ++k) in = col[(size_t)(k >> 2) * 128 + (k & 3)] == (unsigned)j;
+    if (in) ++found; else ++missing;
+  });
+  for (int o = 16; o > 0; o >>= 1) {
+    missing += __shfl_xor_sync(FULL, missing, o);
+    found += __shfl_xor_sync(FULL, found, o);
+  }
+  if (lane == 0) {
+    if (missing) atomicAdd(out, (unsigned long long)missing);
+    atomicAdd(out + 1, (unsigned long long)(cnt - 1 - found));
+    atomicAdd(out + 2, (unsigned long long)cnt);
+  }
+}
+
 __global__ void k_dbg_cells(DP p, int n, const float4* __restrict__ P, const unsigned* __restrict__ ID,
                             int* cell_id, int* perm, int perm_base) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;

@@ -48,7 +48,7 @@ class SphStats(C.Structure):
 EXPORTS = (
     "sph_create", "sph_destroy", "sph_set_particles", "sph_set_particles_host", "sph_step",
     "sph_step_dt", "sph_get_fields", "sph_get_fields_host", "sph_get_stats", "sph_get_stats_ex", "sph_set_profiling",
-    "sph_get_timings", "sph_num_cells", "sph_debug_cells", "sph_debug_neighbours",
+    "sph_get_timings", "sph_num_cells", "sph_debug_cells", "sph_debug_neighbours", "sph_debug_list_check",
     "sph_debug_normals", "sph_debug_sigma", "sph_launch_count", "sph_last_error",
 )
 
@@ -81,6 +81,7 @@ def load():
     L.sph_debug_cells.restype = C.c_int; L.sph_debug_cells.argtypes = [vp] * 6
     L.sph_debug_neighbours.restype = C.c_int; L.sph_debug_neighbours.argtypes = [vp, vp, vp, i64, vp, vp]
     L.sph_debug_normals.restype = C.c_int; L.sph_debug_normals.argtypes = [vp, vp, vp]
+    L.sph_debug_list_check.restype = C.c_int; L.sph_debug_list_check.argtypes = [vp, vp, vp]
     L.sph_debug_sigma.restype = C.c_int; L.sph_debug_sigma.argtypes = [vp, vp, vp]
     L.sph_launch_count.restype = i64; L.sph_launch_count.argtypes = [vp]
     L.sph_last_error.restype = C.c_char_p; L.sph_last_error.argtypes = [vp]
@@ -233,6 +234,12 @@ class Sph:
         ids = np.zeros(max(tot.value, 1), np.int32)
         self._ck(self.L.sph_debug_neighbours(self.ctx, _hp(off), _hp(ids), tot.value, C.byref(tot), self._st()))
         return off, ids[:tot.value]
+
+    def debug_list_check(self):
+        """(missing, extra, total) of the step's neighbour lists against the float32 contract."""
+        out = np.zeros(3, np.int64)
+        self._ck(self.L.sph_debug_list_check(self.ctx, _hp(out), self._st()))
+        return int(out[0]), int(out[1]), int(out[2])
 
     def debug_normals(self):
         nw = np.zeros((self.n, 3), np.float32)

@@ -57,6 +57,34 @@ def test_neighbour_lists_bit_exact(name):
     assert g.get_stats()["npairs"] == int((roff[1:] - roff[:-1])[fluid].sum())
 
 
+@pytest.mark.parametrize("name", list(SMALL) + ["box3d_64", "sloshing_small"])
+def test_step_lists_hold_every_contract_neighbour(name):
+    """The lists the pair passes read (k_build: float16 staged filter, float32 fallback) are a
+    superset of the float32 contract's fluid neighbours (bit-exact vs brute force above), after the
+    set-up and after steps; the filter margin costs only a few per cent of extra entries."""
+    if name == "box3d_64":
+        cfg = inputs.box_sweep_3d(n=64)
+    elif name == "sloshing_small":
+        cfg = inputs.sloshing_spheres_3d(dp=0.02)
+    else:
+        cfg = SMALL[name]
+    g = sph.Sph(cfg)
+    g.set_particles(cfg["pos"], cfg["vel"], cfg["rho"], cfg["tag"])
+    for steps in (0, 1, 7):
+        if steps:
+            g.step(steps)
+        missing, extra, total = g.debug_list_check()
+        off, _ = g.debug_neighbours()
+        fluid = cfg["tag"] >= 0
+        n_contract = int((off[1:] - off[:-1])[fluid].sum()) + int(fluid.sum())   # + self entries
+        assert missing == 0
+        assert total >= int(fluid.sum())
+        assert extra <= 0.06 * total + 8, (extra, total)
+        # fluid-fluid contract pairs + self = list entries minus the margin entries
+        ff = total - extra
+        assert ff <= n_contract
+
+
 def test_neighbour_lists_after_steps_snapshot():
     """Snapshot check (reading A25): take the GPU positions after 25 steps, feed them to the
     oracle's float32 rule, compare lists and cell ids at those positions."""
