@@ -64,7 +64,7 @@ struct sph_ctx {
   double* dt_seq = nullptr;
   int64_t dt_seq_cap = 0;
   StatAcc* stat = nullptr;
-  int sort_passes = 1;
+  int sort_passes = 1, sort_bits = 8;
   // one step captured as a CUDA graph (launch-bound small configurations); rebuilt after sph_set_particles
   cudaGraphExec_t gexec = nullptr;
   cudaStream_t cap_stream = nullptr;
@@ -146,11 +146,18 @@ int radix_sort(sph_ctx* c, cudaStream_t st, int n, unsigned* kA, unsigned* vA, u
   if (n > 0) {
     int nblk = cdiv(n, RS_TILE);
     for (int pass = 0; pass < c->sort_passes; ++pass) {
-      int shift = 8 * pass;
-      LAUNCH(k_radix_hist, nblk, RS_THREADS, st, ki, n, shift, c->hist, nblk);
-      LAUNCH(k_scan_rowsum, 256, 256, st, c->hist, nblk, c->rowsum);
-      LAUNCH(k_scan_apply, 256, 256, st, c->hist, nblk, c->rowsum);
-      LAUNCH(k_radix_scatter, nblk, RS_THREADS, st, ki, vi, n, shift, c->hist, nblk, kt, vt);
+      int shift = c->sort_bits * pass;
+      if (c->sort_bits == 9) {
+        LAUNCH(k_radix_hist<512>, nblk, RS_THREADS, st, ki, n, shift, c->hist, nblk);
+        LAUNCH(k_scan_rowsum, 512, 256, st, c->hist, nblk, c->rowsum);
+        LAUNCH(k_scan_apply, 512, 256, st, c->hist, nblk, c->rowsum);
+        LAUNCH(k_radix_scatter<512>, nblk, RS_THREADS, st, ki, vi, n, shift, c->hist, nblk, kt, vt);
+      } else {
+        LAUNCH(k_radix_hist<256>, nblk, RS_THREADS, st, ki, n, shift, c->hist, nblk);
+        LAUNCH(k_scan_rowsum, 256, 256, st, c->hist, nblk, c->rowsum);
+        LAUNCH(k_scan_apply, 256, 256, st, c->hist, nblk, c->rowsum);
+        LAUNCH(k_radix_scatter<256>, nblk, RS_THREADS, st, ki, vi, n, shift, c->hist, nblk, kt, vt);
+      }
       std::swap(ki, kt);
       std::swap(vi, vt);
     }
@@ -407,7 +414,8 @@ int sph_create(const sph_params* prm, sph_ctx** out) {
   if (c->ncell >= (1ll << 31) - 2) { delete c; return SPH_EINVAL; }
   int bits = 1;
   while ((1ll << bits) < c->ncell) ++bits;
-  c->sort_passes = (bits + 7) / 8;
+  c->sort_bits = (bits + 8) / 9 < (bits + 7) / 8 ? 9 : 8;
+  c->sort_passes = (bits + c->sort_bits - 1) / c->sort_bits;
   c->multi = prm->n_phases > 1;
   *out = c;
   return SPH_OK;
@@ -457,8 +465,8 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
   rc |= dalloc(c, &c->ID0, cap); rc |= dalloc(c, &c->ID1, cap);
   rc |= dalloc(c, &c->keyA, cap); rc |= dalloc(c, &c->valA, cap); rc |= dalloc(c, &c->keyB, cap);
   rc |= dalloc(c, &c->valB, cap);
-  rc |= dalloc(c, &c->hist, (size_t)256 * cdiv(std::max<size_t>(cap, 1), RS_TILE));
-  rc |= dalloc(c, &c->rowsum, 256);
+  rc |= dalloc(c, &c->hist, (size_t)512 * cdiv(std::max<size_t>(cap, 1), RS_TILE));
+  rc |= dalloc(c, &c->rowsum, 512);
   rc |= dalloc(c, &c->lbF, c->ncell + 1); rc |= dalloc(c, &c->lbW, c->ncell + 1);
   rc |= dalloc(c, &c->wnear, c->ncell);
   rc |= dalloc(c, &c->WR, nw); rc |= dalloc(c, &c->WA, (size_t)nw + 16);

@@ -1,17 +1,21 @@
 // sph_sort.cuh — device radix sort of (cell id, index) and cell lower bounds.  Included by sph.cu.
 #pragma once
 // ------------------------------------------------------------------------------------------
-// Device radix sort (stable LSD, 8-bit digits) of (cell id, index).  BASELINE.json north_star
+// Device radix sort (stable LSD) of (cell id, index).  Digits of RB = 8 or 9 bits (ND = 256 / 512
+// bins), whichever needs fewer passes for the grid's cell count: 17-18 bit cell ids (cfg1, cfg4 up
+// to 4 M) sort in 2 passes of 9 bits instead of 3 of 8; a pass is 4 dependent launches and at
+// these sizes latency-bound.  BASELINE.json north_star
 // "cell hash, device radix sort"; the paper only names the step.
 // Per pass: tile histograms -> row sums -> scan -> stable scatter with warp match ranking.
 // ------------------------------------------------------------------------------------------
 constexpr int RS_THREADS = 256, RS_ITEMS = 16, RS_TILE = RS_THREADS * RS_ITEMS, RS_WARPS = 8;
 
+template <int ND>
 __global__ void __launch_bounds__(RS_THREADS)
 k_radix_hist(const unsigned* __restrict__ keys, int n, int shift, unsigned* __restrict__ hist,
              int nblk) {
-  __shared__ unsigned h[256];
-  h[threadIdx.x] = 0;
+  __shared__ unsigned h[ND];
+  for (int d = threadIdx.x; d < ND; d += RS_THREADS) h[d] = 0;
   __syncthreads();
   const int lane = threadIdx.x & 31;
   const int base = blockIdx.x * RS_TILE;
@@ -19,12 +23,12 @@ k_radix_hist(const unsigned* __restrict__ keys, int n, int shift, unsigned* __re
   for (int it = 0; it < RS_ITEMS; ++it) {
     int idx = base + it * RS_THREADS + threadIdx.x;
     bool ok = idx < n;
-    unsigned d = ok ? ((keys[idx] >> shift) & 255u) : 256u;
+    unsigned d = ok ? ((keys[idx] >> shift) & (unsigned)(ND - 1)) : (unsigned)ND;
     unsigned peers = __match_any_sync(FULL, d);
     if (ok && lane == __ffs(peers) - 1) atomicAdd(&h[d], (unsigned)__popc(peers));
   }
   __syncthreads();
-  hist[threadIdx.x * nblk + blockIdx.x] = h[threadIdx.x];
+  for (int d = threadIdx.x; d < ND; d += RS_THREADS) hist[d * nblk + blockIdx.x] = h[d];
 }
 
 __global__ void __launch_bounds__(256)
@@ -51,7 +55,8 @@ k_scan_apply(unsigned* __restrict__ hist, int nblk, const unsigned* __restrict__
   __shared__ unsigned carry_s;
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   // base = sum of rowsum[d'] for d' < digit
-  unsigned b = (threadIdx.x < blockIdx.x) ? rowsum[threadIdx.x] : 0u;
+  unsigned b = 0u;
+  for (int t = threadIdx.x; t < (int)blockIdx.x; t += 256) b += rowsum[t];
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) b += __shfl_xor_sync(FULL, b, o);
   if (lane == 0) sm[wid] = b;
@@ -84,13 +89,14 @@ k_scan_apply(unsigned* __restrict__ hist, int nblk, const unsigned* __restrict__
   }
 }
 
+template <int ND>
 __global__ void __launch_bounds__(RS_THREADS)
 k_radix_scatter(const unsigned* __restrict__ keys, const unsigned* __restrict__ vals, int n, int shift,
                 const unsigned* __restrict__ hist, int nblk, unsigned* __restrict__ keys_out,
                 unsigned* __restrict__ vals_out) {
-  __shared__ unsigned wc[RS_WARPS][256];
+  __shared__ unsigned wc[RS_WARPS][ND];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  for (int i = threadIdx.x; i < RS_WARPS * 256; i += RS_THREADS) (&wc[0][0])[i] = 0;
+  for (int i = threadIdx.x; i < RS_WARPS * ND; i += RS_THREADS) (&wc[0][0])[i] = 0;
   __syncthreads();
   const int base = blockIdx.x * RS_TILE + wid * (RS_ITEMS * 32);
   unsigned k[RS_ITEMS], rank[RS_ITEMS];
@@ -100,7 +106,7 @@ k_radix_scatter(const unsigned* __restrict__ keys, const unsigned* __restrict__ 
     int idx = base + it * 32 + lane;  // warp-contiguous order keeps the sort stable
     bool ok = idx < n;
     k[it] = ok ? keys[idx] : 0xffffffffu;
-    unsigned d = ok ? ((k[it] >> shift) & 255u) : 256u;
+    unsigned d = ok ? ((k[it] >> shift) & (unsigned)(ND - 1)) : (unsigned)ND;
     unsigned peers = __match_any_sync(FULL, d);
     int leader = __ffs(peers) - 1;
     unsigned old = 0;
@@ -113,8 +119,8 @@ k_radix_scatter(const unsigned* __restrict__ keys, const unsigned* __restrict__ 
     __syncwarp();
   }
   __syncthreads();
-  {  // exclusive prefix over warps per digit, plus the scanned global base of this tile
-    unsigned d = threadIdx.x, run = hist[d * nblk + blockIdx.x];
+  for (int d = threadIdx.x; d < ND; d += RS_THREADS) {  // exclusive prefix over warps per digit, plus the scanned global base of this tile
+    unsigned run = hist[d * nblk + blockIdx.x];
 #pragma unroll
     for (int w = 0; w < RS_WARPS; ++w) {
       unsigned t = wc[w][d];
@@ -127,7 +133,7 @@ k_radix_scatter(const unsigned* __restrict__ keys, const unsigned* __restrict__ 
   for (int it = 0; it < RS_ITEMS; ++it) {
     int idx = base + it * 32 + lane;
     if (idx < n) {
-      unsigned d = (k[it] >> shift) & 255u;
+      unsigned d = (k[it] >> shift) & (unsigned)(ND - 1);
       unsigned dst = wc[wid][d] + rank[it];
       keys_out[dst] = k[it];
       vals_out[dst] = vals[idx];
