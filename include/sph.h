@@ -72,7 +72,8 @@ typedef struct {
   uint32_t free_surface_mask;    /* bit k: phase k uses continuity Eq. 2.9/2.21 + reinit Eq. 2.17;
                                     otherwise summation Eq. 2.4 + reinit Eq. 2.18 (reading A13, A15) */
   uint32_t flags;                /* sph_flags */
-  uint32_t max_neighbours;       /* capacity of the per-particle neighbour lists; 0 = default (160 in 3-D, 64 in 2-D) */
+  uint32_t max_neighbours;       /* capacity of the per-particle fluid-fluid neighbour lists; 0 = default (160 in 3-D,
+                                    64 in 2-D); the fluid-wall lists hold 3/4 of it */
   double domain_min[3];          /* box of the cell grid; particles outside are binned in the edge */
   double domain_max[3];          /* cells and counted as escaped (reading A23)                      */
 } sph_params;

@@ -49,6 +49,9 @@ struct sph_ctx {
   uint4* NL = nullptr;     // neighbour lists in groups of 4, per warp: [npad / 32][caps / 4][32] (caps % 4 == 0)
   int* NC = nullptr;       // neighbours per fluid particle
   int caps = 0;
+  uint4* NLW = nullptr;    // fluid-wall neighbour lists, same layout with capsw slots
+  int* NCW = nullptr;
+  int capsw = 0;
   size_t npad = 0;
   unsigned *ID0 = nullptr, *ID1 = nullptr, *IDcur = nullptr, *IDnext = nullptr;
   unsigned *keyA = nullptr, *valA = nullptr, *keyB = nullptr, *valB = nullptr, *hist = nullptr,
@@ -129,7 +132,7 @@ int dalloc(sph_ctx* c, T** p, size_t count) {
 }
 
 void free_all(sph_ctx* c) {
-  void* ptrs[] = {c->R0, c->R1, c->TX, c->A, c->TB, c->ACC, c->SIG, c->DRHO, c->NL, c->NC, c->ID0, c->ID1,
+  void* ptrs[] = {c->R0, c->R1, c->TX, c->A, c->TB, c->ACC, c->SIG, c->DRHO, c->NL, c->NC, c->NLW, c->NCW, c->ID0, c->ID1,
                   c->keyA, c->valA, c->keyB, c->valB, c->hist, c->rowsum, c->lbF, c->lbW, c->WR,
                   c->WA, c->WN, c->WG, c->WK, c->WID, c->wnear, c->S, c->dt_seq, c->stat};
   for (void* p : ptrs)
@@ -215,23 +218,23 @@ int pipeline_after_hash(sph_ctx* c, cudaStream_t st, int init, Prof& pf) {
   pf.mark();  // end wall 1
   if (nf > 0) {
     switch (PAIR_SEL(c) & 5) {  // DIM x EXACT
-      case 0: LAUNCH((k_build<2, false>), cdiv(nf, PB), PB, st, c->dp, c->S, nf, c->A, c->K, c->lbF, c->NL, c->NC, c->caps); break;
-      case 1: LAUNCH((k_build<2, true>), cdiv(nf, PB), PB, st, c->dp, c->S, nf, c->A, c->K, c->lbF, c->NL, c->NC, c->caps); break;
-      case 4: LAUNCH((k_build<3, false>), cdiv(nf, PB), PB, st, c->dp, c->S, nf, c->A, c->K, c->lbF, c->NL, c->NC, c->caps); break;
-      default: LAUNCH((k_build<3, true>), cdiv(nf, PB), PB, st, c->dp, c->S, nf, c->A, c->K, c->lbF, c->NL, c->NC, c->caps); break;
+      case 0: LAUNCH((k_build<2, false>), cdiv(nf, PB), PB, st, c->dp, c->S, nf, c->A, c->K, c->lbF, c->NL, c->NC, c->caps, c->WA, c->lbW, c->wnear, c->NLW, c->NCW, c->capsw); break;
+      case 1: LAUNCH((k_build<2, true>), cdiv(nf, PB), PB, st, c->dp, c->S, nf, c->A, c->K, c->lbF, c->NL, c->NC, c->caps, c->WA, c->lbW, c->wnear, c->NLW, c->NCW, c->capsw); break;
+      case 4: LAUNCH((k_build<3, false>), cdiv(nf, PB), PB, st, c->dp, c->S, nf, c->A, c->K, c->lbF, c->NL, c->NC, c->caps, c->WA, c->lbW, c->wnear, c->NLW, c->NCW, c->capsw); break;
+      default: LAUNCH((k_build<3, true>), cdiv(nf, PB), PB, st, c->dp, c->S, nf, c->A, c->K, c->lbF, c->NL, c->NC, c->caps, c->WA, c->lbW, c->wnear, c->NLW, c->NCW, c->capsw); break;
     }
   }
   pf.mark();  // end list build
   if (nf > 0) {
     PAIR_DISPATCH(k_pass_a, cdiv(nf, PB), st, c->dp, c->S, nf, init, c->A, c->R0, c->K, c->lbF, c->WA, c->WR,
-                  c->lbW, c->wnear, c->R1, c->SIG, c->DRHO, c->NL, c->NC, c->caps);
+                  c->lbW, c->wnear, c->R1, c->SIG, c->DRHO, c->NL, c->NC, c->caps, c->NLW, c->NCW, c->capsw);
   }
   pf.mark();  // end pass A
   launch_wall(c, st, false, c->R1);
   pf.mark();  // end wall 2
   if (nf > 0) {
     PAIR_DISPATCH(k_pass_b, cdiv(nf, PB), st, c->dp, c->S, nf, c->A, c->R1, c->K, c->lbF, c->WA, c->WR,
-                  c->WN, c->lbW, c->wnear, c->TB, c->ACC, c->NL, c->NC, c->caps);
+                  c->WN, c->lbW, c->wnear, c->TB, c->ACC, c->NL, c->NC, c->caps, c->NLW, c->NCW, c->capsw);
   }
   pf.mark();  // end pass B
   CK(cudaGetLastError());
@@ -462,6 +465,8 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
   c->npad = ((size_t)nf + PB - 1) / PB * PB;
   c->caps = c->prm.max_neighbours ? (int)((c->prm.max_neighbours + 3u) & ~3u) : (c->prm.dim == 3 ? 160 : 64);
   rc |= dalloc(c, &c->NL, c->npad * (size_t)(c->caps >> 2)); rc |= dalloc(c, &c->NC, nf);
+  c->capsw = (c->caps * 3 / 4 + 3) & ~3;  // a particle in a corner of three walls has 7/8 of its (then smaller) support in them
+  rc |= dalloc(c, &c->NLW, c->npad * (size_t)(c->capsw >> 2)); rc |= dalloc(c, &c->NCW, nf);
   rc |= dalloc(c, &c->ID0, cap); rc |= dalloc(c, &c->ID1, cap);
   rc |= dalloc(c, &c->keyA, cap); rc |= dalloc(c, &c->valA, cap); rc |= dalloc(c, &c->keyB, cap);
   rc |= dalloc(c, &c->valB, cap);
@@ -631,7 +636,8 @@ int sph_get_stats_ex(sph_ctx* c, sph_stats* out, int32_t with_pairs, void* strea
   if (hs.nonfinite) { c->err = "non-finite particle state"; return SPH_ENONFINITE; }
   if (hs.list_overflow) {
     c->err = "a particle has " + std::to_string(hs.list_overflow) + " neighbours, the lists hold " +
-             std::to_string(c->caps) + ": set sph_params.max_neighbours";
+             std::to_string(c->caps) + " fluid and " + std::to_string(c->capsw) +
+             " wall entries: set sph_params.max_neighbours";
     return SPH_ENEIGHBOURS;
   }
   if (hs.dt_underflow) { c->err = "time step underflow"; return SPH_EDTUNDERFLOW; }

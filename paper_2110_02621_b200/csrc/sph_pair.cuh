@@ -424,16 +424,18 @@ template <int DIM, bool EXACT>
 __global__ void __launch_bounds__(PB)
 k_build(const DP p, SS* __restrict__ S, const int nf, const float4* __restrict__ A,
         const unsigned* __restrict__ K, const int* __restrict__ lbF, uint4* __restrict__ NL,
-        int* __restrict__ NC, const int caps) {
+        int* __restrict__ NC, const int caps,
+        const float4* __restrict__ WA, const int* __restrict__ lbW, const unsigned char* __restrict__ wnear,
+        uint4* __restrict__ NLW, int* __restrict__ NCW, const int capsw) {
   __shared__ unsigned qs[QCAP * PB];
   __shared__ HTile tiles[PB / 32];
   const int i0 = blockIdx.x * PB + threadIdx.x;
   const bool act = i0 < nf;
   const int i = act ? i0 : nf - 1;
   const float4 ai = A[i];
+  const unsigned key = K[i];
   int cx, cy, cz;
-  cell_of_key(p, K[i], cx, cy, cz);
-  ListSink sink(qs + threadIdx.x, NL + (size_t)(i0 >> 5) * (caps >> 2) * 32 + (threadIdx.x & 31), caps >> 2);
+  cell_of_key(p, key, cx, cy, cz);
   HCtx hc;
   hc.ox = __shfl_sync(FULL, ai.x, 0); hc.oy = __shfl_sync(FULL, ai.y, 0); hc.oz = DIM == 3 ? __shfl_sync(FULL, ai.z, 0) : 0.0f;
   {
@@ -441,10 +443,24 @@ k_build(const DP p, SS* __restrict__ S, const int nf, const float4* __restrict__
     hc.bad = act && !(fmaxf(fabsf(x), fmaxf(fabsf(y), fabsf(z))) < 15.9f);
     hc.xi = h2(x, x); hc.yi = h2(y, y); hc.zi = h2(z, z);
   }
-  walk_f<DIM, EXACT, true>(p, A, lbF, act, ai, cx, cy, cz, tiles + (threadIdx.x >> 5), hc, sink);
+  int n = 0, nw = 0;
+  {
+    ListSink sink(qs + threadIdx.x, NL + (size_t)(i0 >> 5) * (caps >> 2) * 32 + (threadIdx.x & 31), caps >> 2);
+    walk_f<DIM, EXACT, true>(p, A, lbF, act, ai, cx, cy, cz, tiles + (threadIdx.x >> 5), hc, sink);
+    n = sink.n;
+  }
+  // fluid-wall lists (same filter over the static wall arrays) for the warps that have a wall
+  // particle in a stencil: both pair passes read them, so the wall candidate walk is also paid once
+  if (__any_sync(FULL, act && wnear[key])) {
+    ListSink sink(qs + threadIdx.x, NLW + (size_t)(i0 >> 5) * (capsw >> 2) * 32 + (threadIdx.x & 31), capsw >> 2);
+    walk_f<DIM, EXACT, true>(p, WA, lbW, act, ai, cx, cy, cz, tiles + (threadIdx.x >> 5), hc, sink);
+    nw = sink.n;
+  }
   if (act) {
-    NC[i] = min(sink.n, caps);
-    if (sink.n > caps) atomicMax(&S->list_overflow, sink.n);
+    NC[i] = min(n, caps);
+    NCW[i] = min(nw, capsw);
+    if (n > caps) atomicMax(&S->list_overflow, n);
+    if (nw > capsw) atomicMax(&S->list_overflow, nw);
   }
 }
 
@@ -516,18 +532,14 @@ k_pass_a(const DP p, const SS* __restrict__ S, const int nf, const int init,
          const float4* __restrict__ WA, const XB* __restrict__ WR,
          const int* __restrict__ lbW, const unsigned char* __restrict__ wnear,
          XB* __restrict__ Rout, float* __restrict__ SIG, float* __restrict__ DRHO,
-         const uint4* __restrict__ NL, const int* __restrict__ NC, const int caps) {
-  __shared__ unsigned qs[QCAP * PB];
-  unsigned* q = qs + threadIdx.x;
+         const uint4* __restrict__ NL, const int* __restrict__ NC, const int caps,
+         const uint4* __restrict__ NLW, const int* __restrict__ NCW, const int capsw) {
   const int i0 = blockIdx.x * PB + threadIdx.x;
   const bool act = i0 < nf;
   const int i = act ? i0 : nf - 1;
-  const float4 ai = A[i];
   const uint4 xi = R[i].x;
   const float4 bi = R[i].b;
   const unsigned key = K[i];
-  int cx, cy, cz;
-  cell_of_key(p, key, cx, cy, cz);
   const int phi = MULTI ? phase_of(xi) : 0;
   const float rho0i = p.rho0[phi], c2i = p.c2[phi], ci = p.c0[phi];
   const float rhoi = rho0i + bi.w, prsi = c2i * bi.w, ZL = rhoi * ci;
@@ -565,7 +577,7 @@ k_pass_a(const DP p, const SS* __restrict__ S, const int nf, const int init,
       const float num = fmaf(ZR, vd, (prsi - bj.w) * g.r);
       accw = fmaf(g.f, div_fast(num, ZL + ZR), accw);
       });
-      walk_q<DIM, EXACT>(p, WA, lbW, act, ai, cx, cy, cz, q, body);
+      walk_l(NLW + (size_t)(i0 >> 5) * (capsw >> 2) * 32 + (threadIdx.x & 31), act ? NCW[i] : 0, body);
     }
   }
   if (!act) return;
@@ -596,18 +608,14 @@ k_pass_b(const DP p, const SS* __restrict__ S, const int nf,
          const float4* __restrict__ WA, const XB* __restrict__ WR,
          const float4* __restrict__ WN, const int* __restrict__ lbW,
          const unsigned char* __restrict__ wnear, float4* __restrict__ Bout, float4* __restrict__ ACC,
-         const uint4* __restrict__ NL, const int* __restrict__ NC, const int caps) {
-  __shared__ unsigned qs[QCAP * PB];
-  unsigned* q = qs + threadIdx.x;
+         const uint4* __restrict__ NL, const int* __restrict__ NC, const int caps,
+         const uint4* __restrict__ NLW, const int* __restrict__ NCW, const int capsw) {
   const int i0 = blockIdx.x * PB + threadIdx.x;
   const bool act = i0 < nf;
   const int i = act ? i0 : nf - 1;
-  const float4 ai = A[i];
   const uint4 xi = R[i].x;
   const float4 bi = R[i].b;
   const unsigned key = K[i];
-  int cx, cy, cz;
-  cell_of_key(p, key, cx, cy, cz);
   const int phi = MULTI ? phase_of(xi) : 0;
   const float rho0i = p.rho0[phi], c2i = p.c2[phi], ci = p.c0[phi];
   const float rhoi = rho0i + bi.w, prsi = c2i * bi.w, ZL = rhoi * ci;
@@ -665,7 +673,7 @@ k_pass_b(const DP p, const SS* __restrict__ S, const int nf,
         }
       }
       });
-      walk_q<DIM, EXACT>(p, WA, lbW, act, ai, cx, cy, cz, q, body);
+      walk_l(NLW + (size_t)(i0 >> 5) * (capsw >> 2) * 32 + (threadIdx.x & 31), act ? NCW[i] : 0, body);
     }
   }
   if (!act) return;
