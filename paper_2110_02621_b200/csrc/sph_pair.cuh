@@ -17,6 +17,9 @@
 #ifndef SPH_PB
 #define SPH_PB 128
 #endif
+#ifndef SPH_MINB
+#define SPH_MINB 8
+#endif
 #ifndef SPH_QCAP
 #define SPH_QCAP 32
 #endif
@@ -525,7 +528,7 @@ k_wall(const DP p, const SS* __restrict__ S, const int nw, const float4* __restr
 // r = 0 and v_ij = 0, nothing to the continuity sum.
 // ------------------------------------------------------------------------------------------
 template <int DIM, bool MULTI, bool EXACT>
-__global__ void __launch_bounds__(PB, 6)
+__global__ void __launch_bounds__(PB, SPH_MINB)
 k_pass_a(const DP p, const SS* __restrict__ S, const int nf, const int init,
          const float4* __restrict__ A, const XB* __restrict__ R,
          const unsigned* __restrict__ K, const int* __restrict__ lbF,
@@ -601,7 +604,7 @@ k_pass_a(const DP p, const SS* __restrict__ S, const int nf, const int init,
 // Eq. 2.13-2.15 (readings A8, A9, A11), gravity, then the second half kick Eq. 2.22.
 // ------------------------------------------------------------------------------------------
 template <int DIM, bool MULTI, bool EXACT>
-__global__ void __launch_bounds__(PB, 6)
+__global__ void __launch_bounds__(PB, SPH_MINB)
 k_pass_b(const DP p, const SS* __restrict__ S, const int nf,
          const float4* __restrict__ A, const XB* __restrict__ R,
          const unsigned* __restrict__ K, const int* __restrict__ lbF,
