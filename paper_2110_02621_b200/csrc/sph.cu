@@ -52,6 +52,8 @@ struct sph_ctx {
   uint4* NLW = nullptr;    // fluid-wall neighbour lists, same layout with capsw slots
   int* NCW = nullptr;
   int capsw = 0;
+  uint4* NLF = nullptr;    // wall-fluid neighbour lists (per wall particle, capsw slots), written by the first wall pass of a step
+  int* NCF = nullptr;
   size_t npad = 0;
   unsigned *ID0 = nullptr, *ID1 = nullptr, *IDcur = nullptr, *IDnext = nullptr;
   unsigned *keyA = nullptr, *valA = nullptr, *keyB = nullptr, *valB = nullptr, *hist = nullptr,
@@ -132,7 +134,7 @@ int dalloc(sph_ctx* c, T** p, size_t count) {
 }
 
 void free_all(sph_ctx* c) {
-  void* ptrs[] = {c->R0, c->R1, c->TX, c->A, c->TB, c->ACC, c->SIG, c->DRHO, c->NL, c->NC, c->NLW, c->NCW, c->ID0, c->ID1,
+  void* ptrs[] = {c->R0, c->R1, c->TX, c->A, c->TB, c->ACC, c->SIG, c->DRHO, c->NL, c->NC, c->NLW, c->NCW, c->NLF, c->NCF, c->ID0, c->ID1,
                   c->keyA, c->valA, c->keyB, c->valB, c->hist, c->rowsum, c->lbF, c->lbW, c->WR,
                   c->WA, c->WN, c->WG, c->WK, c->WID, c->wnear, c->S, c->dt_seq, c->stat};
   for (void* p : ptrs)
@@ -193,9 +195,9 @@ void launch_wall(sph_ctx* c, cudaStream_t st, bool with_vel, const XB* R) {
   if (c->nw == 0 || c->nf == 0) return;
   const int grid = cdiv(c->nw, PB), nw = (int)c->nw;
   if (with_vel) {
-    WALL_DISPATCH(true, grid, st, c->dp, c->S, nw, c->WA, c->WR, c->WK, c->A, R, c->lbF);
+    WALL_DISPATCH(true, grid, st, c->dp, c->S, nw, c->WA, c->WR, c->WK, c->A, R, c->lbF, c->NLF, c->NCF, c->capsw);
   } else {
-    WALL_DISPATCH(false, grid, st, c->dp, c->S, nw, c->WA, c->WR, c->WK, c->A, R, c->lbF);
+    WALL_DISPATCH(false, grid, st, c->dp, c->S, nw, c->WA, c->WR, c->WK, c->A, R, c->lbF, c->NLF, c->NCF, c->capsw);
   }
 }
 
@@ -467,6 +469,7 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
   rc |= dalloc(c, &c->NL, c->npad * (size_t)(c->caps >> 2)); rc |= dalloc(c, &c->NC, nf);
   c->capsw = (c->caps * 3 / 4 + 3) & ~3;  // a particle in a corner of three walls has 7/8 of its (then smaller) support in them
   rc |= dalloc(c, &c->NLW, c->npad * (size_t)(c->capsw >> 2)); rc |= dalloc(c, &c->NCW, nf);
+  rc |= dalloc(c, &c->NLF, ((size_t)nw + PB - 1) / PB * PB * (size_t)(c->capsw >> 2)); rc |= dalloc(c, &c->NCF, nw);
   rc |= dalloc(c, &c->ID0, cap); rc |= dalloc(c, &c->ID1, cap);
   rc |= dalloc(c, &c->keyA, cap); rc |= dalloc(c, &c->valA, cap); rc |= dalloc(c, &c->keyB, cap);
   rc |= dalloc(c, &c->valB, cap);

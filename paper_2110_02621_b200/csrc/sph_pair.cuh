@@ -294,13 +294,14 @@ __device__ __forceinline__ void walk_q(const DP& p, const float4* __restrict__ A
 // List walk: every lane runs over its own column of the warp's neighbour groups; the loop is
 // warp-uniform (to the largest count in the warp), one coalesced 16-byte load gives 4 neighbours
 // whose records are gathered together before the arithmetic.
-template <class Body>
-__device__ __forceinline__ void walk_l(const uint4* __restrict__ g, const int cnt, Body& body) {
+// RO = false: the list was written by this thread earlier in the same kernel (no read-only path).
+template <bool RO = true, class Body>
+__device__ __forceinline__ void walk_l(const uint4* g, const int cnt, Body& body) {
   const int nm = __reduce_max_sync(FULL, cnt);
 #pragma unroll 1
   for (int k = 0; k < nm; k += 4) {
     if (k < cnt) {
-      const uint4 e = __ldg(g + (size_t)(k >> 2) * 32);
+      const uint4 e = RO ? __ldg(g + (size_t)(k >> 2) * 32) : g[(size_t)(k >> 2) * 32];
       decltype(body.load(0u)) ld[4];
       ld[0] = body.load(e.x);
       if (k + 1 < cnt) ld[1] = body.load(e.y);
@@ -473,18 +474,35 @@ k_build(const DP p, SS* __restrict__ S, const int nf, const float4* __restrict__
 // ------------------------------------------------------------------------------------------
 template <int DIM, bool MULTI, bool EXACT, bool WITH_VEL>
 __global__ void __launch_bounds__(PB)
-k_wall(const DP p, const SS* __restrict__ S, const int nw, const float4* __restrict__ WA,
+k_wall(const DP p, SS* __restrict__ S, const int nw, const float4* __restrict__ WA,
        XB* __restrict__ WR, const unsigned* __restrict__ WK,
-       const float4* __restrict__ A, const XB* __restrict__ R, const int* __restrict__ lbF) {
-  __shared__ unsigned qs[QCAP * PB];
-  unsigned* q = qs + threadIdx.x;
+       const float4* __restrict__ A, const XB* __restrict__ R, const int* __restrict__ lbF,
+       uint4* __restrict__ NLF, int* __restrict__ NCF, const int capsf) {
+  // The first wall pass of a step (WITH_VEL) filters the fluid candidates of every wall particle
+  // into a wall-fluid neighbour list; the second one (after pass A, same positions) only reads it.
   const int w0 = blockIdx.x * PB + threadIdx.x;
   const bool act = w0 < nw;
   const int w = act ? w0 : nw - 1;
-  const float4 ai = WA[w];
   const uint4 xi = WR[w].x;
-  int cx, cy, cz;
-  cell_of_key(p, WK[w], cx, cy, cz);
+  uint4* col = NLF + (size_t)(w0 >> 5) * (capsf >> 2) * 32 + (threadIdx.x & 31);
+  int cnt;
+  if (WITH_VEL) {
+    __shared__ unsigned qs[QCAP * PB];
+    const float4 ai = WA[w];
+    int cx, cy, cz;
+    cell_of_key(p, WK[w], cx, cy, cz);
+    ListSink sink(qs + threadIdx.x, col, capsf >> 2);
+    walk_f<DIM, EXACT, false>(p, A, lbF, act, ai, cx, cy, cz, nullptr, HCtx{}, sink);
+    cnt = min(sink.n, capsf);
+    if (act) {
+      NCF[w] = cnt;
+      if (sink.n > capsf) atomicMax(&S->list_overflow, sink.n);
+    }
+    __syncwarp();  // the list walk below reads what this lane wrote (same thread: program order suffices)
+  } else {
+    cnt = act ? NCF[w] : 0;
+  }
+  if (!act) cnt = 0;
   float sW = 0, sp = 0, sWr = 0, srx = 0, sry = 0, srz = 0, svx = 0, svy = 0, svz = 0;
   {
     auto body = make_body(R, [&](const uint4& xj, const float4& bj, const unsigned j) {
@@ -504,7 +522,7 @@ k_wall(const DP p, const SS* __restrict__ S, const int nw, const float4* __restr
     }
     if (WITH_VEL) { svx = fmaf(bj.x, g.w, svx); svy = fmaf(bj.y, g.w, svy); svz = fmaf(bj.z, g.w, svz); }
     });
-    walk_q<DIM, EXACT>(p, A, lbF, act, ai, cx, cy, cz, q, body);
+    walk_l<!WITH_VEL>(col, cnt, body);
   }
   if (!act) return;
   float pwall = 0.f, vx = 0.f, vy = 0.f, vz = 0.f;
