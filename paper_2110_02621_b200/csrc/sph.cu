@@ -15,6 +15,7 @@
 #include <string.h>
 
 #include <algorithm>
+#include <map>
 #include <string>
 #include <vector>
 
@@ -70,6 +71,9 @@ struct sph_ctx {
   int64_t dt_seq_cap = 0;
   StatAcc* stat = nullptr;
   int sort_passes = 1, sort_bits = 8;
+  std::map<void*, size_t> cap_bytes;  // dalloc: capacity of the buffer behind each pointer member
+  float *hpos = nullptr, *hvel = nullptr, *hrho = nullptr;  // staging of sph_set_particles_host
+  int32_t* htagd = nullptr;
   // one step captured as a CUDA graph (launch-bound small configurations); rebuilt after sph_set_particles
   cudaGraphExec_t gexec = nullptr;
   cudaStream_t cap_stream = nullptr;
@@ -125,18 +129,26 @@ namespace {
 
 inline int cdiv(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
 
+// Device buffer of at least `count` elements; a buffer that is already large enough is kept (a second
+// sph_set_particles of the same size allocates nothing: cudaMalloc / cudaFree cost more than the set-up kernels).
 template <typename T>
 int dalloc(sph_ctx* c, T** p, size_t count) {
-  if (*p) { cudaFree(*p); *p = nullptr; }
   if (count == 0) count = 1;
-  CK(cudaMalloc((void**)p, count * sizeof(T)));
+  const size_t bytes = count * sizeof(T);
+  auto it = c->cap_bytes.find((void*)p);
+  if (*p && it != c->cap_bytes.end() && it->second >= bytes) return SPH_OK;
+  if (*p) { cudaFree(*p); *p = nullptr; }
+  c->cap_bytes.erase((void*)p);
+  CK(cudaMalloc((void**)p, bytes));
+  c->cap_bytes[(void*)p] = bytes;
   return SPH_OK;
 }
 
 void free_all(sph_ctx* c) {
   void* ptrs[] = {c->R0, c->R1, c->TX, c->A, c->TB, c->ACC, c->SIG, c->DRHO, c->NL, c->NC, c->NLW, c->NCW, c->NLF, c->NCF, c->ID0, c->ID1,
                   c->keyA, c->valA, c->keyB, c->valB, c->hist, c->rowsum, c->lbF, c->lbW, c->WR,
-                  c->WA, c->WN, c->WG, c->WK, c->WID, c->wnear, c->S, c->dt_seq, c->stat};
+                  c->WA, c->WN, c->WG, c->WK, c->WID, c->wnear, c->S, c->dt_seq, c->stat,
+                  c->hpos, c->hvel, c->hrho, c->htagd};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   for (auto e : c->ev) cudaEventDestroy(e);
@@ -533,12 +545,11 @@ int sph_set_particles_host(sph_ctx* c, int64_t n, const float* pos, const float*
   if (!c) return SPH_EINVAL;
   if (n < 0 || (n > 0 && (!pos || !vel || !rho || !tag))) { c->err = "bad arguments"; return SPH_EINVAL; }
   cudaStream_t st = (cudaStream_t)stream;
-  float *dpos = nullptr, *dvel = nullptr, *drho = nullptr;
-  int32_t* dtag = nullptr;
   size_t m = (size_t)std::max<int64_t>(n, 1);
-  CK(cudaMalloc((void**)&dpos, m * 12)); CK(cudaMalloc((void**)&dvel, m * 12));
-  CK(cudaMalloc((void**)&drho, m * 4)); CK(cudaMalloc((void**)&dtag, m * 4));
-  int rc = SPH_OK;
+  int rc = dalloc(c, &c->hpos, m * 3) | dalloc(c, &c->hvel, m * 3) | dalloc(c, &c->hrho, m) | dalloc(c, &c->htagd, m);
+  if (rc) return rc;
+  float *dpos = c->hpos, *dvel = c->hvel, *drho = c->hrho;
+  int32_t* dtag = c->htagd;
   cudaError_t e = cudaSuccess;
   if (n) {
     e = cudaMemcpyAsync(dpos, pos, n * 12, cudaMemcpyHostToDevice, st);
@@ -549,7 +560,6 @@ int sph_set_particles_host(sph_ctx* c, int64_t n, const float* pos, const float*
   if (e != cudaSuccess) { c->err = cudaGetErrorString(e); rc = SPH_ECUDA; }
   if (rc == SPH_OK) rc = sph_set_particles(c, n, dpos, dvel, drho, dtag, stream);
   cudaStreamSynchronize(st);
-  cudaFree(dpos); cudaFree(dvel); cudaFree(drho); cudaFree(dtag);
   return rc;
 }
 
