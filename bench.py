@@ -43,14 +43,14 @@ UNIT = "fluid particle-steps/s"
 FLOPS_HIT = {"pass_a": 40.0, "pass_b": 50.0, "wall": 30.0}
 CAND_FLOPS = 8.0
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from `ncu --set full` captures of these
-# exact workloads (profiles/r01c_README.md); other workloads report traffic = null.
+# exact workloads (profiles/r01d_README.md); other workloads report traffic = null.
 NCU_TRAFFIC_BYTES = {
-    ("cfg1_dam_break_3d_box", "k_pass_a"): 263.07e6 + 20.68e6,
-    ("cfg1_dam_break_3d_box", "k_pass_b"): 264.77e6 + 17.90e6,
-    ("cfg1_dam_break_3d_box", "k_build"): 111.05e6 + 254.09e6,
-    ("cfg4_box_160", "k_pass_a"): 1614.1e6 + 158.9e6,
-    ("cfg4_box_160", "k_pass_b"): 1622.1e6 + 132.9e6,
-    ("cfg4_box_160", "k_build"): 719.7e6 + 1881.0e6,
+    ("cfg1_dam_break_3d_box", "k_pass_a"): 258.72e6 + 19.75e6,
+    ("cfg1_dam_break_3d_box", "k_pass_b"): 260.52e6 + 19.17e6,
+    ("cfg1_dam_break_3d_box", "k_build"): 86.55e6 + 235.02e6,
+    ("cfg4_box_160", "k_pass_a"): 1579.9e6 + 158.0e6,
+    ("cfg4_box_160", "k_pass_b"): 1588.0e6 + 143.2e6,
+    ("cfg4_box_160", "k_build"): 571.7e6 + 1768.3e6,
 }
 FP32_LANES_PER_SM = 128
 N_SM = 148
