@@ -168,6 +168,19 @@ int sph_debug_cells(sph_ctx* ctx, int32_t* cell_id_host, int32_t* perm_host,
 int sph_debug_neighbours(sph_ctx* ctx, int64_t* offsets_host, int32_t* ids_host, int64_t cap,
                          int64_t* total_host, void* stream);
 
+/* On-device probes (SURVEY.md section 8(f) NEXT-3; PAPER.md:296 pressure sensors, :304 water-level
+ * probes; the paper prints neither formula: readings A29 / A30 of DESIGN.md section 3).  m probes,
+ * xyz_host = m*3 floats (z ignored in 2-D); all pointers HOST, each call synchronises the stream; the
+ * state probed is the one sph_get_fields would return.
+ * sph_probe_pressure: p_host[k] = sum_f p_f W(|x_k - r_f|) / sum_f W over the fluid particles within
+ *   2h of x_k (Wendland C2, reading A1), 0 where there is none; wsum_host[k] = sum_f W (1/m^d).
+ * sph_probe_gauge: eta_host[k] = max { z_f + dp/2 : phase 0, horizontal distance to (x_k[, y_k]) < h }
+ *   ("z" is y in 2-D), NaN where there is no such particle.
+ * Errors: SPH_EINVAL (NULL pointers, m < 0, no particles), SPH_ECUDA. */
+int sph_probe_pressure(sph_ctx* ctx, int32_t m, const float* xyz_host, float* p_host, float* wsum_host,
+                       void* stream);
+int sph_probe_gauge(sph_ctx* ctx, int32_t m, const float* xyz_host, float* eta_host, void* stream);
+
 /* Checks the step's fluid-fluid neighbour lists (built once per step by the candidate filter,
  * DESIGN.md section 5) against the float32 contract of reading A24 on the current positions:
  * out3_host[0] = contract neighbours missing from a list (must be 0: the filter is conservative),

@@ -27,6 +27,7 @@ namespace {
 #include "sph_aux.cuh"
 #include "sph_pair.cuh"
 #include "sph_debug.cuh"
+#include "sph_probe.cuh"
 }  // namespace
 
 // ============================================================================================
@@ -757,6 +758,33 @@ int sph_debug_neighbours(sph_ctx* c, int64_t* offsets, int32_t* ids, int64_t cap
   }
   cudaFree(dcnt);
   return rc;
+}
+
+static int probe_common(sph_ctx* c, int32_t m, const float* xyz, float* o1, float* o2, int gauge, void* stream) {
+  if (!c || m < 0 || (m > 0 && (!xyz || !o1 || (!gauge && !o2)))) { if (c) c->err = "bad arguments"; return SPH_EINVAL; }
+  if (!c->loaded) { c->err = "no particles"; return SPH_EINVAL; }
+  if (m == 0) return SPH_OK;
+  cudaStream_t st = (cudaStream_t)stream;
+  float* d = nullptr;
+  CK(cudaMalloc((void**)&d, (size_t)m * 5 * sizeof(float)));
+  cudaError_t e = cudaMemcpyAsync(d, xyz, (size_t)m * 12, cudaMemcpyHostToDevice, st);
+  const int nf = (int)c->nf;
+  if (gauge) LAUNCH(k_probe_gauge, m, 256, st, c->dp, nf, m, d, c->R1, d + 3 * m);
+  else LAUNCH(k_probe_pressure, m, 32, st, c->dp, nf, m, d, c->R1, c->lbF, d + 3 * m, d + 4 * m);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(o1, d + 3 * m, (size_t)m * 4, cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess && !gauge) e = cudaMemcpyAsync(o2, d + 4 * m, (size_t)m * 4, cudaMemcpyDeviceToHost, st);
+  cudaError_t e2 = cudaStreamSynchronize(st);
+  cudaFree(d);
+  if (e != cudaSuccess || e2 != cudaSuccess) { c->err = cudaGetErrorString(e != cudaSuccess ? e : e2); return SPH_ECUDA; }
+  return SPH_OK;
+}
+
+int sph_probe_pressure(sph_ctx* c, int32_t m, const float* xyz, float* p_out, float* wsum_out, void* stream) {
+  return probe_common(c, m, xyz, p_out, wsum_out, 0, stream);
+}
+
+int sph_probe_gauge(sph_ctx* c, int32_t m, const float* xyz, float* eta_out, void* stream) {
+  return probe_common(c, m, xyz, eta_out, nullptr, 1, stream);
 }
 
 int sph_debug_list_check(sph_ctx* c, int64_t* out3, void* stream) {

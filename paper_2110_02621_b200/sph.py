@@ -48,7 +48,7 @@ class SphStats(C.Structure):
 EXPORTS = (
     "sph_create", "sph_destroy", "sph_set_particles", "sph_set_particles_host", "sph_step",
     "sph_step_dt", "sph_get_fields", "sph_get_fields_host", "sph_get_stats", "sph_get_stats_ex", "sph_set_profiling",
-    "sph_get_timings", "sph_num_cells", "sph_debug_cells", "sph_debug_neighbours", "sph_debug_list_check",
+    "sph_get_timings", "sph_num_cells", "sph_debug_cells", "sph_debug_neighbours", "sph_debug_list_check", "sph_probe_pressure", "sph_probe_gauge",
     "sph_debug_normals", "sph_debug_sigma", "sph_launch_count", "sph_last_error",
 )
 
@@ -82,6 +82,8 @@ def load():
     L.sph_debug_neighbours.restype = C.c_int; L.sph_debug_neighbours.argtypes = [vp, vp, vp, i64, vp, vp]
     L.sph_debug_normals.restype = C.c_int; L.sph_debug_normals.argtypes = [vp, vp, vp]
     L.sph_debug_list_check.restype = C.c_int; L.sph_debug_list_check.argtypes = [vp, vp, vp]
+    L.sph_probe_pressure.restype = C.c_int; L.sph_probe_pressure.argtypes = [vp, C.c_int32, vp, vp, vp, vp]
+    L.sph_probe_gauge.restype = C.c_int; L.sph_probe_gauge.argtypes = [vp, C.c_int32, vp, vp, vp]
     L.sph_debug_sigma.restype = C.c_int; L.sph_debug_sigma.argtypes = [vp, vp, vp]
     L.sph_launch_count.restype = i64; L.sph_launch_count.argtypes = [vp]
     L.sph_last_error.restype = C.c_char_p; L.sph_last_error.argtypes = [vp]
@@ -234,6 +236,20 @@ class Sph:
         ids = np.zeros(max(tot.value, 1), np.int32)
         self._ck(self.L.sph_debug_neighbours(self.ctx, _hp(off), _hp(ids), tot.value, C.byref(tot), self._st()))
         return off, ids[:tot.value]
+
+    def probe_pressure(self, points):
+        """Shepard-averaged fluid pressure at points (m,3) -> (p (m,), wsum (m,)); reading A29."""
+        pts = np.ascontiguousarray(points, np.float32).reshape(-1, 3)
+        p = np.zeros(len(pts), np.float32); w = np.zeros(len(pts), np.float32)
+        self._ck(self.L.sph_probe_pressure(self.ctx, len(pts), _hp(pts), _hp(p), _hp(w), self._st()))
+        return p, w
+
+    def probe_gauge(self, points):
+        """Free-surface height of phase 0 at the horizontal positions of points (m,3); reading A30."""
+        pts = np.ascontiguousarray(points, np.float32).reshape(-1, 3)
+        eta = np.zeros(len(pts), np.float32)
+        self._ck(self.L.sph_probe_gauge(self.ctx, len(pts), _hp(pts), _hp(eta), self._st()))
+        return eta
 
     def debug_list_check(self):
         """(missing, extra, total) of the step's neighbour lists against the float32 contract."""

@@ -416,3 +416,42 @@ def test_neighbour_list_overflow_is_reported_not_dropped():
     g2 = sph.Sph(ok)
     g2.set_particles(cfg["pos"], cfg["vel"], cfg["rho"], cfg["tag"])
     assert g2.get_stats()["rc"] == 0
+
+
+# ------------------------------------------------------------------------- probes (NEXT-3, readings A29 / A30)
+@pytest.mark.parametrize("name,steps", [("cfg0", 30), ("box3d_13", 5), ("box2d_two_phase", 10)])
+def test_probes_match_oracle(name, steps):
+    """sph_probe_pressure / sph_probe_gauge against oracle/probes.py evaluated on the ORACLE's own
+    state after the same steps (same dt sequence): pressures to 1e-4 of rho0 g H, kernel sums to
+    1e-4 relative, gauges to 1e-5 H (the surface particle is the same one on both sides)."""
+    from oracle import probes
+    cfg = SMALL[name]
+    o, g = make_pair(cfg)
+    dts = []
+    for _ in range(steps):
+        dts.append(o.step(1))
+    g.step(steps, dts=np.asarray(dts, np.float64).ravel())
+    fo = o.fields()
+    dim, dp, H = cfg["dim"], cfg["dp"], float(cfg.get("H", 1.0))
+    fl = cfg["tag"] >= 0
+    lo, hi = fo["pos"][fl].min(0), fo["pos"][fl].max(0)
+    rng = np.random.default_rng(17)
+    pts = lo + rng.random((24, 3)) * (hi - lo)
+    pts[:4] += 3.0 * dp * (rng.random((4, 3)) - 0.5)        # some near or beyond the fluid's edge
+    pts[4] = lo - 10.0 * dp                                  # one with no fluid in reach
+    if dim == 2:
+        pts[:, 2] = 0.0
+    pts = pts.astype(np.float32)
+    p_ref, w_ref = probes.pressure_probes(cfg, fo["pos"], fo["p"], cfg["tag"], pts.astype(np.float64))
+    p_gpu, w_gpu = g.probe_pressure(pts)
+    S = cfg["rho0"][0] * float(np.linalg.norm(cfg["g"]) or 1.0) * H
+    assert np.max(np.abs(p_gpu - p_ref)) / S < TOL
+    assert np.max(np.abs(w_gpu - w_ref) / np.maximum(w_ref, 1e-3 * w_ref.max())) < TOL
+    assert p_gpu[4] == 0.0 and w_gpu[4] == 0.0
+    e_ref = probes.wave_gauges(cfg, fo["pos"], cfg["tag"], pts.astype(np.float64))
+    e_gpu = g.probe_gauge(pts)
+    assert np.array_equal(np.isnan(e_ref), np.isnan(e_gpu)) and np.isnan(e_gpu[4])
+    ok = ~np.isnan(e_ref)
+    assert ok.sum() >= 10
+    assert np.max(np.abs(e_gpu[ok] - e_ref[ok])) < 1e-5 * H
+    assert g.probe_pressure(np.zeros((0, 3), np.float32))[0].shape == (0,)

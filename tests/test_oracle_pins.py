@@ -460,3 +460,74 @@ def test_long_run_keeps_particles_inside_P17():
     s = o.stats()
     assert s["escaped"] == 0 and s["mass"] == pytest.approx(2000.0, rel=1e-12)
     assert 1.2 < s["x_front"] < 4.0 and s["ek"] > 0
+
+
+# ------------------------------------------------------------------------- probes (readings A29, A30)
+def _lattice_block(dim, n, dp):
+    ax = (np.arange(n) + 0.5) * dp
+    g = np.meshgrid(*([ax] * dim), indexing="ij")
+    pos = np.stack([a.ravel() for a in g], 1)
+    if dim == 2:
+        pos = np.concatenate([pos, np.zeros((len(pos), 1))], 1)
+    return pos
+
+
+@pytest.mark.parametrize("dim", [2, 3])
+def test_P19_pressure_probe_constant_linear_and_kernel_values(dim):
+    """oracle/probes.py, reading A29.  (i) Normalised average of a constant is the constant at any
+    point; (ii) of a field linear in the coordinates, at a point about which the lattice is
+    symmetric (a particle site or a cell centre), the field's value there — the first moments cancel
+    by symmetry; (iii) the kernel it uses has the Wendland C2 values W(0) = alpha_d and
+    W(h) = alpha_d (1/2)^4 * 3 and vanishes at 2h (closed forms, not the oracle's C routine);
+    (iv) no fluid within 2h gives 0; walls do not count."""
+    from oracle import probes
+    dp, n = 0.02, 12
+    h = 1.3 * dp
+    pos = _lattice_block(dim, n, dp)
+    tag = np.zeros(len(pos), np.int32)
+    cfg = dict(dim=dim, h=h, dp=dp)
+    up = dim - 1
+    rng = np.random.default_rng(5)
+    pts = np.zeros((4, 3))
+    pts[:, :dim] = 0.5 * n * dp + (rng.random((4, dim)) - 0.5) * 2 * dp
+    pc, ws = probes.pressure_probes(cfg, pos, np.full(len(pos), 123.5), tag, pts)
+    assert np.allclose(pc, 123.5, rtol=1e-13) and np.all(ws > 0)
+    # linear field a + b.x at a site and at a cell centre
+    b = np.array([3.0, -7.0, 11.0])[:dim]
+    field = 5.0 + pos[:, :dim] @ b
+    site = np.zeros(3); site[:dim] = (n // 2 + 0.5) * dp          # an interior particle site
+    centre = site.copy(); centre[:dim] += 0.5 * dp
+    for x in (site, centre):
+        got, _ = probes.pressure_probes(cfg, pos, field, tag, x[None, :])
+        assert got[0] == pytest.approx(5.0 + x[:dim] @ b, rel=1e-12)
+    alpha = 7.0 / (4 * math.pi * h * h) if dim == 2 else 21.0 / (16 * math.pi * h ** 3)
+    assert probes.wendland_c2(0.0, h, dim) == pytest.approx(alpha, rel=1e-14)
+    assert probes.wendland_c2(h, h, dim) == pytest.approx(alpha * 3.0 / 16.0, rel=1e-14)
+    assert probes.wendland_c2(2.0 * h, h, dim) == 0.0 and probes.wendland_c2(1.999 * h, h, dim) > 0.0
+    # one particle: the sum of weights at distance r is W(r), the average is its pressure
+    one = np.zeros((1, 3)); x = np.zeros((1, 3)); x[0, 0] = 0.7 * h
+    got, ws = probes.pressure_probes(cfg, one, np.array([42.0]), np.zeros(1, np.int32), x)
+    assert got[0] == pytest.approx(42.0) and ws[0] == pytest.approx(alpha * (1 - 0.35) ** 4 * (1 + 1.4), rel=1e-13)
+    far = np.full((1, 3), 10.0); far[0, 2] = 0.0 if dim == 2 else 10.0
+    got, ws = probes.pressure_probes(cfg, pos, field, tag, far)
+    assert got[0] == 0.0 and ws[0] == 0.0
+    got, ws = probes.pressure_probes(cfg, pos, field, np.full(len(pos), -1, np.int32), site[None, :])
+    assert got[0] == 0.0 and ws[0] == 0.0
+
+
+@pytest.mark.parametrize("dim", [2, 3])
+def test_P20_wave_gauge_of_a_resting_block(dim):
+    """oracle/probes.py, reading A30: a block of n layers at spacing dp whose lowest layer sits at
+    dp/2 gauges n dp = H; only phase 0 counts; a gauge with no particle within h horizontally is NaN."""
+    from oracle import probes
+    dp, n = 0.05, 8
+    pos = _lattice_block(dim, n, dp)
+    cfg = dict(dim=dim, h=1.3 * dp, dp=dp)
+    up = dim - 1
+    tag = np.zeros(len(pos), np.int32)
+    pts = np.zeros((2, 3)); pts[0, :up] = 0.5 * n * dp; pts[1, :up] = -3.0
+    eta = probes.wave_gauges(cfg, pos, tag, pts)
+    assert eta[0] == pytest.approx(n * dp, rel=1e-14) and np.isnan(eta[1])
+    tag2 = tag.copy(); tag2[pos[:, up] > 0.5 * n * dp] = 1            # upper half is the light phase
+    eta = probes.wave_gauges(cfg, pos, tag2, pts)
+    assert eta[0] == pytest.approx(0.5 * n * dp, rel=1e-14)
