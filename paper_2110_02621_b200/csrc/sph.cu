@@ -166,15 +166,13 @@ int radix_sort(sph_ctx* c, cudaStream_t st, int n, unsigned* kA, unsigned* vA, u
     for (int pass = 0; pass < c->sort_passes; ++pass) {
       int shift = c->sort_bits * pass;
       if (c->sort_bits == 9) {
-        LAUNCH(k_radix_hist<512>, nblk, RS_THREADS, st, ki, n, shift, c->hist, nblk);
-        LAUNCH(k_scan_rowsum, 512, 256, st, c->hist, nblk, c->rowsum);
+        LAUNCH(k_radix_hist<512>, nblk, RS_THREADS, st, ki, n, shift, c->hist, nblk, c->rowsum);
         LAUNCH(k_scan_apply, 512, 256, st, c->hist, nblk, c->rowsum);
-        LAUNCH(k_radix_scatter<512>, nblk, RS_THREADS, st, ki, vi, n, shift, c->hist, nblk, kt, vt);
+        LAUNCH(k_radix_scatter<512>, nblk, RS_THREADS, st, ki, vi, n, shift, c->hist, nblk, kt, vt, c->rowsum);
       } else {
-        LAUNCH(k_radix_hist<256>, nblk, RS_THREADS, st, ki, n, shift, c->hist, nblk);
-        LAUNCH(k_scan_rowsum, 256, 256, st, c->hist, nblk, c->rowsum);
+        LAUNCH(k_radix_hist<256>, nblk, RS_THREADS, st, ki, n, shift, c->hist, nblk, c->rowsum);
         LAUNCH(k_scan_apply, 256, 256, st, c->hist, nblk, c->rowsum);
-        LAUNCH(k_radix_scatter<256>, nblk, RS_THREADS, st, ki, vi, n, shift, c->hist, nblk, kt, vt);
+        LAUNCH(k_radix_scatter<256>, nblk, RS_THREADS, st, ki, vi, n, shift, c->hist, nblk, kt, vt, c->rowsum);
       }
       std::swap(ki, kt);
       std::swap(vi, vt);
@@ -223,20 +221,22 @@ int pipeline_after_hash(sph_ctx* c, cudaStream_t st, int init, Prof& pf) {
   c->K = ks;
   pf.mark();  // end sort
   if (nf > 0) {
-    LAUNCH(k_reorder, cdiv(nf, 256), 256, st, c->dp, nf, vs, c->TX, c->TB, c->IDcur, c->R0, c->A, c->IDnext);
-    // no pointer ping-pong: every step then issues the same launches with the same arguments (CUDA graph)
-    CK(cudaMemcpyAsync(c->IDcur, c->IDnext, sizeof(unsigned) * nf, cudaMemcpyDeviceToDevice, st));
+    // reorder + cell lower bounds in one launch; no pointer ping-pong: every step issues the same launches
+    // with the same arguments (CUDA graph), k_build copies IDnext back to IDcur
+    LAUNCH(k_reorder, std::max(cdiv(nf, 256), cdiv(c->ncell + 1, 256)), 256, st, c->dp, nf, vs, c->TX, c->TB, c->IDcur,
+           c->R0, c->A, c->IDnext, ks, (int)c->ncell, c->lbF);
+  } else {
+    LAUNCH(k_cell_bounds, cdiv(c->ncell + 1, 256), 256, st, ks, nf, (int)c->ncell, c->lbF);
   }
-  LAUNCH(k_cell_bounds, cdiv(c->ncell + 1, 256), 256, st, ks, nf, (int)c->ncell, c->lbF);
   pf.mark();  // end reorder
   launch_wall(c, st, true, c->R0);
   pf.mark();  // end wall 1
   if (nf > 0) {
     switch (PAIR_SEL(c) & 5) {  // DIM x EXACT
-      case 0: LAUNCH((k_build<2, false>), cdiv(nf, PB), PB, st, c->dp, c->S, nf, c->A, c->K, c->lbF, c->NL, c->NC, c->caps, c->WA, c->lbW, c->wnear, c->NLW, c->NCW, c->capsw); break;
-      case 1: LAUNCH((k_build<2, true>), cdiv(nf, PB), PB, st, c->dp, c->S, nf, c->A, c->K, c->lbF, c->NL, c->NC, c->caps, c->WA, c->lbW, c->wnear, c->NLW, c->NCW, c->capsw); break;
-      case 4: LAUNCH((k_build<3, false>), cdiv(nf, PB), PB, st, c->dp, c->S, nf, c->A, c->K, c->lbF, c->NL, c->NC, c->caps, c->WA, c->lbW, c->wnear, c->NLW, c->NCW, c->capsw); break;
-      default: LAUNCH((k_build<3, true>), cdiv(nf, PB), PB, st, c->dp, c->S, nf, c->A, c->K, c->lbF, c->NL, c->NC, c->caps, c->WA, c->lbW, c->wnear, c->NLW, c->NCW, c->capsw); break;
+      case 0: LAUNCH((k_build<2, false>), cdiv(nf, PB), PB, st, c->dp, c->S, nf, c->A, c->K, c->lbF, c->NL, c->NC, c->caps, c->WA, c->lbW, c->wnear, c->NLW, c->NCW, c->capsw, c->IDcur, c->IDnext); break;
+      case 1: LAUNCH((k_build<2, true>), cdiv(nf, PB), PB, st, c->dp, c->S, nf, c->A, c->K, c->lbF, c->NL, c->NC, c->caps, c->WA, c->lbW, c->wnear, c->NLW, c->NCW, c->capsw, c->IDcur, c->IDnext); break;
+      case 4: LAUNCH((k_build<3, false>), cdiv(nf, PB), PB, st, c->dp, c->S, nf, c->A, c->K, c->lbF, c->NL, c->NC, c->caps, c->WA, c->lbW, c->wnear, c->NLW, c->NCW, c->capsw, c->IDcur, c->IDnext); break;
+      default: LAUNCH((k_build<3, true>), cdiv(nf, PB), PB, st, c->dp, c->S, nf, c->A, c->K, c->lbF, c->NL, c->NC, c->caps, c->WA, c->lbW, c->wnear, c->NLW, c->NCW, c->capsw, c->IDcur, c->IDnext); break;
     }
   }
   pf.mark();  // end list build
@@ -488,6 +488,7 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
   rc |= dalloc(c, &c->valB, cap);
   rc |= dalloc(c, &c->hist, (size_t)512 * cdiv(std::max<size_t>(cap, 1), RS_TILE));
   rc |= dalloc(c, &c->rowsum, 512);
+  if (!rc) CK(cudaMemsetAsync(c->rowsum, 0, 512 * sizeof(unsigned), (cudaStream_t)stream));  // radix digit totals: zero between passes
   rc |= dalloc(c, &c->lbF, c->ncell + 1); rc |= dalloc(c, &c->lbW, c->ncell + 1);
   rc |= dalloc(c, &c->wnear, c->ncell);
   rc |= dalloc(c, &c->WR, nw); rc |= dalloc(c, &c->WA, (size_t)nw + 16);
@@ -513,7 +514,8 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
     unsigned *ks, *vs;
     rc = radix_sort(c, st, nw, c->keyA, c->valA, c->keyB, c->valB, &ks, &vs);
     if (rc) { cudaFree(idx); return rc; }
-    LAUNCH(k_reorder, cdiv(nw, 256), 256, st, c->dp, nw, vs, c->TX, c->TB, c->ID0, c->WR, c->WA, c->WID);
+    LAUNCH(k_reorder, cdiv(nw, 256), 256, st, c->dp, nw, vs, c->TX, c->TB, c->ID0, c->WR, c->WA, c->WID,
+           (const unsigned*)nullptr, -1, (int*)nullptr);
     CK(cudaMemcpyAsync(c->WK, ks, sizeof(unsigned) * nw, cudaMemcpyDeviceToDevice, st));
     LAUNCH(k_image, cdiv(nw, 256), 256, st, c->dp, nw, c->WR, c->WG);
     LAUNCH(k_cell_bounds, cdiv(c->ncell + 1, 256), 256, st, ks, nw, (int)c->ncell, c->lbW);

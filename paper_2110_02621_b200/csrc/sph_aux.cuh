@@ -35,12 +35,25 @@ __global__ void k_load(DP p, int n, int is_wall, const int* __restrict__ idx, co
   vals[i] = (unsigned)i;
 }
 
-// Gather into cell-sorted order and derive the centred float32 image used by the candidate filter.
+// Gather into cell-sorted order and derive the centred float32 image used by the candidate filter;
+// the same launch computes the cell lower bounds (one thread per cell, independent work: one graph
+// node less per step).  lb[c] = number of sorted particles with key < c, c = 0..ncell: the three cells
+// of an x-row of the stencil are one contiguous range [lb[c0], lb[c1+1]).  Binary search in the
+// sorted keys (the tank may be mostly dry: no serial gap filling).
 __global__ void __launch_bounds__(256)
 k_reorder(DP p, int n, const unsigned* __restrict__ vals, const uint4* __restrict__ TX,
           const float4* __restrict__ TB, const unsigned* __restrict__ IDin, XB* __restrict__ R,
-          float4* __restrict__ A, unsigned* __restrict__ IDout) {
+          float4* __restrict__ A, unsigned* __restrict__ IDout,
+          const unsigned* __restrict__ keys, int ncell, int* __restrict__ lb) {
   const int s = blockIdx.x * 256 + threadIdx.x;
+  if (s <= ncell) {
+    int lo = 0, hi = n;
+    while (lo < hi) {
+      const int mid = (lo + hi) >> 1;
+      if (keys[mid] < (unsigned)s) lo = mid + 1; else hi = mid;
+    }
+    lb[s] = lo;
+  }
   if (s >= n) return;
   const unsigned v = vals[s];
   const uint4 x = TX[v];

@@ -430,7 +430,8 @@ k_build(const DP p, SS* __restrict__ S, const int nf, const float4* __restrict__
         const unsigned* __restrict__ K, const int* __restrict__ lbF, uint4* __restrict__ NL,
         int* __restrict__ NC, const int caps,
         const float4* __restrict__ WA, const int* __restrict__ lbW, const unsigned char* __restrict__ wnear,
-        uint4* __restrict__ NLW, int* __restrict__ NCW, const int capsw) {
+        uint4* __restrict__ NLW, int* __restrict__ NCW, const int capsw,
+        unsigned* __restrict__ IDcur, const unsigned* __restrict__ IDnext) {
   __shared__ unsigned qs[QCAP * PB];
   __shared__ HTile tiles[PB / 32];
   const int i0 = blockIdx.x * PB + threadIdx.x;
@@ -461,6 +462,7 @@ k_build(const DP p, SS* __restrict__ S, const int nf, const float4* __restrict__
     nw = sink.n;
   }
   if (act) {
+    IDcur[i] = IDnext[i];  // caller ids of the new order (k_reorder wrote IDnext from IDcur: no ping-pong of pointers)
     NC[i] = min(n, caps);
     NCW[i] = min(nw, capsw);
     if (n > caps) atomicMax(&S->list_overflow, n);

@@ -3,17 +3,18 @@
 // ------------------------------------------------------------------------------------------
 // Device radix sort (stable LSD) of (cell id, index).  Digits of RB = 8 or 9 bits (ND = 256 / 512
 // bins), whichever needs fewer passes for the grid's cell count: 17-18 bit cell ids (cfg1, cfg4 up
-// to 4 M) sort in 2 passes of 9 bits instead of 3 of 8; a pass is 4 dependent launches and at
+// to 4 M) sort in 2 passes of 9 bits instead of 3 of 8; a pass is 3 dependent launches and at
 // these sizes latency-bound.  BASELINE.json north_star
 // "cell hash, device radix sort"; the paper only names the step.
-// Per pass: tile histograms -> row sums -> scan -> stable scatter with warp match ranking.
+// Per pass: tile histograms (+ per-digit totals by atomics) -> scan -> stable scatter with warp match
+// ranking: 3 dependent launches.
 // ------------------------------------------------------------------------------------------
 constexpr int RS_THREADS = 256, RS_ITEMS = 16, RS_TILE = RS_THREADS * RS_ITEMS, RS_WARPS = 8;
 
 template <int ND>
 __global__ void __launch_bounds__(RS_THREADS)
 k_radix_hist(const unsigned* __restrict__ keys, int n, int shift, unsigned* __restrict__ hist,
-             int nblk) {
+             int nblk, unsigned* __restrict__ rowsum) {
   __shared__ unsigned h[ND];
   for (int d = threadIdx.x; d < ND; d += RS_THREADS) h[d] = 0;
   __syncthreads();
@@ -28,23 +29,9 @@ k_radix_hist(const unsigned* __restrict__ keys, int n, int shift, unsigned* __re
     if (ok && lane == __ffs(peers) - 1) atomicAdd(&h[d], (unsigned)__popc(peers));
   }
   __syncthreads();
-  for (int d = threadIdx.x; d < ND; d += RS_THREADS) hist[d * nblk + blockIdx.x] = h[d];
-}
-
-__global__ void __launch_bounds__(256)
-k_scan_rowsum(const unsigned* __restrict__ hist, int nblk, unsigned* __restrict__ rowsum) {
-  __shared__ unsigned sm[8];
-  unsigned s = 0;
-  const unsigned* row = hist + (size_t)blockIdx.x * nblk;
-  for (int i = threadIdx.x; i < nblk; i += 256) s += row[i];
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(FULL, s, o);
-  if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = s;
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    unsigned t = 0;
-    for (int w = 0; w < 8; ++w) t += sm[w];
-    rowsum[blockIdx.x] = t;
+  for (int d = threadIdx.x; d < ND; d += RS_THREADS) {
+    hist[d * nblk + blockIdx.x] = h[d];
+    if (h[d]) atomicAdd(&rowsum[d], h[d]);  // per-digit totals (zeroed by the previous scatter): no separate row-sum launch
   }
 }
 
@@ -93,7 +80,9 @@ template <int ND>
 __global__ void __launch_bounds__(RS_THREADS)
 k_radix_scatter(const unsigned* __restrict__ keys, const unsigned* __restrict__ vals, int n, int shift,
                 const unsigned* __restrict__ hist, int nblk, unsigned* __restrict__ keys_out,
-                unsigned* __restrict__ vals_out) {
+                unsigned* __restrict__ vals_out, unsigned* __restrict__ rowsum) {
+  if (blockIdx.x == 0)  // the scan has consumed the digit totals: clear them for the next pass's histogram
+    for (int d = threadIdx.x; d < ND; d += RS_THREADS) rowsum[d] = 0;
   __shared__ unsigned wc[RS_WARPS][ND];
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   for (int i = threadIdx.x; i < RS_WARPS * ND; i += RS_THREADS) (&wc[0][0])[i] = 0;
