@@ -52,6 +52,14 @@ NCU_TRAFFIC_BYTES = {
     ("cfg4_box_160", "k_pass_b"): 1588.0e6 + 143.2e6,
     ("cfg4_box_160", "k_build"): 571.7e6 + 1768.3e6,
 }
+# l1tex__data_pipe_lsu_wavefronts (fraction of peak) and sm__issue_active of the same captures: the pair
+# passes are bound by the tag stage of L1 (record gathers), not by FP32 issue.
+NCU_L1_ISSUE = {
+    ("cfg1_dam_break_3d_box", "k_pass_a"): (0.760, 0.547),
+    ("cfg1_dam_break_3d_box", "k_pass_b"): (0.748, 0.559),
+    ("cfg4_box_160", "k_pass_a"): (0.859, 0.606),
+    ("cfg4_box_160", "k_pass_b"): (0.887, 0.650),
+}
 FP32_LANES_PER_SM = 128
 N_SM = 148
 
@@ -312,6 +320,8 @@ def run_gpu(args):
     roofline = {"bound": "alu", "kernel": "k_" + dom, "achieved": kern[dom]["tflops_hit_only"],
                 "peak": peak, "unit": "TFLOP/s", "frac": kern[dom]["frac_hit_only"],
                 "traffic": NCU_TRAFFIC_BYTES.get((cfg["name"], "k_" + dom)),
+                "l1_data_pipe_frac_ncu": (NCU_L1_ISSUE.get((cfg["name"], "k_" + dom)) or (None, None))[0],
+                "issue_active_frac_ncu": (NCU_L1_ISSUE.get((cfg["name"], "k_" + dom)) or (None, None))[1],
                 "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 flop x clocks.max.sm (DESIGN.md §7); MEASURED_PEAKS.json holds no non-tensor FP32 peak",
                 "flops_per_hit": FLOPS_HIT[dom], "flops_per_candidate": CAND_FLOPS,
                 # list build + pass A + pass B together (the candidate walk is k_build's):
