@@ -93,17 +93,20 @@ struct ListSink {
     asm volatile("st.shared.u32 [%0], %1;" ::"r"(qa), "r"(j) : "memory");
     qa += PB * 4;
   }
-  // Two candidates at once: r2 and thr are half2; candidate u (index kk + u in the lane's range of
-  // len entries, list index j0 + u) is pushed iff r2.u < thr.u and 0 <= kk + u < len.
-  __device__ __forceinline__ void push2(const unsigned r2, const unsigned thr, const int kk, const int len, const unsigned j0) {
+  // Two candidates at once: r2 and thr are half2; candidates C and C + 1 of the chunk (list indices
+  // j0 and j0 + 1) are pushed iff r2 < thr, C (+1) < rem (the lane's remaining range) and, for the
+  // first one, ok0 (false only for the padding candidate in front of an odd range start).
+  template <int C>
+  __device__ __forceinline__ void push2(const unsigned r2, const unsigned thr, const int rem, const int ok0, const unsigned j0) {
     asm volatile(
         "{\n"
-        ".reg .pred p, q;\n"
+        ".reg .pred p, q, v;\n"
         ".reg .u32 t;\n"
         "setp.lt.f16x2 p|q, %1, %2;\n"
-        "setp.lt.and.u32 p, %3, %4, p;\n"
-        "add.u32 t, %3, 1;\n"
-        "setp.lt.and.u32 q, t, %4, q;\n"
+        "setp.ne.s32 v, %4, 0;\n"
+        "and.pred p, p, v;\n"
+        "setp.gt.and.s32 p, %3, %7, p;\n"
+        "setp.gt.and.s32 q, %3, %8, q;\n"
         "@p st.shared.u32 [%0], %5;\n"
         "@p add.u32 %0, %0, %6;\n"
         "add.u32 t, %5, 1;\n"
@@ -111,7 +114,7 @@ struct ListSink {
         "@q add.u32 %0, %0, %6;\n"
         "}"
         : "+r"(qa)
-        : "r"(r2), "r"(thr), "r"(kk), "r"(len), "r"(j0), "n"(PB * 4)
+        : "r"(r2), "r"(thr), "r"(rem), "r"(ok0), "r"(j0), "n"(PB * 4), "n"(C), "n"(C + 1)
         : "memory");
   }
   __device__ __forceinline__ void flush(const bool last) {
@@ -243,18 +246,24 @@ __device__ __forceinline__ void walk_f(const DP& p, const float4* __restrict__ A
             xy[u] = tile->xy[pi + u];
             if (DIM == 3) zz[u] = tile->z[pi + u];
           }
-          const int kk = 2 * kp - odd;           // index of the chunk's first candidate in the lane's range
+          const int rem = odd + len - 2 * kp;    // candidates C of this chunk with C < rem are in the lane's range,
+          const int ok0 = (kp > 0) | (odd ^ 1);  // except the one in front of an odd range start
           const unsigned j0 = (unsigned)(t0 + 2 * (pb + kp));
+          unsigned r2[CHS / 2];
 #pragma unroll
           for (int u = 0; u < CHS / 2; ++u) {
             const unsigned dx = hsub2(hc.xi, xy[u].x), dy = hsub2(hc.yi, xy[u].y);
-            unsigned r2 = hfma2(dy, dy, hmul2(dx, dx));
+            r2[u] = hfma2(dy, dy, hmul2(dx, dx));
             if (DIM == 3) {
               const unsigned dz = hsub2(hc.zi, zz[u]);
-              r2 = hfma2(dz, dz, r2);
+              r2[u] = hfma2(dz, dz, r2[u]);
             }
-            sink.push2(r2, p.thr_h2, kk + 2 * u, len, j0 + 2 * u);
           }
+          static_assert(CHS == 8, "four pair records per chunk");
+          sink.template push2<0>(r2[0], p.thr_h2, rem, ok0, j0);
+          sink.template push2<2>(r2[1], p.thr_h2, rem, 1, j0 + 2);
+          sink.template push2<4>(r2[2], p.thr_h2, rem, 1, j0 + 4);
+          sink.template push2<6>(r2[3], p.thr_h2, rem, 1, j0 + 6);
           sink.after_chunk(CHS);
         }
       }
