@@ -75,6 +75,8 @@ struct sph_ctx {
   std::map<void*, size_t> cap_bytes;  // dalloc: capacity of the buffer behind each pointer member
   float *hpos = nullptr, *hvel = nullptr, *hrho = nullptr;  // staging of sph_set_particles_host
   int32_t* htagd = nullptr;
+  float* hout = nullptr;   // staging of sph_get_fields_host
+  int* hidx = nullptr;     // caller indices of one class during sph_set_particles
   // one step captured as a CUDA graph (launch-bound small configurations); rebuilt after sph_set_particles
   cudaGraphExec_t gexec = nullptr;
   cudaStream_t cap_stream = nullptr;
@@ -149,7 +151,7 @@ void free_all(sph_ctx* c) {
   void* ptrs[] = {c->R0, c->R1, c->TX, c->A, c->TB, c->ACC, c->SIG, c->DRHO, c->NL, c->NC, c->NLW, c->NCW, c->NLF, c->NCF, c->ID0, c->ID1,
                   c->keyA, c->valA, c->keyB, c->valB, c->hist, c->rowsum, c->lbF, c->lbW, c->WR,
                   c->WA, c->WN, c->WG, c->WK, c->WID, c->wnear, c->S, c->dt_seq, c->stat,
-                  c->hpos, c->hvel, c->hrho, c->htagd};
+                  c->hpos, c->hvel, c->hrho, c->htagd, c->hout, c->hidx};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   for (auto e : c->ev) cudaEventDestroy(e);
@@ -505,15 +507,15 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
     float g0[3] = {(float)c->prm.g[0], (float)c->prm.g[1], (float)c->prm.g[2]};
     CK(cudaMemcpyAsync((char*)c->S + offsetof(SS, g), g0, sizeof(g0), cudaMemcpyHostToDevice, st));
   }
-  int* idx = nullptr;
-  CK(cudaMalloc((void**)&idx, sizeof(int) * std::max<size_t>(cap, 1)));
+  if (dalloc(c, &c->hidx, std::max<size_t>(cap, 1))) return SPH_ECUDA;  // kept across calls
+  int* idx = c->hidx;
   // ---- wall structure, built once ----
   if (nw > 0) {
     CK(cudaMemcpyAsync(idx, wid.data(), sizeof(int) * nw, cudaMemcpyHostToDevice, st));
     LAUNCH(k_load, cdiv(nw, 256), 256, st, c->dp, nw, 1, idx, pos, vel, rho, tag, c->TX, c->TB, c->ID0, c->keyA, c->valA);
     unsigned *ks, *vs;
     rc = radix_sort(c, st, nw, c->keyA, c->valA, c->keyB, c->valB, &ks, &vs);
-    if (rc) { cudaFree(idx); return rc; }
+    if (rc) return rc;
     LAUNCH(k_reorder, cdiv(nw, 256), 256, st, c->dp, nw, vs, c->TX, c->TB, c->ID0, c->WR, c->WA, c->WID,
            (const unsigned*)nullptr, -1, (int*)nullptr);
     CK(cudaMemcpyAsync(c->WK, ks, sizeof(unsigned) * nw, cudaMemcpyDeviceToDevice, st));
@@ -535,7 +537,6 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
   pf.on = false;
   rc = pipeline_after_hash(c, st, 1, pf);
   cudaError_t e = cudaStreamSynchronize(st);
-  cudaFree(idx);
   if (rc) return rc;
   if (e != cudaSuccess) { c->err = cudaGetErrorString(e); return SPH_ECUDA; }
   c->loaded = true;
@@ -592,8 +593,8 @@ int sph_get_fields_host(sph_ctx* c, float* pos, float* vel, float* rho, float* p
   if (!c->loaded) { c->err = "no particles"; return SPH_EINVAL; }
   cudaStream_t st = (cudaStream_t)stream;
   const size_t n = (size_t)std::max<int64_t>(c->n, 1);
-  float* buf = nullptr;
-  CK(cudaMalloc((void**)&buf, n * 11 * sizeof(float)));
+  if (dalloc(c, &c->hout, n * 11)) return SPH_ECUDA;  // kept across calls
+  float* buf = c->hout;
   float *dpos = buf, *dvel = buf + 3 * n, *dacc = buf + 6 * n, *drho = buf + 9 * n, *dp = buf + 10 * n;
   int rc = sph_get_fields(c, pos ? dpos : nullptr, vel ? dvel : nullptr, rho ? drho : nullptr,
                           p ? dp : nullptr, acc ? dacc : nullptr, stream);
@@ -606,7 +607,6 @@ int sph_get_fields_host(sph_ctx* c, float* pos, float* vel, float* rho, float* p
     if (p && e == cudaSuccess) e = cudaMemcpyAsync(p, dp, c->n * 4, cudaMemcpyDeviceToHost, st);
   }
   cudaError_t e2 = cudaStreamSynchronize(st);
-  cudaFree(buf);
   if (rc) return rc;
   if (e != cudaSuccess || e2 != cudaSuccess) {
     c->err = cudaGetErrorString(e != cudaSuccess ? e : e2);

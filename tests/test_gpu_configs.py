@@ -30,6 +30,26 @@ def _steps_and_compare(cfg, nsteps, names=("rho", "p", "acc", "vel", "pos")):
     assert sg["escaped"] == 0 and sg["nonfinite"] == 0
     assert abs(sg["mass"] - so["mass"]) <= 1e-10 * so["mass"]   # the oracle adds 671 000 doubles one by one
     assert abs(sg["ek"] - so["ek"]) <= 1e-3 * so["ek"] + 1e-12
+    # the lists the passes read hold every float32-contract neighbour (k_build's float16 filter)
+    missing, extra, total = g.debug_list_check()
+    assert missing == 0 and extra <= 0.06 * total
+    # probes (readings A29 / A30) on the oracle's own state, sampled points
+    from oracle import probes
+    fo = o.fields()
+    fl = cfg["tag"] >= 0
+    lo, hi = fo["pos"][fl].min(0), fo["pos"][fl].max(0)
+    pts = (lo + np.random.default_rng(23).random((16, 3)) * (hi - lo)).astype(np.float32)
+    if cfg["dim"] == 2:
+        pts[:, 2] = 0.0
+    p_ref, _ = probes.pressure_probes(cfg, fo["pos"], fo["p"], cfg["tag"], pts.astype(np.float64))
+    p_gpu, _ = g.probe_pressure(pts)
+    S = cfg["rho0"][0] * float(np.linalg.norm(cfg["g"]) or 1.0) * float(cfg.get("H", 1.0))
+    assert np.max(np.abs(p_gpu - p_ref)) / S < TOL
+    e_ref = probes.wave_gauges(cfg, fo["pos"], cfg["tag"], pts.astype(np.float64))
+    e_gpu = g.probe_gauge(pts)
+    ok = ~np.isnan(e_ref)
+    assert np.array_equal(ok, ~np.isnan(e_gpu))
+    assert ok.sum() == 0 or np.max(np.abs(e_gpu[ok] - e_ref[ok])) < 1e-5 * float(cfg.get("H", 1.0))
     return o, g
 
 
