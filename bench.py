@@ -43,20 +43,20 @@ UNIT = "fluid particle-steps/s"
 FLOPS_HIT = {"pass_a": 40.0, "pass_b": 50.0, "wall": 30.0}
 CAND_FLOPS = 8.0
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from `ncu --set full` captures of these
-# exact workloads (profiles/r01d_README.md); other workloads report traffic = null.
+# exact workloads (profiles/r01e_README.md); other workloads report traffic = null.
 NCU_TRAFFIC_BYTES = {
-    ("cfg1_dam_break_3d_box", "k_pass_a"): 258.72e6 + 19.75e6,
-    ("cfg1_dam_break_3d_box", "k_pass_b"): 260.52e6 + 19.17e6,
-    ("cfg1_dam_break_3d_box", "k_build"): 86.55e6 + 235.02e6,
-    ("cfg4_box_160", "k_pass_a"): 1579.9e6 + 158.0e6,
-    ("cfg4_box_160", "k_pass_b"): 1588.0e6 + 143.2e6,
-    ("cfg4_box_160", "k_build"): 571.7e6 + 1768.3e6,
+    ("cfg1_dam_break_3d_box", "k_pass_a"): 258.86e6 + 19.56e6,
+    ("cfg1_dam_break_3d_box", "k_pass_b"): 260.51e6 + 18.69e6,
+    ("cfg1_dam_break_3d_box", "k_build"): 90.55e6 + 240.98e6,
+    ("cfg4_box_160", "k_pass_a"): 1579.8e6 + 157.9e6,
+    ("cfg4_box_160", "k_pass_b"): 1588.0e6 + 142.6e6,
+    ("cfg4_box_160", "k_build"): 595.6e6 + 1790.4e6,
 }
 # l1tex__data_pipe_lsu_wavefronts (fraction of peak) and sm__issue_active of the same captures: the pair
 # passes are bound by the tag stage of L1 (record gathers), not by FP32 issue.
 NCU_L1_ISSUE = {
     ("cfg1_dam_break_3d_box", "k_pass_a"): (0.760, 0.547),
-    ("cfg1_dam_break_3d_box", "k_pass_b"): (0.748, 0.559),
+    ("cfg1_dam_break_3d_box", "k_pass_b"): (0.753, 0.562),
     ("cfg4_box_160", "k_pass_a"): (0.859, 0.606),
     ("cfg4_box_160", "k_pass_b"): (0.887, 0.650),
 }
