@@ -337,21 +337,26 @@ def run_gpu(args):
     KE = K
     g2.set_particles(pin["pos"].numpy(), pin["vel"].numpy(), pin["rho"].numpy(), pin["tag"].numpy())
     g2.step(1)  # warm the allocator / module load outside the timed region
-    barrier()
-    t0 = time.perf_counter()
-    g2.set_particles(pin["pos"].numpy(), pin["vel"].numpy(), pin["rho"].numpy(), pin["tag"].numpy())
-    for _ in range(KE):
-        g2.step(1)
-        s2 = g2.get_stats(with_pairs=False)   # device -> host read of the step's result (t, dt, E_k, mass, x_front)
-    g2.get_fields_into_host(pos=out["pos"].numpy(), vel=out["vel"].numpy(), rho=out["rho"].numpy())
-    torch.cuda.synchronize()
-    e2e_s = time.perf_counter() - t0
+    # host-side wall clock: the region is repeated and the median repetition kept (the box's host
+    # cores are shared; every repetition does the full region: upload + set-up, KE steps, read-back)
+    reps = []
+    for _rep in range(3):
+        barrier()
+        t0 = time.perf_counter()
+        g2.set_particles(pin["pos"].numpy(), pin["vel"].numpy(), pin["rho"].numpy(), pin["tag"].numpy())
+        for _ in range(KE):
+            g2.step(1)
+            s2 = g2.get_stats(with_pairs=False)   # device -> host read of the step's result (t, dt, E_k, mass, x_front)
+        g2.get_fields_into_host(pos=out["pos"].numpy(), vel=out["vel"].numpy(), rho=out["rho"].numpy())
+        torch.cuda.synchronize()
+        reps.append(time.perf_counter() - t0)
+    e2e_s = sorted(reps)[1]
     e2e_s = max_over_ranks(e2e_s, "cuda")
     h2d = (n * (12 + 12 + 4 + 4)) / KE
     d2h = (n * 4 + n * (12 + 12 + 4)) / KE + 88      # tag read-back + fields, + sph_stats per step
     e2e = {"value": world * nfl * KE / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d,
            "d2h_bytes_per_step": d2h,
-           "region": "sph_set_particles_host + %d x (sph_step(1) + sph_get_stats_ex(no pair count)) + sph_get_fields_host" % KE}
+           "region": "sph_set_particles_host + %d x (sph_step(1) + sph_get_stats_ex(no pair count)) + sph_get_fields_host; median of 3 repetitions" % KE}
     g2.close()
 
     # ---- CPU oracle on the host cores (rank 0, N = 1 only) -----------------------------------------
