@@ -164,18 +164,18 @@ int radix_sort(sph_ctx* c, cudaStream_t st, int n, unsigned* kA, unsigned* vA, u
                unsigned** ko, unsigned** vo) {
   unsigned *ki = kA, *vi = vA, *kt = kB, *vt = vB;
   if (n > 0) {
-    int nblk = cdiv(n, RS_TILE);
+    const int items = rs_items((size_t)n), nblk = cdiv(n, RS_THREADS * items);
     for (int pass = 0; pass < c->sort_passes; ++pass) {
       int shift = c->sort_bits * pass;
-      if (c->sort_bits == 9) {
-        LAUNCH(k_radix_hist<512>, nblk, RS_THREADS, st, ki, n, shift, c->hist, nblk, c->rowsum);
-        LAUNCH(k_scan_apply, 512, 256, st, c->hist, nblk, c->rowsum);
-        LAUNCH(k_radix_scatter<512>, nblk, RS_THREADS, st, ki, vi, n, shift, c->hist, nblk, kt, vt, c->rowsum);
-      } else {
-        LAUNCH(k_radix_hist<256>, nblk, RS_THREADS, st, ki, n, shift, c->hist, nblk, c->rowsum);
-        LAUNCH(k_scan_apply, 256, 256, st, c->hist, nblk, c->rowsum);
-        LAUNCH(k_radix_scatter<256>, nblk, RS_THREADS, st, ki, vi, n, shift, c->hist, nblk, kt, vt, c->rowsum);
-      }
+#define RS_PASS(ND, IT)                                                                                   \
+  do {                                                                                                    \
+    LAUNCH((k_radix_hist<ND, IT>), nblk, RS_THREADS, st, ki, n, shift, c->hist, nblk, c->rowsum);         \
+    LAUNCH(k_scan_apply, ND, 256, st, c->hist, nblk, c->rowsum);                                          \
+    LAUNCH((k_radix_scatter<ND, IT>), nblk, RS_THREADS, st, ki, vi, n, shift, c->hist, nblk, kt, vt, c->rowsum); \
+  } while (0)
+      if (c->sort_bits == 9) { if (items == 4) RS_PASS(512, 4); else RS_PASS(512, 16); }
+      else { if (items == 4) RS_PASS(256, 4); else RS_PASS(256, 16); }
+#undef RS_PASS
       std::swap(ki, kt);
       std::swap(vi, vt);
     }
@@ -488,7 +488,8 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
   rc |= dalloc(c, &c->ID0, cap); rc |= dalloc(c, &c->ID1, cap);
   rc |= dalloc(c, &c->keyA, cap); rc |= dalloc(c, &c->valA, cap); rc |= dalloc(c, &c->keyB, cap);
   rc |= dalloc(c, &c->valB, cap);
-  rc |= dalloc(c, &c->hist, (size_t)512 * cdiv(std::max<size_t>(cap, 1), RS_TILE));
+  rc |= dalloc(c, &c->hist, (size_t)512 * std::max(cdiv(std::max(nf, 1), RS_THREADS * rs_items((size_t)nf)),
+                                                  cdiv(std::max(nw, 1), RS_THREADS * rs_items((size_t)nw))));
   rc |= dalloc(c, &c->rowsum, 512);
   if (!rc) CK(cudaMemsetAsync(c->rowsum, 0, 512 * sizeof(unsigned), (cudaStream_t)stream));  // radix digit totals: zero between passes
   rc |= dalloc(c, &c->lbF, c->ncell + 1); rc |= dalloc(c, &c->lbW, c->ncell + 1);

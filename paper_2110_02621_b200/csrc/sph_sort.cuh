@@ -9,9 +9,12 @@
 // Per pass: tile histograms (+ per-digit totals by atomics) -> scan -> stable scatter with warp match
 // ranking: 3 dependent launches.
 // ------------------------------------------------------------------------------------------
-constexpr int RS_THREADS = 256, RS_ITEMS = 16, RS_TILE = RS_THREADS * RS_ITEMS, RS_WARPS = 8;
+// Keys per thread: 16 (tile of 4096) for large inputs; 4 (tile of 1024) below RS_SMALL_N keys, where
+// 4096-key tiles leave most SMs idle and every block runs a serial chain of 16 match rounds.
+constexpr int RS_THREADS = 256, RS_WARPS = 8, RS_SMALL_N = 2 << 20;
+inline int rs_items(size_t n) { return n < (size_t)RS_SMALL_N ? 4 : 16; }
 
-template <int ND>
+template <int ND, int RS_ITEMS>
 __global__ void __launch_bounds__(RS_THREADS)
 k_radix_hist(const unsigned* __restrict__ keys, int n, int shift, unsigned* __restrict__ hist,
              int nblk, unsigned* __restrict__ rowsum) {
@@ -19,6 +22,7 @@ k_radix_hist(const unsigned* __restrict__ keys, int n, int shift, unsigned* __re
   for (int d = threadIdx.x; d < ND; d += RS_THREADS) h[d] = 0;
   __syncthreads();
   const int lane = threadIdx.x & 31;
+  constexpr int RS_TILE = RS_THREADS * RS_ITEMS;
   const int base = blockIdx.x * RS_TILE;
 #pragma unroll 4
   for (int it = 0; it < RS_ITEMS; ++it) {
@@ -76,7 +80,7 @@ k_scan_apply(unsigned* __restrict__ hist, int nblk, const unsigned* __restrict__
   }
 }
 
-template <int ND>
+template <int ND, int RS_ITEMS>
 __global__ void __launch_bounds__(RS_THREADS)
 k_radix_scatter(const unsigned* __restrict__ keys, const unsigned* __restrict__ vals, int n, int shift,
                 const unsigned* __restrict__ hist, int nblk, unsigned* __restrict__ keys_out,
@@ -87,6 +91,7 @@ k_radix_scatter(const unsigned* __restrict__ keys, const unsigned* __restrict__ 
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   for (int i = threadIdx.x; i < RS_WARPS * ND; i += RS_THREADS) (&wc[0][0])[i] = 0;
   __syncthreads();
+  constexpr int RS_TILE = RS_THREADS * RS_ITEMS;
   const int base = blockIdx.x * RS_TILE + wid * (RS_ITEMS * 32);
   unsigned k[RS_ITEMS], rank[RS_ITEMS];
   const unsigned lt = (1u << lane) - 1u;
