@@ -455,3 +455,36 @@ def test_probes_match_oracle(name, steps):
     assert ok.sum() >= 10
     assert np.max(np.abs(e_gpu[ok] - e_ref[ok])) < 1e-5 * H
     assert g.probe_pressure(np.zeros((0, 3), np.float32))[0].shape == (0,)
+
+
+def test_two_phase_hydrostatic_tank_profile_and_energy():
+    """The paper's two-phase hydrostatic tank (case X1) at a size the oracle runs in
+    seconds: water below air (density ratio 1000) at rest.  Long-run comparison on integral
+    quantities: kinetic energy within 1 % of the oracle's (same dt sequence), mass exact, and the
+    probed pressure profile (reading A29) within 6 % (L2) of rho0_w g H of the analytic
+    p(z) = rho_a g (top - z) + (rho_w - rho_a) g max(H - z, 0) the paper compares against in its Fig. 4
+    (its first-order L2 error at this resolution is of that size)."""
+    from oracle import probes
+    dp, H = 0.02, 0.5
+    cfg = inputs.two_phase_2d(dp=dp, tank=(1.0, 1.0), column=(1.0, H), equal_c=True)
+    o, g = make_pair(cfg)
+    nsteps = 400
+    dts = o.step(nsteps)
+    g.step(nsteps, dts=dts)
+    so, sg = o.stats(), g.get_stats()
+    assert sg["escaped"] == 0 and so["escaped"] == 0
+    assert abs(sg["mass"] - so["mass"]) <= 1e-10 * so["mass"]
+    assert abs(sg["ek"] - so["ek"]) <= 1e-2 * so["ek"] + 1e-9
+    top = 1.0
+    zs = np.linspace(0.06, 0.94, 23)
+    pts = np.stack([np.full_like(zs, 0.5), zs, np.zeros_like(zs)], 1).astype(np.float32)
+    p_gpu, _ = g.probe_pressure(pts)
+    fo = o.fields()
+    p_orc, _ = probes.pressure_probes(cfg, fo["pos"], fo["p"], cfg["tag"], pts.astype(np.float64))
+    S = 1000.0 * 9.81 * H
+    assert np.max(np.abs(p_gpu - p_orc)) / S < 1e-3            # 400 steps: integral-quantity tolerance, not 1e-4
+    ref = 1.0 * 9.81 * (top - zs) + 999.0 * 9.81 * np.maximum(H - zs, 0.0)
+    l2 = np.sqrt(np.mean((p_gpu - ref) ** 2)) / S
+    assert l2 < 0.06, l2      # measured 0.038 at dp = 0.02 after 400 steps (start-up transient included)
+    # total energy scale of the paper's case: T_tot = rho g L H^2 / 2 = 1226.25 J (PAPER.md:244); the tank stays at rest
+    assert sg["ek"] < 2e-3 * 1226.25
