@@ -64,6 +64,10 @@ struct orc_params {
   uint32_t reserved;
   double domain_min[3];
   double domain_max[3];
+  // NEXT-1: rigid wall motion x_w(t) = x_w(t_start) + A [sin(2 pi f t) - sin(2 pi f t_start)]
+  double wall_osc_amp[3];
+  double wall_osc_freq;
+  double t_start;       // time at orc_set_particles (0 in every BASELINE.json configuration)
 };
 
 const double PI = 3.14159265358979323846264338327950288;
@@ -168,6 +172,7 @@ struct Ctx {
   double V0 = 0, sigma0 = 0, t = 0, dt_last = 0;
   int64_t steps = 0, npairs = 0, escaped = 0;
   std::vector<double> r, v, a;          // n*3
+  std::vector<double> r0;               // positions at orc_set_particles (wall entries used by the wall motion)
   std::vector<double> rho, p, m, sigma, drho;
   std::vector<int32_t> tag;
   std::vector<double> pw;               // wall pressure (only wall entries used)
@@ -186,6 +191,23 @@ void gravity_at(const Ctx& S, double t, double g[3]) {
   if (S.P.g_osc_period > 0.0) {
     double s = std::sin(2.0 * PI * t / S.P.g_osc_period);
     for (int k = 0; k < 3; ++k) g[k] += S.P.g_osc_amp[k] * s;
+  }
+}
+
+// NEXT-1.  Prescribed rigid wall kinematics, "x = A0 sin(2 pi f0 t)": displacement since
+// orc_set_particles, wall velocity and wall acceleration a_w (the a_w of Eq. 2.12).
+inline bool walls_move(const Ctx& S) {
+  return S.P.wall_osc_freq > 0.0 &&
+         (S.P.wall_osc_amp[0] != 0.0 || S.P.wall_osc_amp[1] != 0.0 || S.P.wall_osc_amp[2] != 0.0);
+}
+void wall_motion(const Ctx& S, double t, double s[3], double vwall[3], double aw[3]) {
+  for (int k = 0; k < 3; ++k) s[k] = vwall[k] = aw[k] = 0.0;
+  if (!walls_move(S)) return;
+  const double w = 2.0 * PI * S.P.wall_osc_freq;
+  for (int k = 0; k < S.P.dim; ++k) {
+    s[k] = S.P.wall_osc_amp[k] * (std::sin(w * t) - std::sin(w * S.P.t_start));
+    vwall[k] = S.P.wall_osc_amp[k] * w * std::cos(w * t);
+    aw[k] = -S.P.wall_osc_amp[k] * w * w * std::sin(w * t);
   }
 }
 
@@ -353,9 +375,12 @@ double time_step(const Ctx& S) {
   return dt;
 }
 
-// O-4.  PAPER.md:111-116, Eq. 2.12 (readings A4-A7).  a_w = 0, v_wall = 0
-// (static walls in every configuration).
-void wall_extrapolate(Ctx& S, const double g[3], bool with_velocity) {
+// O-4.  PAPER.md:111-116, Eq. 2.12 (readings A4-A7) at time t: the lever term carries g - a_w(t), the
+// mirror 2 v_wall(t) - <v_f> (a_w = 0, v_wall = 0 for the static walls of every BASELINE.json configuration).
+void wall_extrapolate(Ctx& S, const double g_in[3], bool with_velocity, double t) {
+  double sdis[3], vwall[3], aw[3];
+  wall_motion(S, t, sdis, vwall, aw);
+  const double g[3] = {g_in[0] - aw[0], g_in[1] - aw[1], g_in[2] - aw[2]};
   const int dim = S.P.dim;
   const double h = S.P.h;
   const bool multi = S.P.n_phases > 1;
@@ -386,7 +411,7 @@ void wall_extrapolate(Ctx& S, const double g[3], bool with_velocity) {
     if (sW == 0.0) {
       S.pw[w] = 0.0;
       if (with_velocity)
-        for (int k = 0; k < 3; ++k) S.vw[3 * w + k] = 0.0;
+        for (int k = 0; k < 3; ++k) S.vw[3 * w + k] = vwall[k];   // reading A7
       continue;
     }
     double lever = g[0] * sr[0] + g[1] * sr[1] + g[2] * sr[2];  // (g - a_w) . sum
@@ -394,7 +419,7 @@ void wall_extrapolate(Ctx& S, const double g[3], bool with_velocity) {
     if (with_velocity)
       for (int k = 0; k < 3; ++k)
         S.vw[3 * w + k] =
-            (S.P.flags & ORC_FLAG_WALL_VEL_MIRROR) ? 2.0 * 0.0 - sv[k] / sW : 0.0;
+            (S.P.flags & ORC_FLAG_WALL_VEL_MIRROR) ? 2.0 * vwall[k] - sv[k] / sW : vwall[k];
   }
 }
 
@@ -549,13 +574,20 @@ void step_once(Ctx& S, double dt) {
       S.r[3 * i + k] += dt * S.v[3 * i + k];
     }
   }
+  if (walls_move(S)) {                               // NEXT-1: walls at t^{n+1}
+    double sdis[3], vwall[3], aw[3];
+    wall_motion(S, S.t + dt, sdis, vwall, aw);
+    for (int64_t i = 0; i < S.n; ++i)
+      if (is_wall(S, i))
+        for (int k = 0; k < S.P.dim; ++k) S.r[3 * i + k] = S.r0[3 * i + k] + sdis[k];
+  }
   build_neighbours(S);
   double g[3];
   gravity_at(S, S.t + dt, g);                        // reading A28
-  wall_extrapolate(S, g, true);                      // O-4
+  wall_extrapolate(S, g, true, S.t + dt);            // O-4
   pass_continuity(S);                                // O-5
   density_update(S, dt);                             // O-6
-  wall_extrapolate(S, g, false);                     // O-7 (wall pressure only)
+  wall_extrapolate(S, g, false, S.t + dt);           // O-7 (wall pressure only)
   pass_momentum(S, g);                               // O-7
   for (int64_t i = 0; i < S.n; ++i) {                // O-8, Eq. 2.22
     if (is_wall(S, i)) continue;
@@ -666,13 +698,14 @@ int orc_set_particles(void* hd, int64_t n, const float* pos, const float* vel, c
       S.p[i] = S.P.c0[ph] * S.P.c0[ph] * (S.rho[i] - S.P.rho0[ph]);   // Eq. 2.3
     }
   }
-  S.t = 0; S.steps = 0; S.dt_last = 0;
+  S.r0 = S.r;
+  S.t = S.P.t_start; S.steps = 0; S.dt_last = 0;
   build_neighbours(S);
   wall_normals(S);
   number_density(S);
   double g[3];
-  gravity_at(S, 0.0, g);
-  wall_extrapolate(S, g, true);
+  gravity_at(S, S.t, g);
+  wall_extrapolate(S, g, true, S.t);
   pass_momentum(S, g);   // (dv/dt)^0, reading A18
   return 0;
 }

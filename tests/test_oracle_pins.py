@@ -531,3 +531,78 @@ def test_P20_wave_gauge_of_a_resting_block(dim):
     tag2 = tag.copy(); tag2[pos[:, up] > 0.5 * n * dp] = 1            # upper half is the light phase
     eta = probes.wave_gauges(cfg, pos, tag2, pts)
     assert eta[0] == pytest.approx(0.5 * n * dp, rel=1e-14)
+
+
+# ------------------------------------------------------------------------- NEXT-1: moving walls (oracle side)
+def test_P21_wall_kinematics_and_accelerating_frame_wall_pressure():
+    """PAPER.md:116 (a_w in Eq. 2.12), :252 (x = A0 sin(2 pi f0 t)).
+    (i) Kinematics: after steps of given dt the wall particles sit at x(t_start) + A [sin(w t) - sin(w t_start)],
+    fluid-independent (closed form).
+    (ii) Eq. 2.12 with a_w: a tank accelerating upwards with a_w = gmag in zero gravity holds the same
+    hydrostatic field as the tank at rest under gravity -gmag, so the wall pressures must equal pin P4's
+    closed form rho0 gmag (H - y_w): t_start = 3T/4 gives a_w = +A w^2, v_wall = 0."""
+    dp, nx, K, c = 1.0 / 64, 12, 10, 10.0
+    fl = lattice(2, nx, dp)
+    fl = fl[fl[:, 1] < K * dp]
+    k = np.round(fl[:, 1] / dp - 0.5)
+    rho_f = 1000.0 + (K - k) * 2.0 ** -10
+    gmag = c * c * 2.0 ** -10 / (dp * 1000.0)
+    H = (K + 0.5) * dp
+    wl = np.array([[(i + 0.5) * dp, -(j + 0.5) * dp] for i in range(nx) for j in range(3)])
+    pos = np.concatenate([fl, wl])
+    tag = np.concatenate([np.zeros(len(fl)), -np.ones(len(wl))])
+    rho = np.concatenate([rho_f, np.full(len(wl), 1000.0)])
+    f0 = 2.0
+    w = 2.0 * math.pi * f0
+    A = gmag / (w * w)
+    cfg = custom(2, pos, tag, rho, dp=dp, g=(0, 0, 0), c0=(c,), wall_osc_amp=(0.0, A, 0.0), wall_osc_freq=f0,
+                 t_start=0.75 / f0)
+    o = run(cfg)
+    pw = o.fields()["p"][len(fl):]
+    expect = 1000.0 * gmag * (H - wl[:, 1])
+    near = wl[:, 1] > -2.4 * dp
+    assert np.max(np.abs(pw - expect)[near]) < 3e-5 * expect.max()
+    # without the a_w term the lever vanishes (g = 0) and the miss is of the size of the term itself
+    o_static = run(custom(2, pos, tag, rho, dp=dp, g=(0, 0, 0), c0=(c,)))
+    pw0 = o_static.fields()["p"][len(fl):]
+    assert np.max(np.abs(pw0 - expect)[near]) > 100 * 3e-5 * expect.max()
+    # (i) kinematics over three steps of unequal dt
+    dts = np.array([1.0e-4, 2.5e-4, 0.7e-4])
+    x0 = o.fields()["pos"][len(fl):].copy()
+    o.step(3, dts=dts)
+    t0, t1 = 0.75 / f0, 0.75 / f0 + dts.sum()
+    x1 = o.fields()["pos"][len(fl):]
+    assert np.allclose(x1[:, 1] - x0[:, 1], A * (math.sin(w * t1) - math.sin(w * t0)), rtol=0, atol=1e-15)
+    assert np.array_equal(x1[:, 0], x0[:, 0])
+
+
+def test_P22_fluid_moving_with_the_walls_feels_no_wall_motion():
+    """Mirror velocity with a moving wall (reading A6, v_w = 2 v_wall - <v_f>) and Galilean invariance:
+    at t = 0 the wall velocity is A w e_x and a_w = 0; a fluid moving uniformly with that velocity must
+    get the density rates (Eq. 2.9, the only place the wall velocity enters: Eq. 2.11 has no velocity
+    term, reading A20) and the accelerations of the same fluid at rest between walls at rest."""
+    cfg0 = inputs.dam_break_2d(dp=0.05, tank=(1.0, 0.8), column=(1.0, 0.4))
+    dt = np.array([1.0e-9])
+
+    def rates(cfg):
+        o = run(cfg)
+        o.step(1, dts=dt)
+        f = o.fields()
+        return f["drho"], f["acc"]
+
+    d0, a0 = rates(cfg0)
+    f0, A = 1.5, 0.02
+    u = A * 2.0 * math.pi * f0
+    vel = cfg0["vel"].copy()
+    vel[cfg0["tag"] >= 0, 0] = np.float32(u)
+    cfg1 = dict(cfg0, wall_osc_amp=(A, 0.0, 0.0), wall_osc_freq=f0, vel=vel)
+    d1, a1 = rates(cfg1)
+    fl = cfg0["tag"] >= 0
+    sa = np.abs(a0[fl]).max()
+    sd = 1000.0 * u / cfg0["h"]          # size of a density rate that a relative velocity u would cause
+    # u is rounded to float32 on input, the wall moves with the float64 value: residual relative motion 1e-8 u
+    assert np.max(np.abs(a1[fl] - a0[fl])) < 1e-6 * sa
+    assert np.max(np.abs(d1[fl] - d0[fl])) < 1e-6 * sd
+    # with the walls at rest the same moving fluid is compressed against them (the pin is not vacuous)
+    d2, _ = rates(dict(cfg0, vel=vel))
+    assert np.max(np.abs(d2[fl] - d0[fl])) > 1e-2 * sd
