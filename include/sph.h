@@ -76,6 +76,10 @@ typedef struct {
                                     64 in 2-D); the fluid-wall lists hold 3/4 of it */
   double domain_min[3];          /* box of the cell grid; particles outside are binned in the edge */
   double domain_max[3];          /* cells and counted as escaped (reading A23)                      */
+  double wall_osc_amp[3];        /* NEXT-1: all walls translate rigidly, x_w(t) = x_w(0) + wall_osc_amp *   */
+  double wall_osc_freq;          /* sin(2 pi wall_osc_freq t); a_w enters Eq. 2.12,
+                                    v_wall the mirror of reading A6; 0 = static walls.  The wall cell list is
+                                    then rebuilt every step; the domain box must contain the whole excursion */
 } sph_params;
 
 typedef struct {

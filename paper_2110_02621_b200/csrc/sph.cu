@@ -72,6 +72,10 @@ struct sph_ctx {
   int64_t dt_seq_cap = 0;
   StatAcc* stat = nullptr;
   int sort_passes = 1, sort_bits = 8;
+  // NEXT-1 (moving walls): wall positions and caller ids in set-up order, sort buffers of the per-step re-sort
+  int moving = 0;
+  uint4* WX0 = nullptr;
+  unsigned *WID0 = nullptr, *WkeyA = nullptr, *WkeyB = nullptr, *WvalA = nullptr, *WvalB = nullptr;
   std::map<void*, size_t> cap_bytes;  // dalloc: capacity of the buffer behind each pointer member
   float *hpos = nullptr, *hvel = nullptr, *hrho = nullptr;  // staging of sph_set_particles_host
   int32_t* htagd = nullptr;
@@ -151,7 +155,8 @@ void free_all(sph_ctx* c) {
   void* ptrs[] = {c->R0, c->R1, c->TX, c->A, c->TB, c->ACC, c->SIG, c->DRHO, c->NL, c->NC, c->NLW, c->NCW, c->NLF, c->NCF, c->ID0, c->ID1,
                   c->keyA, c->valA, c->keyB, c->valB, c->hist, c->rowsum, c->lbF, c->lbW, c->WR,
                   c->WA, c->WN, c->WG, c->WK, c->WID, c->wnear, c->S, c->dt_seq, c->stat,
-                  c->hpos, c->hvel, c->hrho, c->htagd, c->hout, c->hidx};
+                  c->hpos, c->hvel, c->hrho, c->htagd, c->hout, c->hidx,
+                  c->WX0, c->WID0, c->WkeyA, c->WkeyB, c->WvalA, c->WvalB};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   for (auto e : c->ev) cudaEventDestroy(e);
@@ -214,6 +219,26 @@ void launch_wall(sph_ctx* c, cudaStream_t st, bool with_vel, const XB* R) {
   }
 }
 
+// NEXT-1 (moving walls): the walls at their positions of t^{n+1}, re-sorted into the cell grid (the
+// same kernels as the set-up; TX / TB are free between the fluid reorder and pass B).
+int wall_rebuild(sph_ctx* c, cudaStream_t st) {
+  const int nw = (int)c->nw;
+  if (nw == 0) return SPH_OK;
+  LAUNCH(k_wall_shift, cdiv(nw, 256), 256, st, c->dp, c->S, nw, c->WX0, c->TX, c->TB, c->WkeyA, c->WvalA);
+  unsigned *ks, *vs;
+  int rc = radix_sort(c, st, nw, c->WkeyA, c->WvalA, c->WkeyB, c->WvalB, &ks, &vs);
+  if (rc) return rc;
+  LAUNCH(k_reorder, cdiv(nw, 256), 256, st, c->dp, nw, vs, c->TX, c->TB, c->WID0, c->WR, c->WA, c->WID,
+         (const unsigned*)nullptr, -1, (int*)nullptr);
+  CK(cudaMemcpyAsync(c->WK, ks, sizeof(unsigned) * nw, cudaMemcpyDeviceToDevice, st));
+  LAUNCH(k_image, cdiv(nw, 256), 256, st, c->dp, nw, c->WR, c->WG);
+  LAUNCH(k_cell_bounds, cdiv(c->ncell + 1, 256), 256, st, ks, nw, (int)c->ncell, c->lbW);
+  if (c->prm.dim == 3) LAUNCH(k_normals<3>, cdiv(nw, 128), 128, st, c->dp, nw, c->WR, c->WK, c->lbW, c->WN);
+  else LAUNCH(k_normals<2>, cdiv(nw, 128), 128, st, c->dp, nw, c->WR, c->WK, c->lbW, c->WN);
+  LAUNCH(k_wnear, cdiv(c->ncell, 256), 256, st, c->dp, (int)c->ncell, c->lbW, c->wnear);
+  return SPH_OK;
+}
+
 // Everything after the drift: sort, reorder, cell ranges, wall pass, pass A, wall pass, pass B.
 int pipeline_after_hash(sph_ctx* c, cudaStream_t st, int init, Prof& pf) {
   const int nf = (int)c->nf;
@@ -229,6 +254,10 @@ int pipeline_after_hash(sph_ctx* c, cudaStream_t st, int init, Prof& pf) {
            c->R0, c->A, c->IDnext, ks, (int)c->ncell, c->lbF);
   } else {
     LAUNCH(k_cell_bounds, cdiv(c->ncell + 1, 256), 256, st, ks, nf, (int)c->ncell, c->lbF);
+  }
+  if (c->moving && !init) {
+    rc = wall_rebuild(c, st);
+    if (rc) return rc;
   }
   pf.mark();  // end reorder
   launch_wall(c, st, true, c->R0);
@@ -429,6 +458,10 @@ int sph_create(const sph_params* prm, sph_ctx** out) {
     d.dmin[k] = (float)prm->domain_min[k]; d.dmax[k] = (float)prm->domain_max[k];
     d.g[k] = prm->g[k]; d.gamp[k] = prm->g_osc_amp[k];
   }
+  for (int k = 0; k < 3; ++k) d.wamp[k] = k < prm->dim ? prm->wall_osc_amp[k] : 0.0;
+  d.womega = 6.283185307179586476925286766559 * prm->wall_osc_freq;
+  c->moving = prm->wall_osc_freq > 0.0 && (d.wamp[0] != 0.0 || d.wamp[1] != 0.0 || d.wamp[2] != 0.0);
+  if (!c->moving) { d.womega = 0.0; d.wamp[0] = d.wamp[1] = d.wamp[2] = 0.0; }
   d.gperiod = prm->g_osc_period; d.cmax = cmax; d.cfl = prm->cfl; d.hD = h; d.dpD = dp;
   c->ncell = (int64_t)nc[0] * nc[1] * nc[2];
   if (c->ncell >= (1ll << 31) - 2) { delete c; return SPH_EINVAL; }
@@ -507,6 +540,12 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
   {  // gravity at t = 0 (sin(0) = 0)
     float g0[3] = {(float)c->prm.g[0], (float)c->prm.g[1], (float)c->prm.g[2]};
     CK(cudaMemcpyAsync((char*)c->S + offsetof(SS, g), g0, sizeof(g0), cudaMemcpyHostToDevice, st));
+    // walls at t = 0: no displacement, a_w = 0, v_wall = A omega
+    CK(cudaMemcpyAsync((char*)c->S + offsetof(SS, gw), g0, sizeof(g0), cudaMemcpyHostToDevice, st));
+    float v0[3] = {(float)(c->dp.wamp[0] * c->dp.womega), (float)(c->dp.wamp[1] * c->dp.womega), (float)(c->dp.wamp[2] * c->dp.womega)};
+    CK(cudaMemcpyAsync((char*)c->S + offsetof(SS, vwall), v0, sizeof(v0), cudaMemcpyHostToDevice, st));
+    CK(cudaMemsetAsync((char*)c->S + offsetof(SS, sq), 0, 3 * sizeof(int), st));
+    CK(cudaStreamSynchronize(st));  // g0 / v0 are stack variables
   }
   if (dalloc(c, &c->hidx, std::max<size_t>(cap, 1))) return SPH_ECUDA;  // kept across calls
   int* idx = c->hidx;
@@ -514,6 +553,13 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
   if (nw > 0) {
     CK(cudaMemcpyAsync(idx, wid.data(), sizeof(int) * nw, cudaMemcpyHostToDevice, st));
     LAUNCH(k_load, cdiv(nw, 256), 256, st, c->dp, nw, 1, idx, pos, vel, rho, tag, c->TX, c->TB, c->ID0, c->keyA, c->valA);
+    if (c->moving) {  // NEXT-1: keep the set-up order for the per-step re-sort
+      rc = dalloc(c, &c->WX0, nw) | dalloc(c, &c->WID0, nw) | dalloc(c, &c->WkeyA, nw) | dalloc(c, &c->WkeyB, nw) |
+           dalloc(c, &c->WvalA, nw) | dalloc(c, &c->WvalB, nw);
+      if (rc) return rc;
+      CK(cudaMemcpyAsync(c->WX0, c->TX, sizeof(uint4) * nw, cudaMemcpyDeviceToDevice, st));
+      CK(cudaMemcpyAsync(c->WID0, c->ID0, sizeof(unsigned) * nw, cudaMemcpyDeviceToDevice, st));
+    }
     unsigned *ks, *vs;
     rc = radix_sort(c, st, nw, c->keyA, c->valA, c->keyB, c->valB, &ks, &vs);
     if (rc) return rc;

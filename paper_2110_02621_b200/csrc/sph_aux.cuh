@@ -35,6 +35,23 @@ __global__ void k_load(DP p, int n, int is_wall, const int* __restrict__ idx, co
   vals[i] = (unsigned)i;
 }
 
+// NEXT-1 (moving walls): wall particles in set-up order at their displaced positions X0 + sq, with the
+// cell hash of the new position; input of the per-step wall re-sort.
+__global__ void __launch_bounds__(256)
+k_wall_shift(DP p, const SS* __restrict__ S, int nw, const uint4* __restrict__ X0, uint4* __restrict__ TX,
+             float4* __restrict__ TB, unsigned* __restrict__ keys, unsigned* __restrict__ vals) {
+  const int i = blockIdx.x * 256 + threadIdx.x;
+  if (i >= nw) return;
+  uint4 x = X0[i];
+  x.x += (unsigned)S->sq[0]; x.y += (unsigned)S->sq[1];
+  if (p.dim == 3) x.z += (unsigned)S->sq[2];
+  TX[i] = x;
+  TB[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+  keys[i] = cell_key(p, fx_image(x.x, p.O[0], p.Q), fx_image(x.y, p.O[1], p.Q),
+                     p.dim == 3 ? fx_image(x.z, p.O[2], p.Q) : 0.0f);
+  vals[i] = (unsigned)i;
+}
+
 // Gather into cell-sorted order and derive the centred float32 image used by the candidate filter;
 // the same launch computes the cell lower bounds (one thread per cell, independent work: one graph
 // node less per step).  lb[c] = number of sorted particles with key < c, c = 0..ncell: the three cells
@@ -105,6 +122,15 @@ k_dt(DP p, SS* __restrict__ S, int nf, const float4* __restrict__ B, const doubl
   }
   grav(S->t + dt);
   S->g[0] = (float)g[0]; S->g[1] = (float)g[1]; S->g[2] = (float)g[2];
+  {  // NEXT-1: rigid wall motion at t^{n+1}: displacement, velocity, g - a_w
+    double sn = 0.0, cs = 1.0;
+    if (p.womega != 0.0) sincos(p.womega * (S->t + dt), &sn, &cs);  // static walls: gw = g, v_wall = 0, no displacement
+    for (int k = 0; k < 3; ++k) {
+      S->sq[k] = (int)rint(p.wamp[k] * sn / p.Q);
+      S->vwall[k] = (float)(p.wamp[k] * p.womega * cs);
+      S->gw[k] = (float)(g[k] + p.wamp[k] * p.womega * p.womega * sn);
+    }
+  }
   S->dt_d = dt;
   S->dt = (float)dt;
   S->t += dt;

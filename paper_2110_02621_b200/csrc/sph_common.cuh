@@ -39,6 +39,7 @@ struct DP {
   double massD[SPH_MAX_PHASES];
   double a_over_s0;
   double g[3], gamp[3], gperiod;
+  double wamp[3], womega;  // NEXT-1: wall motion x_w(t) = x_w(0) + wamp sin(womega t); womega = 0: static walls
 };
 
 // Per-particle record gathered by the pair bodies: one 32-byte sector, one 256-bit load.
@@ -61,6 +62,9 @@ struct SS {
   double dt_d;
   float dt;
   float g[3];            // gravity at t^{n+1} (reading A28)
+  float gw[3];           // g - a_w at t^{n+1}: the lever term of Eq. 2.12; = g for static walls
+  float vwall[3];        // wall velocity at t^{n+1} (mirror of reading A6)
+  int sq[3];             // wall displacement since sph_set_particles, in units of Q
   unsigned vmax2_bits;   // max |v|^2 over fluid, float bits (non-negative -> ordered as uint)
   unsigned blocks_done;
   long long steps;

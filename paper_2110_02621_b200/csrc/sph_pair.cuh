@@ -536,13 +536,13 @@ k_wall(const DP p, SS* __restrict__ S, const int nw, const float4* __restrict__ 
     walk_l<!WITH_VEL>(col, cnt, body);
   }
   if (!act) return;
-  float pwall = 0.f, vx = 0.f, vy = 0.f, vz = 0.f;
+  float pwall = 0.f, vx = S->vwall[0], vy = S->vwall[1], vz = S->vwall[2];  // reading A7: v_w = v_wall
   if (sW > 0.f) {
-    const float lever = p.Qf * (S->g[0] * srx + S->g[1] * sry + S->g[2] * srz);
+    const float lever = p.Qf * (S->gw[0] * srx + S->gw[1] * sry + S->gw[2] * srz);  // (g - a_w) . sum
     pwall = (sp + lever) / (MULTI ? sWr : sW);
     if (WITH_VEL && (p.flags & SPH_FLAG_WALL_VEL_MIRROR)) {
-      const float is = 1.0f / sW;
-      vx = -svx * is; vy = -svy * is; vz = -svz * is;
+      const float is = 1.0f / sW;  // reading A6: v_w = 2 v_wall - <v_f>
+      vx = fmaf(2.0f, vx, -svx * is); vy = fmaf(2.0f, vy, -svy * is); vz = fmaf(2.0f, vz, -svz * is);
     }
   }
   if (WITH_VEL) WR[w].b = make_float4(vx, vy, vz, pwall);

@@ -34,6 +34,7 @@ class SphParams(C.Structure):
         ("penalty_phase_mask", C.c_uint32), ("free_surface_mask", C.c_uint32),
         ("flags", C.c_uint32), ("max_neighbours", C.c_uint32),
         ("domain_min", C.c_double * 3), ("domain_max", C.c_double * 3),
+        ("wall_osc_amp", C.c_double * 3), ("wall_osc_freq", C.c_double),
     ]
 
 
@@ -103,6 +104,8 @@ def make_params(cfg: dict) -> SphParams:
         P.g_osc_amp[k] = cfg.get("g_osc_amp", (0, 0, 0))[k]
         P.domain_min[k] = cfg["domain_min"][k]
         P.domain_max[k] = cfg["domain_max"][k]
+        P.wall_osc_amp[k] = cfg.get("wall_osc_amp", (0, 0, 0))[k]
+    P.wall_osc_freq = cfg.get("wall_osc_freq", 0.0)
     P.g_osc_period = cfg.get("g_osc_period", 0.0)
     P.cfl = cfg.get("cfl", 0.25)
     P.penalty_strength = cfg.get("penalty_strength", 1.0)
