@@ -75,6 +75,7 @@ struct sph_ctx {
   // NEXT-1 (moving walls): wall positions and caller ids in set-up order, sort buffers of the per-step re-sort
   int moving = 0;
   uint4* WX0 = nullptr;
+  float4* WN0 = nullptr;   // wall normals in set-up order (translation-invariant)
   unsigned *WID0 = nullptr, *WkeyA = nullptr, *WkeyB = nullptr, *WvalA = nullptr, *WvalB = nullptr;
   std::map<void*, size_t> cap_bytes;  // dalloc: capacity of the buffer behind each pointer member
   float *hpos = nullptr, *hvel = nullptr, *hrho = nullptr;  // staging of sph_set_particles_host
@@ -156,7 +157,7 @@ void free_all(sph_ctx* c) {
                   c->keyA, c->valA, c->keyB, c->valB, c->hist, c->rowsum, c->lbF, c->lbW, c->WR,
                   c->WA, c->WN, c->WG, c->WK, c->WID, c->wnear, c->S, c->dt_seq, c->stat,
                   c->hpos, c->hvel, c->hrho, c->htagd, c->hout, c->hidx,
-                  c->WX0, c->WID0, c->WkeyA, c->WkeyB, c->WvalA, c->WvalB};
+                  c->WX0, c->WN0, c->WID0, c->WkeyA, c->WkeyB, c->WvalA, c->WvalB};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   for (auto e : c->ev) cudaEventDestroy(e);
@@ -233,8 +234,7 @@ int wall_rebuild(sph_ctx* c, cudaStream_t st) {
   CK(cudaMemcpyAsync(c->WK, ks, sizeof(unsigned) * nw, cudaMemcpyDeviceToDevice, st));
   LAUNCH(k_image, cdiv(nw, 256), 256, st, c->dp, nw, c->WR, c->WG);
   LAUNCH(k_cell_bounds, cdiv(c->ncell + 1, 256), 256, st, ks, nw, (int)c->ncell, c->lbW);
-  if (c->prm.dim == 3) LAUNCH(k_normals<3>, cdiv(nw, 128), 128, st, c->dp, nw, c->WR, c->WK, c->lbW, c->WN);
-  else LAUNCH(k_normals<2>, cdiv(nw, 128), 128, st, c->dp, nw, c->WR, c->WK, c->lbW, c->WN);
+  LAUNCH(k_gather4, cdiv(nw, 256), 256, st, nw, vs, c->WN0, c->WN);  // normals: translation-invariant
   LAUNCH(k_wnear, cdiv(c->ncell, 256), 256, st, c->dp, (int)c->ncell, c->lbW, c->wnear);
   return SPH_OK;
 }
@@ -554,7 +554,7 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
     CK(cudaMemcpyAsync(idx, wid.data(), sizeof(int) * nw, cudaMemcpyHostToDevice, st));
     LAUNCH(k_load, cdiv(nw, 256), 256, st, c->dp, nw, 1, idx, pos, vel, rho, tag, c->TX, c->TB, c->ID0, c->keyA, c->valA);
     if (c->moving) {  // NEXT-1: keep the set-up order for the per-step re-sort
-      rc = dalloc(c, &c->WX0, nw) | dalloc(c, &c->WID0, nw) | dalloc(c, &c->WkeyA, nw) | dalloc(c, &c->WkeyB, nw) |
+      rc = dalloc(c, &c->WX0, nw) | dalloc(c, &c->WN0, nw) | dalloc(c, &c->WID0, nw) | dalloc(c, &c->WkeyA, nw) | dalloc(c, &c->WkeyB, nw) |
            dalloc(c, &c->WvalA, nw) | dalloc(c, &c->WvalB, nw);
       if (rc) return rc;
       CK(cudaMemcpyAsync(c->WX0, c->TX, sizeof(uint4) * nw, cudaMemcpyDeviceToDevice, st));
@@ -570,6 +570,7 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
     LAUNCH(k_cell_bounds, cdiv(c->ncell + 1, 256), 256, st, ks, nw, (int)c->ncell, c->lbW);
     if (c->prm.dim == 3) LAUNCH(k_normals<3>, cdiv(nw, 128), 128, st, c->dp, nw, c->WR, c->WK, c->lbW, c->WN);
     else LAUNCH(k_normals<2>, cdiv(nw, 128), 128, st, c->dp, nw, c->WR, c->WK, c->lbW, c->WN);
+    if (c->moving) LAUNCH(k_unsort4, cdiv(nw, 256), 256, st, nw, vs, c->WN, c->WN0);
   } else {
     LAUNCH(k_cell_bounds, cdiv(c->ncell + 1, 256), 256, st, c->keyA, 0, (int)c->ncell, c->lbW);
   }

@@ -35,6 +35,19 @@ __global__ void k_load(DP p, int n, int is_wall, const int* __restrict__ idx, co
   vals[i] = (unsigned)i;
 }
 
+// NEXT-1: the wall normals are invariant under the rigid translation: kept in set-up order (k_unsort4 at
+// the set-up), gathered into the new cell order every step (k_gather4) instead of being recomputed.
+__global__ void __launch_bounds__(256)
+k_unsort4(int n, const unsigned* __restrict__ vals, const float4* __restrict__ in, float4* __restrict__ out) {
+  const int s = blockIdx.x * 256 + threadIdx.x;
+  if (s < n) out[vals[s]] = in[s];
+}
+__global__ void __launch_bounds__(256)
+k_gather4(int n, const unsigned* __restrict__ vals, const float4* __restrict__ in, float4* __restrict__ out) {
+  const int s = blockIdx.x * 256 + threadIdx.x;
+  if (s < n) out[s] = in[vals[s]];
+}
+
 // NEXT-1 (moving walls): wall particles in set-up order at their displaced positions X0 + sq, with the
 // cell hash of the new position; input of the per-step wall re-sort.
 __global__ void __launch_bounds__(256)
