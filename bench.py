@@ -242,6 +242,11 @@ def run_gpu(args):
         torch.cuda.synchronize()
 
     cfg = make_config(args.config)
+    if args.wall_osc:
+        # NEXT-1: rigid wall motion x_w(t) = x_w(0) + A0 sin(2 pi f0 t) along x;
+        # not the headline workload: the line's config.workload says so.
+        a0, f0 = (float(x) for x in args.wall_osc.split(","))
+        cfg["wall_osc_amp"], cfg["wall_osc_freq"] = (a0, 0.0, 0.0), f0
     nfl, nwl = cfg["n_fluid"], cfg["n_wall"]
     K, W = args.steps, max(args.warmup, 0)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")  # > 126 MB L2
@@ -372,7 +377,8 @@ def run_gpu(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
-            "config": {"workload": cfg["name"], "n_fluid": nfl, "n_wall": nwl, "dim": cfg["dim"],
+            "config": {"workload": cfg["name"] + ("+wall_osc(%s)" % args.wall_osc if args.wall_osc else ""),
+                       "n_fluid": nfl, "n_wall": nwl, "dim": cfg["dim"],
                        "dp": cfg["dp"], "l2": "flushed between timed steps (256 MiB write)",
                        "parallelism": "replicas only" if world > 1 else "1 gpu"},
             "pair_interactions_per_s": pairs_s, "pairs_per_step": fluid_pairs,
@@ -436,6 +442,8 @@ def main():
     ap.add_argument("--cpu-steps", type=int, default=25,
                     help="oracle steps of the cpu_baseline leg (cfg1 full size: about 0.4 s per step on 16 cores)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--wall-osc", default="", metavar="A0,F0",
+                    help="move the walls along x as A0 sin(2 pi F0 t) (metres, Hz); implies a non-headline line")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
