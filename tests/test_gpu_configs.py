@@ -60,6 +60,30 @@ def test_cfg1_dam_break_3d_box_full_size():
     _steps_and_compare(cfg, 3)
 
 
+def test_cfg1_moving_walls_full_size():
+    """Config 1 at full size with the wall motion `bench.py --wall-osc 0.01,0.5` times (NEXT-1,
+    PAPER.md:252, :116): set-up, then 3 steps on the oracle's dt sequence; the walls sit on
+    x_w(0) + A0 sin(2 pi f0 t)."""
+    cfg = dict(inputs.dam_break_3d_box())
+    cfg["wall_osc_amp"], cfg["wall_osc_freq"] = (0.01, 0.0, 0.0), 0.5
+    o, g = make_pair(cfg)
+    e0 = compare_fields(cfg, o, g, names=("rho", "p", "acc"))
+    assert max(e0.values()) < TOL, ("set-up", e0)
+    dts = o.step(3)
+    g.step(3, dts=dts)
+    e = compare_fields(cfg, o, g, names=("rho", "p", "acc", "vel", "pos"))
+    assert max(e.values()) < TOL, e
+    wall = cfg["tag"] < 0
+    pg = g.get_fields(device=False, which=("pos",))["pos"]
+    want = cfg["pos"][wall].astype(np.float64)
+    want[:, 0] += 0.01 * np.sin(2.0 * np.pi * 0.5 * float(np.sum(dts)))
+    assert np.max(np.abs(pg[wall] - want)) < 2e-7 * max(1.0, np.abs(want).max())
+    sg = g.get_stats()
+    assert sg["escaped"] == 0 and sg["nonfinite"] == 0
+    missing, extra, total = g.debug_list_check()
+    assert missing == 0 and extra <= 0.06 * total
+
+
 def test_cfg1_cells_bit_exact_full_size():
     cfg = inputs.dam_break_3d_box()
     g = sph.Sph(cfg)
