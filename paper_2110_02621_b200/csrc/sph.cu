@@ -77,6 +77,13 @@ struct sph_ctx {
   uint4* WX0 = nullptr;
   float4* WN0 = nullptr;   // wall normals in set-up order (translation-invariant)
   unsigned *WID0 = nullptr, *WkeyA = nullptr, *WkeyB = nullptr, *WvalA = nullptr, *WvalB = nullptr;
+  // the re-sort runs on its own stream beside the fluid's predict / sort / reorder (it depends on k_dt only):
+  // own scratch, fork / join events (captured into the step graph as a parallel branch)
+  uint4* WTX = nullptr;
+  float4* WTB = nullptr;
+  unsigned *Whist = nullptr, *Wrowsum = nullptr;
+  cudaStream_t wstream = nullptr;
+  cudaEvent_t evFork = nullptr, evJoin = nullptr;
   std::map<void*, size_t> cap_bytes;  // dalloc: capacity of the buffer behind each pointer member
   float *hpos = nullptr, *hvel = nullptr, *hrho = nullptr;  // staging of sph_set_particles_host
   int32_t* htagd = nullptr;
@@ -157,17 +164,22 @@ void free_all(sph_ctx* c) {
                   c->keyA, c->valA, c->keyB, c->valB, c->hist, c->rowsum, c->lbF, c->lbW, c->WR,
                   c->WA, c->WN, c->WG, c->WK, c->WID, c->wnear, c->S, c->dt_seq, c->stat,
                   c->hpos, c->hvel, c->hrho, c->htagd, c->hout, c->hidx,
-                  c->WX0, c->WN0, c->WID0, c->WkeyA, c->WkeyB, c->WvalA, c->WvalB};
+                  c->WX0, c->WN0, c->WID0, c->WkeyA, c->WkeyB, c->WvalA, c->WvalB,
+                  c->WTX, c->WTB, c->Whist, c->Wrowsum};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   for (auto e : c->ev) cudaEventDestroy(e);
   if (c->gexec) cudaGraphExecDestroy(c->gexec);
   if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
+  if (c->evFork) cudaEventDestroy(c->evFork);
+  if (c->evJoin) cudaEventDestroy(c->evJoin);
+  if (c->wstream) cudaStreamDestroy(c->wstream);
 }
 
 // Stable radix sort of (keys, vals); result pointers returned in *ko, *vo.
 int radix_sort(sph_ctx* c, cudaStream_t st, int n, unsigned* kA, unsigned* vA, unsigned* kB, unsigned* vB,
-               unsigned** ko, unsigned** vo) {
+               unsigned** ko, unsigned** vo, unsigned* hist = nullptr, unsigned* rowsum = nullptr) {
+  if (!hist) { hist = c->hist; rowsum = c->rowsum; }
   unsigned *ki = kA, *vi = vA, *kt = kB, *vt = vB;
   if (n > 0) {
     const int items = rs_items((size_t)n), nblk = cdiv(n, RS_THREADS * items);
@@ -175,9 +187,9 @@ int radix_sort(sph_ctx* c, cudaStream_t st, int n, unsigned* kA, unsigned* vA, u
       int shift = c->sort_bits * pass;
 #define RS_PASS(ND, IT)                                                                                   \
   do {                                                                                                    \
-    LAUNCH((k_radix_hist<ND, IT>), nblk, RS_THREADS, st, ki, n, shift, c->hist, nblk, c->rowsum);         \
-    LAUNCH(k_scan_apply, ND, 256, st, c->hist, nblk, c->rowsum);                                          \
-    LAUNCH((k_radix_scatter<ND, IT>), nblk, RS_THREADS, st, ki, vi, n, shift, c->hist, nblk, kt, vt, c->rowsum); \
+    LAUNCH((k_radix_hist<ND, IT>), nblk, RS_THREADS, st, ki, n, shift, hist, nblk, rowsum);               \
+    LAUNCH(k_scan_apply, ND, 256, st, hist, nblk, rowsum);                                                \
+    LAUNCH((k_radix_scatter<ND, IT>), nblk, RS_THREADS, st, ki, vi, n, shift, hist, nblk, kt, vt, rowsum); \
   } while (0)
       if (c->sort_bits == 9) { if (items == 4) RS_PASS(512, 4); else RS_PASS(512, 16); }
       else { if (items == 4) RS_PASS(256, 4); else RS_PASS(256, 16); }
@@ -221,19 +233,20 @@ void launch_wall(sph_ctx* c, cudaStream_t st, bool with_vel, const XB* R) {
 }
 
 // NEXT-1 (moving walls): the walls at their positions of t^{n+1}, re-sorted into the cell grid (the
-// same kernels as the set-up; TX / TB are free between the fluid reorder and pass B).
+// same kernels as the set-up, on scratch of their own: `st` is the wall stream, which runs beside the
+// fluid's predict / sort / reorder).
 int wall_rebuild(sph_ctx* c, cudaStream_t st) {
   const int nw = (int)c->nw;
   if (nw == 0) return SPH_OK;
-  LAUNCH(k_wall_shift, cdiv(nw, 256), 256, st, c->dp, c->S, nw, c->WX0, c->TX, c->TB, c->WkeyA, c->WvalA);
+  LAUNCH(k_wall_shift, cdiv(nw, 256), 256, st, c->dp, c->S, nw, c->WX0, c->WTX, c->WTB, c->WkeyA, c->WvalA);
   unsigned *ks, *vs;
-  int rc = radix_sort(c, st, nw, c->WkeyA, c->WvalA, c->WkeyB, c->WvalB, &ks, &vs);
+  int rc = radix_sort(c, st, nw, c->WkeyA, c->WvalA, c->WkeyB, c->WvalB, &ks, &vs, c->Whist, c->Wrowsum);
   if (rc) return rc;
-  LAUNCH(k_reorder, cdiv(nw, 256), 256, st, c->dp, nw, vs, c->TX, c->TB, c->WID0, c->WR, c->WA, c->WID,
-         (const unsigned*)nullptr, -1, (int*)nullptr);
+  // gather + wall cell lower bounds in one launch, as for the fluid
+  LAUNCH(k_reorder, std::max(cdiv(nw, 256), cdiv(c->ncell + 1, 256)), 256, st, c->dp, nw, vs, c->WTX, c->WTB, c->WID0,
+         c->WR, c->WA, c->WID, ks, (int)c->ncell, c->lbW);
   CK(cudaMemcpyAsync(c->WK, ks, sizeof(unsigned) * nw, cudaMemcpyDeviceToDevice, st));
   LAUNCH(k_image, cdiv(nw, 256), 256, st, c->dp, nw, c->WR, c->WG);
-  LAUNCH(k_cell_bounds, cdiv(c->ncell + 1, 256), 256, st, ks, nw, (int)c->ncell, c->lbW);
   LAUNCH(k_gather4, cdiv(nw, 256), 256, st, nw, vs, c->WN0, c->WN);  // normals: translation-invariant
   LAUNCH(k_wnear, cdiv(c->ncell, 256), 256, st, c->dp, (int)c->ncell, c->lbW, c->wnear);
   return SPH_OK;
@@ -255,10 +268,7 @@ int pipeline_after_hash(sph_ctx* c, cudaStream_t st, int init, Prof& pf) {
   } else {
     LAUNCH(k_cell_bounds, cdiv(c->ncell + 1, 256), 256, st, ks, nf, (int)c->ncell, c->lbF);
   }
-  if (c->moving && !init) {
-    rc = wall_rebuild(c, st);
-    if (rc) return rc;
-  }
+  if (c->moving && !init && c->nw > 0) CK(cudaStreamWaitEvent(st, c->evJoin, 0));  // join the wall branch of one_step
   pf.mark();  // end reorder
   launch_wall(c, st, true, c->R0);
   pf.mark();  // end wall 1
@@ -304,6 +314,16 @@ int do_steps(sph_ctx* c, int32_t n_steps, const double* dt_host, cudaStream_t st
   auto one_step = [&](cudaStream_t q, const double* seq, int s, Prof& pf) -> int {
     pf.mark();  // start
     LAUNCH(k_dt, dt_grid, 256, q, c->dp, c->S, nf, c->TB, seq, s);
+    if (c->moving && c->nw > 0) {
+      // NEXT-1: the wall re-sort needs the displacement of t^{n+1} (k_dt) and nothing of the fluid: fork
+      // it onto the wall stream; pipeline_after_hash joins before the first wall pass.  Under capture
+      // the events make it a parallel branch of the step graph.
+      CK(cudaEventRecord(c->evFork, q));
+      CK(cudaStreamWaitEvent(c->wstream, c->evFork, 0));
+      int rcw = wall_rebuild(c, c->wstream);
+      if (rcw) return rcw;
+      CK(cudaEventRecord(c->evJoin, c->wstream));
+    }
     if (nf > 0)
       LAUNCH(k_predict, cdiv(nf, 256), 256, q, c->dp, c->S, nf, c->R1, c->TB, c->ACC, c->SIG, c->TX, c->keyA, c->valA);
     pf.mark();  // end predict
@@ -555,8 +575,13 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
     LAUNCH(k_load, cdiv(nw, 256), 256, st, c->dp, nw, 1, idx, pos, vel, rho, tag, c->TX, c->TB, c->ID0, c->keyA, c->valA);
     if (c->moving) {  // NEXT-1: keep the set-up order for the per-step re-sort
       rc = dalloc(c, &c->WX0, nw) | dalloc(c, &c->WN0, nw) | dalloc(c, &c->WID0, nw) | dalloc(c, &c->WkeyA, nw) | dalloc(c, &c->WkeyB, nw) |
-           dalloc(c, &c->WvalA, nw) | dalloc(c, &c->WvalB, nw);
+           dalloc(c, &c->WvalA, nw) | dalloc(c, &c->WvalB, nw) | dalloc(c, &c->WTX, nw) | dalloc(c, &c->WTB, nw) |
+           dalloc(c, &c->Whist, (size_t)512 * cdiv(nw, RS_THREADS * rs_items((size_t)nw))) | dalloc(c, &c->Wrowsum, 512);
       if (rc) return rc;
+      CK(cudaMemsetAsync(c->Wrowsum, 0, 512 * sizeof(unsigned), st));
+      if (!c->wstream) CK(cudaStreamCreateWithFlags(&c->wstream, cudaStreamNonBlocking));
+      if (!c->evFork) CK(cudaEventCreateWithFlags(&c->evFork, cudaEventDisableTiming));
+      if (!c->evJoin) CK(cudaEventCreateWithFlags(&c->evJoin, cudaEventDisableTiming));
       CK(cudaMemcpyAsync(c->WX0, c->TX, sizeof(uint4) * nw, cudaMemcpyDeviceToDevice, st));
       CK(cudaMemcpyAsync(c->WID0, c->ID0, sizeof(unsigned) * nw, cudaMemcpyDeviceToDevice, st));
     }
