@@ -381,10 +381,18 @@ def test_stage_timings_and_launch_count():
     assert g.launch_count() > l0
 
 
-def test_graph_replay_equals_direct_launches_bitwise():
+@pytest.mark.parametrize("moving", [False, True])
+def test_graph_replay_equals_direct_launches_bitwise(moving):
     """sph_step replays one captured step as a CUDA graph; SPH_FLAG_NO_GRAPH issues the same
-    kernels directly.  Same kernels, same arguments: the states must be bit-identical."""
-    cfg = inputs.box_sweep_3d(n=14)
+    kernels directly.  Same kernels, same arguments: the states must be bit-identical.  With moving
+    walls the wall re-sort is a parallel branch of the graph (fork after k_dt, join before the first
+    wall pass) and two real streams in the direct path."""
+    cfg = dict(inputs.box_sweep_3d(n=14))
+    if moving:
+        pad = 0.01
+        cfg["domain_min"] = [x - pad for x in cfg["domain_min"]]
+        cfg["domain_max"] = [x + pad for x in cfg["domain_max"]]
+        cfg["wall_osc_amp"], cfg["wall_osc_freq"] = (0.003, 0.0, 0.002), 4.0
     cfg2 = dict(cfg)
     cfg2["flags"] = cfg["flags"] | 4          # SPH_FLAG_NO_GRAPH
     out = []
@@ -392,9 +400,9 @@ def test_graph_replay_equals_direct_launches_bitwise():
         g = sph.Sph(c)
         g.set_particles(c["pos"], c["vel"], c["rho"], c["tag"])
         g.step(3)
-        g.step(4)                             # second call reuses the captured graph
+        g.step(40 if moving else 4)           # second call reuses the captured graph
         out.append(g.get_fields(device=False))
-        assert g.get_stats()["steps"] == 7
+        assert g.get_stats()["steps"] == (43 if moving else 7)
     for k in out[0]:
         assert np.array_equal(out[0][k], out[1][k]), k
 
