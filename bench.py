@@ -6,14 +6,16 @@ Contract (driver): `python bench.py --gpus N --steps K --warmup W` prints ONE JS
   step      one sph_step(1): dt reduction, reinit, kick, drift, cell hash, radix sort, reorder,
             wall extrapolation x2, neighbour-list build, pair pass A, pair pass B (+ second kick)
             on one synthetic config (replayed as a CUDA graph of the same kernels)
-  workload  BASELINE.json configs[1] (3-D dam break with box obstacle, ~0.68 M fluid + ~0.47 M wall)
-            unless --config says otherwise; inputs are seeded/synthetic (paper_2110_02621_b200.inputs)
+  workload  BASELINE.json configs[4] at N_fluid = 16.8 M (cfg4_256: the size the target's ">= 50 % of the
+            roofline at >= 16 M particles" is quoted at; the other sizes of the sweep and configs 0-3 via
+            --config); inputs are seeded/synthetic (paper_2110_02621_b200.inputs)
   value     fluid particle-steps/s with the state resident in HBM (CUDA events on the launching
             stream; L2 flushed between timed steps; max over ranks)
   e2e       same metric through the HOST-pointer C-ABI calls: sph_set_particles_host + K x
             (sph_step(1) + sph_get_stats) + sph_get_fields_host, all inside the timed region
   roofline  the dominant kernel (largest stage time) against the FP32 ALU peak
-  cpu_baseline  the CPU oracle (oracle/, as it stands) on the host cores, bounded sample
+  cpu_baseline  the CPU oracle (oracle/, as it stands) on the host cores, on a bounded sample of the same
+            workload: for the cfg4 sweep its 1 M size (cfg4_100), else the config itself
 
 N > 1: replicas only: every rank runs the same configuration independently, no
 data-path collective; value = particle-steps of all ranks / max-over-ranks time; scaling "weak".
@@ -42,24 +44,41 @@ UNIT = "fluid particle-steps/s"
 # separately (CAND_FLOPS each) because they are overhead of the 27-cell walk, not of the method.
 FLOPS_HIT = {"pass_a": 40.0, "pass_b": 50.0, "wall": 30.0}
 CAND_FLOPS = 8.0
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from `ncu --set full` captures of these
-# exact workloads (profiles/r01e_README.md); other workloads report traffic = null.
-NCU_TRAFFIC_BYTES = {
-    ("cfg1_dam_break_3d_box", "k_pass_a"): 258.86e6 + 19.56e6,
-    ("cfg1_dam_break_3d_box", "k_pass_b"): 260.51e6 + 18.69e6,
-    ("cfg1_dam_break_3d_box", "k_build"): 90.55e6 + 240.98e6,
-    ("cfg4_box_160", "k_pass_a"): 1579.8e6 + 157.9e6,
-    ("cfg4_box_160", "k_pass_b"): 1588.0e6 + 142.6e6,
-    ("cfg4_box_160", "k_build"): 595.6e6 + 1790.4e6,
-}
-# l1tex__data_pipe_lsu_wavefronts (fraction of peak) and sm__issue_active of the same captures: the pair
-# passes are bound by the tag stage of L1 (record gathers), not by FP32 issue.
-NCU_L1_ISSUE = {
-    ("cfg1_dam_break_3d_box", "k_pass_a"): (0.760, 0.547),
-    ("cfg1_dam_break_3d_box", "k_pass_b"): (0.753, 0.562),
-    ("cfg4_box_160", "k_pass_a"): (0.859, 0.606),
-    ("cfg4_box_160", "k_pass_b"): (0.887, 0.650),
-}
+# ncu counters of the dominant kernels (dram bytes per launch, L1 data-pipe wavefronts and issue-active as
+# fractions of peak) are looked up in a committed table of `ncu --set full` captures, profiles/ncu_kernels.csv,
+# keyed by workload, kernel AND the hash of the kernel sources they were captured from (csrc_hash() below):
+# a capture of other sources is stale and yields null, never a number.
+NCU_TABLE = os.path.join(ROOT, "profiles", "ncu_kernels.csv")
+
+
+def csrc_hash():
+    """sha256 (first 16 hex digits) over include/sph.h and paper_2110_02621_b200/csrc/*, sorted by name."""
+    import glob
+    import hashlib
+    h = hashlib.sha256()
+    files = [os.path.join(ROOT, "include", "sph.h")] + sorted(glob.glob(os.path.join(ROOT, "paper_2110_02621_b200", "csrc", "*")))
+    for f in files:
+        h.update(os.path.basename(f).encode())
+        with open(f, "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_lookup(workload, kernel):
+    """Row of profiles/ncu_kernels.csv for (workload, kernel, csrc_hash()) or None."""
+    import csv
+    try:
+        with open(NCU_TABLE) as fh:
+            rows = [r for r in csv.DictReader(l for l in fh if not l.startswith("#"))]
+    except OSError:
+        return None
+    hsh = csrc_hash()
+    for r in rows:
+        if r["workload"] == workload and r["kernel"] == kernel and r["csrc_hash"] == hsh:
+            return r
+    return None
+
+
 FP32_LANES_PER_SM = 128
 N_SM = 148
 
@@ -86,8 +105,12 @@ def make_config(name):
         return inputs.sloshing_spheres_3d()
     if name == "cfg3_4m":
         return inputs.sloshing_spheres_3d(dp=0.00585)
+    if name == "cfg3_small":
+        return inputs.sloshing_spheres_3d(dp=0.0125)
     if name.startswith("cfg4_"):
         return inputs.box_sweep_3d(n=int(name.split("_")[1]))
+    if name.startswith("x1_"):   # NEXT-2: the paper's two-phase hydrostatic tank, e.g. x1_0.005
+        return inputs.hydrostatic_tank_x1(dp=float(name.split("_")[1]))
     raise SystemExit("unknown --config %r" % name)
 
 
@@ -198,17 +221,28 @@ def oracle_rate(cfg, steps, warmup=0):
     return cfg["n_fluid"] * steps / dt, dt, os.cpu_count() or 1
 
 
+def cpu_sample_config(name):
+    """Bounded sample of workload `name` for the oracle legs (about 10-30 s of CPU work for 10-25 steps):
+    the cfg4 sweep is sampled at its 1 M size (same recipe), cfg3 at dp = 0.0125,
+    cfg1 at full size when few steps are asked for, everything else as is."""
+    if name.startswith("cfg4_") and int(name.split("_")[1]) > 100:
+        return "cfg4_100", "cfg4 sweep at its N_fluid = 1 M size"
+    if name in ("cfg3", "cfg3_4m"):
+        return "cfg3_small", "cfg3 geometry at dp = 0.0125"
+    return name, "full size"
+
+
 def run_reference(args):
     """--impl reference: the CPU oracle as it stands (this tier's reference arm), rank 0 only."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
-    full = (args.steps + args.warmup) <= 30 and args.config == "cfg1"
-    name = args.config if full else ("cfg1_small" if args.config == "cfg1" else args.config)
+    name, what = cpu_sample_config(args.config)
+    if name == "cfg1" and (args.steps + args.warmup) > 30:
+        name, what = "cfg1_small", "cfg1 at dp = 0.02"
     cfg = make_config(name)
     rate, secs, cores = oracle_rate(cfg, args.steps, args.warmup)
-    sample = "%s (%d fluid + %d wall particles), %d steps after %d warm-up" % (
-        cfg["name"] + ("" if full or name == args.config else " at dp=0.02"), cfg["n_fluid"],
-        cfg["n_wall"], args.steps, args.warmup)
+    sample = "%s: %s (%d fluid + %d wall particles), %d steps after %d warm-up" % (
+        what, cfg["name"], cfg["n_fluid"], cfg["n_wall"], args.steps, args.warmup)
     line = {
         "impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * secs / max(args.steps, 1),
@@ -295,7 +329,14 @@ def run_gpu(args):
     wall_pairs = int((off[1:] - off[:-1])[tag < 0].sum())
     fluid_pairs = int(st["npairs"])
     sm_max = clocks.get("sm_max_mhz") or 1965.0
-    peak = N_SM * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12       # TFLOP/s at max SM clock
+    peak_derived = N_SM * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12       # TFLOP/s at max SM clock
+    # measured non-tensor FP32 peak (SURVEY.md section 8(d) "Peaks"): register-resident FMA loop, this device, now
+    fma_sampler = ClockSampler(local)
+    fma_sampler.start()
+    peak = sph.fma_peak_tflops()
+    for _ in range(20):             # keep the loop running long enough for nvidia-smi to sample its clocks
+        peak = max(peak, sph.fma_peak_tflops())
+    fma_clocks = fma_sampler.stop()
     kern = {}
     # Pair stages.  The 27-cell candidate walk runs once per step in k_build (fluid-fluid) and inside
     # k_wall / the wall part of the passes (fluid-wall); the fluid pair passes read the neighbour lists.
@@ -322,12 +363,15 @@ def run_gpu(args):
         if t > 0:
             kern[name] = {"ms": 1e3 * t, "gbs": b * nfl / t / 1e9, "frac_hbm": b * nfl / t / 1e9 / hbm}
     dom = max(("pass_a", "pass_b"), key=lambda k: stage_ms[k])   # the list build is reported under "kernels"
+    ncu = ncu_lookup(cfg["name"], "k_" + dom)
     roofline = {"bound": "alu", "kernel": "k_" + dom, "achieved": kern[dom]["tflops_hit_only"],
                 "peak": peak, "unit": "TFLOP/s", "frac": kern[dom]["frac_hit_only"],
-                "traffic": NCU_TRAFFIC_BYTES.get((cfg["name"], "k_" + dom)),
-                "l1_data_pipe_frac_ncu": (NCU_L1_ISSUE.get((cfg["name"], "k_" + dom)) or (None, None))[0],
-                "issue_active_frac_ncu": (NCU_L1_ISSUE.get((cfg["name"], "k_" + dom)) or (None, None))[1],
-                "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 flop x clocks.max.sm (DESIGN.md §7); MEASURED_PEAKS.json holds no non-tensor FP32 peak",
+                "traffic": float(ncu["dram_bytes"]) if ncu else None,
+                "l1_data_pipe_frac_ncu": float(ncu["l1_data_pipe_frac"]) if ncu else None,
+                "issue_active_frac_ncu": float(ncu["issue_active_frac"]) if ncu else None,
+                "ncu_capture": (ncu["capture"] if ncu else None), "csrc_hash": csrc_hash(),
+                "peak_source": "measured: sph_debug_fma_peak (register-resident FMA loop, 8 chains x 2048 threads per SM) on this device in this run",
+                "peak_derived": peak_derived, "peak_clocks": {"sm_mhz": fma_clocks.get("sm_mhz"), "sm_max_mhz": fma_clocks.get("sm_max_mhz")},
                 "flops_per_hit": FLOPS_HIT[dom], "flops_per_candidate": CAND_FLOPS,
                 # list build + pass A + pass B together (the candidate walk is k_build's):
                 "pair_stages": pair_stages}
@@ -368,9 +412,11 @@ def run_gpu(args):
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
         osteps = args.cpu_steps
-        rate, secs, cores = oracle_rate(cfg, osteps)
+        cname, what = cpu_sample_config(args.config)
+        ccfg = cfg if cname == args.config else make_config(cname)
+        rate, secs, cores = oracle_rate(ccfg, osteps)
         cpu = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
-               "sample": "%s full size (%d fluid + %d wall), %d steps, %.1f s" % (cfg["name"], nfl, nwl, osteps, secs)}
+               "sample": "%s: %s (%d fluid + %d wall), %d steps, %.1f s" % (what, ccfg["name"], ccfg["n_fluid"], ccfg["n_wall"], osteps, secs)}
 
     if rank == 0:
         line = {
@@ -438,13 +484,18 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="cfg1")
-    ap.add_argument("--cpu-steps", type=int, default=25,
-                    help="oracle steps of the cpu_baseline leg (cfg1 full size: about 0.4 s per step on 16 cores)")
+    ap.add_argument("--config", default="cfg4_256",
+                    help="cfg0 cfg1 cfg2a cfg2b cfg3 cfg3_4m cfg4_<n> (n^3 fluid particles) x1_<dp>; default cfg4_256 (16.8 M)")
+    ap.add_argument("--cpu-steps", type=int, default=20,
+                    help="oracle steps of the cpu_baseline leg (1 M particles: about 0.6 s per step on 16 cores)")
+    ap.add_argument("--csrc-hash", action="store_true", help="print the hash profiles/ncu_kernels.csv is keyed by and exit")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--wall-osc", default="", metavar="A0,F0",
                     help="move the walls along x as A0 sin(2 pi F0 t) (metres, Hz); implies a non-headline line")
     args = ap.parse_args()
+    if args.csrc_hash:
+        print(csrc_hash())
+        return
     if args.impl == "reference":
         run_reference(args)
     else:

@@ -40,8 +40,12 @@ enum { SPH_MAX_PHASES = 4, SPH_TAG_WALL = -1 };
 enum sph_flags {
   SPH_FLAG_REINIT = 1,          /* density reinitialisation each step, Eq. 2.17/2.18 */
   SPH_FLAG_WALL_VEL_MIRROR = 2, /* v_w = 2 v_wall - <v_f> (Adami-style mirror; reading A6), else v_w = v_wall */
-  SPH_FLAG_NO_GRAPH = 4         /* sph_step issues every kernel itself instead of replaying one captured step
+  SPH_FLAG_NO_GRAPH = 4,        /* sph_step issues every kernel itself instead of replaying one captured step
                                    as a CUDA graph (same kernels, same results) */
+  SPH_FLAG_WALL_ADAMI_ONLY = 8  /* NEXT-4 ablation, PAPER.md:99, :250 ("compare the results with the method of Adami et
+                                   al. (2012)"): the wall model without the paper's extensions: Eq. 2.12 in its
+                                   single-phase form for every phase (no division by rho_f) and no
+                                   penalty force F_p (Eq. 2.13), whatever penalty_phase_mask says */
 };
 
 enum sph_error {
@@ -69,8 +73,10 @@ typedef struct {
   double cfl;                    /* 0.25 in Eq. 2.23 and 2.24 */
   double penalty_strength;       /* gamma_p (paper: 1) */
   uint32_t penalty_phase_mask;   /* bit k: phase k receives F_p, Eq. 2.13 (reading A11) PAPER.md:120 */
-  uint32_t free_surface_mask;    /* bit k: phase k uses continuity Eq. 2.9/2.21 + reinit Eq. 2.17;
-                                    otherwise summation Eq. 2.4 + reinit Eq. 2.18 (reading A13, A15) */
+  uint32_t free_surface_mask;    /* bit k: phase k uses continuity Eq. 2.9/2.21 + reinit Eq. 2.17, and in a multi-phase
+                                    run its number density sigma_i counts its own phase and the walls only (reading
+                                    A13b, "free-surface-like flow"); otherwise summation Eq. 2.4 + reinit
+                                    Eq. 2.18 with sigma_i over every neighbour (reading A13, A15) */
   uint32_t flags;                /* sph_flags */
   uint32_t max_neighbours;       /* capacity of the per-particle fluid-fluid neighbour lists; 0 = default (160 in 3-D,
                                     64 in 2-D); the fluid-wall lists hold 3/4 of it */
@@ -192,6 +198,20 @@ int sph_probe_gauge(sph_ctx* ctx, int32_t m, const float* xyz_host, float* eta_h
  * reading B2), out3_host[2] = list entries in total (self entries included).  HOST pointer to 3
  * values; synchronises the stream.  Errors: SPH_EINVAL without particles, SPH_ECUDA. */
 int sph_debug_list_check(sph_ctx* ctx, int64_t* out3_host, void* stream);
+
+/* The neighbour lists the pair passes (pass A, pass B) and the second wall pass of a step actually READ, in CSR
+ * form with caller ids: row of a fluid particle = its fluid-fluid list (the self entry included) followed by its
+ * fluid-wall list; row of a wall particle = its wall-fluid list.  Entries are in list order (not sorted) and
+ * include the false positives of the conservative candidate filter (reading B2: they add exactly 0).  Same
+ * argument meaning as sph_debug_neighbours; all pointers HOST; synchronises.  A host-side test compares them
+ * with the oracle's float32 contract lists (superset, every extra entry within the documented margin). */
+int sph_debug_step_lists(sph_ctx* ctx, int64_t* offsets_host, int32_t* ids_host, int64_t cap,
+                         int64_t* total_host, void* stream);
+
+/* Measured non-tensor FP32 peak of the current device: a register-resident FMA loop (8 independent chains per
+ * thread, 2048 threads per SM, no memory traffic), best of 4 timed launches after 2 warm-up launches, in
+ * TFLOP/s (fma = 2 flop).  SURVEY.md section 8(d) "Peaks"; bench.py's roofline denominator.  Needs no context. */
+int sph_debug_fma_peak(double* tflops_host, void* stream);
 
 /* Wall normals Eq. 2.16 in caller order (n*3, zero for fluid entries); HOST pointer. */
 int sph_debug_normals(sph_ctx* ctx, float* normals_host, void* stream);

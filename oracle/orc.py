@@ -13,6 +13,10 @@ MAX_PHASES = 4
 TAG_WALL = -1
 FLAG_REINIT = 1
 FLAG_WALL_VEL_MIRROR = 2
+FLAG_WALL_ADAMI_ONLY = 8
+VAR_REINIT_LITERAL = 1   # study-only variants (NEXT-2): see sph_oracle.cpp
+VAR_SUM_RAW = 2
+VAR_SIGMA_ALL = 4
 
 
 class OrcParams(C.Structure):
@@ -23,7 +27,7 @@ class OrcParams(C.Structure):
         ("g", C.c_double * 3), ("g_osc_amp", C.c_double * 3), ("g_osc_period", C.c_double),
         ("cfl", C.c_double), ("penalty_strength", C.c_double),
         ("penalty_phase_mask", C.c_uint32), ("free_surface_mask", C.c_uint32),
-        ("flags", C.c_uint32), ("reserved", C.c_uint32),
+        ("flags", C.c_uint32), ("variant", C.c_uint32),
         ("domain_min", C.c_double * 3), ("domain_max", C.c_double * 3),
         ("wall_osc_amp", C.c_double * 3), ("wall_osc_freq", C.c_double), ("t_start", C.c_double),
     ]
@@ -86,6 +90,7 @@ def make_params(cfg: dict) -> OrcParams:
     P.penalty_phase_mask = cfg.get("penalty_phase_mask", 0)
     P.free_surface_mask = cfg.get("free_surface_mask", 1)
     P.flags = cfg.get("flags", FLAG_REINIT | FLAG_WALL_VEL_MIRROR)
+    P.variant = cfg.get("oracle_variant", 0)
     return P
 
 

@@ -45,6 +45,21 @@ constexpr int ORC_MAX_PHASES = 4;
 constexpr int ORC_TAG_WALL = -1;
 constexpr uint32_t ORC_FLAG_REINIT = 1u;
 constexpr uint32_t ORC_FLAG_WALL_VEL_MIRROR = 2u;
+// NEXT-4 ablation ("compare the results with the method of Adami et al. (2012)"): the wall
+// model WITHOUT the paper's extensions: Eq. 2.12 in its single-phase form for every phase (no division by
+// rho_f) and no penalty force F_p (Eq. 2.13).
+constexpr uint32_t ORC_FLAG_WALL_ADAMI_ONLY = 8u;
+// Study-only variants of two readings (NEXT-2, DESIGN.md section 3 A13 / A15); never set by the parity tests:
+//   REINIT_LITERAL  the printed assignment of PAPER.md:155: Eq. 2.17 for the light (summation) phases,
+//                   Eq. 2.18 for the heavy (continuity) phases, i.e. the reverse of reading A13;
+//   SUM_RAW         Eq. 2.4 as printed, rho_i = m_i sum_j W_ij (incl. the self term), instead of the
+//                   normalised form rho0 sigma / sigma0 of reading A15.
+constexpr uint32_t ORC_VAR_REINIT_LITERAL = 1u;
+constexpr uint32_t ORC_VAR_SUM_RAW = 2u;
+//   SIGMA_ALL       sigma_i of a free-surface (continuity) phase counts neighbours of EVERY phase, as the
+//                   first build of this oracle did; reading A13b counts the particle's own phase and the
+//                   walls only (see number density below).
+constexpr uint32_t ORC_VAR_SIGMA_ALL = 4u;
 
 struct orc_params {
   int32_t dim;
@@ -61,7 +76,7 @@ struct orc_params {
   uint32_t penalty_phase_mask;
   uint32_t free_surface_mask;
   uint32_t flags;
-  uint32_t reserved;
+  uint32_t variant;     // ORC_VAR_* (0 in every parity run)
   double domain_min[3];
   double domain_max[3];
   // NEXT-1: rigid wall motion x_w(t) = x_w(t_start) + A [sin(2 pi f t) - sin(2 pi f t_start)]
@@ -323,7 +338,19 @@ void wall_normals(Ctx& S) {
   }
 }
 
-// sigma_i = W(0) + sum_j W_ij over neighbours of any tag (A14).
+// Which neighbours j enter sigma_i ("sigma_i = sum W_ij"; reading A13b).  PAPER.md:155: "the
+// light phase experiences the heavy phase like moving wall boundary, while the heavy phase undergoes a
+// free-surface-like flow with variable free-surface pressure": in a multi-phase run the number density
+// of a free-surface (heavy) phase particle counts its own phase and the walls, NOT the light phase, so
+// that Eq. 2.17 sees the interface as the free surface the sentence describes; an internal-flow (light)
+// phase particle counts every neighbour (the heavy phase is its moving wall).  Single phase: everything.
+inline bool counts_in_sigma(const Ctx& S, int64_t i, int64_t j) {
+  if (S.P.n_phases < 2 || (S.P.variant & ORC_VAR_SIGMA_ALL) || is_wall(S, i)) return true;
+  if (!((S.P.free_surface_mask >> S.tag[i]) & 1u)) return true;
+  return is_wall(S, j) || S.tag[j] == S.tag[i];
+}
+
+// sigma_i = W(0) + sum_j W_ij (A14, A13b).
 void number_density(Ctx& S) {
   const int dim = S.P.dim;
   const double h = S.P.h;
@@ -333,6 +360,7 @@ void number_density(Ctx& S) {
     double s = w0;
     for (int64_t q = S.nb_off[i]; q < S.nb_off[i + 1]; ++q) {
       int64_t j = S.nb[q];
+      if (!counts_in_sigma(S, i, j)) continue;
       double r2 = 0;
       for (int k = 0; k < 3; ++k) {
         double d = S.r[3 * i + k] - S.r[3 * j + k];
@@ -352,6 +380,7 @@ void reinitialise(Ctx& S) {
     if (is_wall(S, i)) continue;
     int ph = S.tag[i];
     int fs = (S.P.free_surface_mask >> ph) & 1u;
+    if (S.P.variant & ORC_VAR_REINIT_LITERAL) fs = !fs;
     S.rho[i] = reinit_density(S.rho[i], S.P.rho0[ph], S.sigma[i], S.sigma0, fs);
     S.p[i] = S.P.c0[ph] * S.P.c0[ph] * (S.rho[i] - S.P.rho0[ph]);  // Eq. 2.3
   }
@@ -383,7 +412,7 @@ void wall_extrapolate(Ctx& S, const double g_in[3], bool with_velocity, double t
   const double g[3] = {g_in[0] - aw[0], g_in[1] - aw[1], g_in[2] - aw[2]};
   const int dim = S.P.dim;
   const double h = S.P.h;
-  const bool multi = S.P.n_phases > 1;
+  const bool multi = S.P.n_phases > 1 && !(S.P.flags & ORC_FLAG_WALL_ADAMI_ONLY);
 #pragma omp parallel for schedule(dynamic, 256)
   for (int64_t w = 0; w < S.n; ++w) {
     if (!is_wall(S, w)) continue;
@@ -467,7 +496,7 @@ void pass_continuity(Ctx& S) {
         r2 += d[k] * d[k];
       }
       double r = std::sqrt(r2);
-      sig += kernel_w(dim, h, r);
+      if (counts_in_sigma(S, i, j)) sig += kernel_w(dim, h, r);
       if (r == 0.0) continue;  // reading A21
       Right R = right_state(S, i, j);
       double e[3], UL = 0, UR = 0;
@@ -500,8 +529,10 @@ void density_update(Ctx& S, double dt) {
     int ph = S.tag[i];
     if ((S.P.free_surface_mask >> ph) & 1u)
       S.rho[i] += dt * S.drho[i];
+    else if (S.P.variant & ORC_VAR_SUM_RAW)
+      S.rho[i] = S.m[i] * S.sigma[i];                         // Eq. 2.4 as printed
     else
-      S.rho[i] = S.P.rho0[ph] * S.sigma[i] / S.sigma0;
+      S.rho[i] = S.P.rho0[ph] * S.sigma[i] / S.sigma0;        // reading A15
     S.p[i] = S.P.c0[ph] * S.P.c0[ph] * (S.rho[i] - S.P.rho0[ph]);
   }
 }
@@ -519,7 +550,7 @@ void pass_momentum(Ctx& S, const double g[3]) {
     }
     const int ph = S.tag[i];
     const double ci = S.P.c0[ph];
-    const bool pen = (S.P.penalty_phase_mask >> ph) & 1u;
+    const bool pen = ((S.P.penalty_phase_mask >> ph) & 1u) && !(S.P.flags & ORC_FLAG_WALL_ADAMI_ONLY);
     double a[3] = {g[0], g[1], g[2]};
     if (dim == 2) a[2] = 0.0;
     for (int64_t q = S.nb_off[i]; q < S.nb_off[i + 1]; ++q) {

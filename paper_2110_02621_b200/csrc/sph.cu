@@ -12,6 +12,7 @@
 #include <math.h>
 #include <stdint.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <algorithm>
@@ -282,9 +283,14 @@ int pipeline_after_hash(sph_ctx* c, cudaStream_t st, int init, Prof& pf) {
   }
   pf.mark();  // end list build
   if (nf > 0) {
+    // third template parameter of k_pass_a: SUBQ (residuals in sigma), not the filter form
+#undef PAIR_SEL
+#define PAIR_SEL(c) (((c)->prm.dim == 3 ? 4 : 0) | ((c)->multi ? 2 : 0) | ((c)->dp.subq ? 1 : 0))
     PAIR_DISPATCH(k_pass_a, cdiv(nf, PB), st, c->dp, c->S, nf, init, c->A, c->R0, c->K, c->lbF, c->WA, c->WR,
                   c->lbW, c->wnear, c->R1, c->SIG, c->DRHO, c->NL, c->NC, c->caps, c->NLW, c->NCW, c->capsw);
   }
+#undef PAIR_SEL
+#define PAIR_SEL(c) (((c)->prm.dim == 3 ? 4 : 0) | ((c)->multi ? 2 : 0) | ((c)->dp.exact_filter ? 1 : 0))
   pf.mark();  // end pass A
   launch_wall(c, st, false, c->R1);
   pf.mark();  // end wall 2
@@ -448,6 +454,11 @@ int sph_create(const sph_params* prm, sph_ctx** out) {
     d.sub_per_m = 1024.0 / d.Q;
     d.Qf = (float)d.Q; d.qh = (float)(d.Q / h); d.qhD = d.Q / h;
     d.mhqD[0] = -0.5 * d.qhD; d.mhqD[1] = d.mhqD[0] / 1024.0; d.tqD[0] = 2.0 * d.qhD; d.tqD[1] = d.tqD[0] / 1024.0;
+    // sigma from residual-exact separations (k_pass_a<.., SUBQ>) when the quantum is coarse for the case: the
+    // acceleration error from positions rounded to Q is about 15 (Q / h) (L / h) g (measured: 5.5e-4 g at
+    // config 4's 16.8 M size, Q / h = 1.4e-7, L / h = 200), so the 1e-4 bar needs (Q / h)(L / h) < 2e-6
+    d.subq = (prm->n_phases > 1 || (d.Q / h) * (Lmax / h) > 2e-6 || getenv("SPH_FORCE_SUBQ")) ? 1 : 0;
+    if (getenv("SPH_NO_SUBQ") && prm->n_phases == 1) d.subq = 0;
     d.gradcQ = (float)(-5.0 * alpha / (h * h) * d.Q);
     d.two_over_dp = (float)(2.0 * d.Q / dp);
     // candidate filter margin: rounding of the expanded form |xj|^2 - 2 xi.xj + |xi|^2 on images
@@ -466,7 +477,7 @@ int sph_create(const sph_params* prm, sph_ctx** out) {
     }
   }
   d.gamma_p = (float)prm->penalty_strength;
-  d.pen_mask = prm->penalty_phase_mask; d.fs_mask = prm->free_surface_mask; d.flags = prm->flags;
+  d.pen_mask = (prm->flags & SPH_FLAG_WALL_ADAMI_ONLY) ? 0u : prm->penalty_phase_mask; d.fs_mask = prm->free_surface_mask; d.flags = prm->flags;
   const double edge = 2.0 * h * (1.0 + 1.0 / 1024.0);  // reading A24
   d.inv_edge = (float)(1.0 / edge);
   d.ox = (float)prm->domain_min[0]; d.oy = (float)prm->domain_min[1]; d.oz = (float)prm->domain_min[2];
@@ -879,6 +890,79 @@ int sph_debug_list_check(sph_ctx* c, int64_t* out3, void* stream) {
   cudaFree(d);
   if (e != cudaSuccess || e2 != cudaSuccess) { c->err = cudaGetErrorString(e != cudaSuccess ? e : e2); return SPH_ECUDA; }
   for (int k = 0; k < 3; ++k) out3[k] = (int64_t)h[k];
+  return SPH_OK;
+}
+
+int sph_debug_step_lists(sph_ctx* c, int64_t* offsets, int32_t* ids, int64_t cap, int64_t* total, void* stream) {
+  if (!c || !offsets || !total) return SPH_EINVAL;
+  if (!c->loaded) { c->err = "no particles"; return SPH_EINVAL; }
+  cudaStream_t st = (cudaStream_t)stream;
+  const int64_t n = c->n;
+  int* dcnt = nullptr;
+  CK(cudaMalloc((void**)&dcnt, std::max<int64_t>(n, 1) * 4));
+  CK(cudaMemsetAsync(dcnt, 0, std::max<int64_t>(n, 1) * 4, st));
+  auto run = [&](int mode, const long long* doff, int* dids, long long dcap) {
+    if (c->nf)
+      LAUNCH(k_list_export, cdiv(c->nf, 256), 256, st, (int)c->nf, mode, c->IDcur, c->NL, c->NC, c->caps, c->IDcur,
+             c->NLW, c->NCW, c->capsw, c->WID, dcnt, doff, dids, dcap);
+    if (c->nw && c->nf)
+      LAUNCH(k_list_export, cdiv(c->nw, 256), 256, st, (int)c->nw, mode, c->WID, c->NLF, c->NCF, c->capsw, c->IDcur,
+             (const uint4*)nullptr, (const int*)nullptr, 0, (const unsigned*)nullptr, dcnt, doff, dids, dcap);
+  };
+  run(0, nullptr, nullptr, 0);
+  std::vector<int> hc((size_t)n);
+  if (n) CK(cudaMemcpyAsync(hc.data(), dcnt, n * 4, cudaMemcpyDeviceToHost, st));
+  CK(cudaStreamSynchronize(st));
+  offsets[0] = 0;
+  for (int64_t i = 0; i < n; ++i) offsets[i + 1] = offsets[i] + hc[i];
+  *total = offsets[n];
+  int rc = SPH_OK;
+  if (ids && cap > 0 && n > 0) {
+    long long* doff = nullptr;
+    int* dids = nullptr;
+    CK(cudaMalloc((void**)&doff, (n + 1) * 8));
+    CK(cudaMalloc((void**)&dids, std::max<int64_t>(cap, 1) * 4));
+    CK(cudaMemcpyAsync(doff, offsets, (n + 1) * 8, cudaMemcpyHostToDevice, st));
+    run(1, doff, dids, cap);
+    int64_t m = std::min<int64_t>(cap, *total);
+    cudaError_t e = cudaMemcpyAsync(ids, dids, m * 4, cudaMemcpyDeviceToHost, st);
+    cudaError_t e2 = cudaStreamSynchronize(st);
+    cudaFree(doff); cudaFree(dids);
+    if (e != cudaSuccess || e2 != cudaSuccess) {
+      c->err = cudaGetErrorString(e != cudaSuccess ? e : e2);
+      rc = SPH_ECUDA;
+    }
+  }
+  cudaFree(dcnt);
+  return rc;
+}
+
+int sph_debug_fma_peak(double* tflops_host, void* stream) {
+  if (!tflops_host) return SPH_EINVAL;
+  *tflops_host = 0.0;
+  cudaStream_t st = (cudaStream_t)stream;
+  int dev = 0, nsm = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+    return SPH_ECUDA;
+  float* d = nullptr;
+  if (cudaMalloc((void**)&d, 4) != cudaSuccess) return SPH_ENOMEM;
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  const int blocks = nsm * 8, iters = 4096;   // 8 blocks of 256 threads per SM: 2048 resident threads
+  double best = 0.0;
+  for (int rep = 0; rep < 6; ++rep) {  // the first repetitions warm the clocks up; best of the rest
+    cudaEventRecord(e0, st);
+    k_fma_peak<<<blocks, 256, 0, st>>>(d, iters, 0.999f, 0.001f);
+    cudaEventRecord(e1, st);
+    if (cudaEventSynchronize(e1) != cudaSuccess) { cudaFree(d); return SPH_ECUDA; }
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    const double flop = (double)blocks * 256.0 * (double)iters * 64.0 * 2.0;
+    if (rep >= 2 && ms > 0.f) best = std::max(best, flop / (ms * 1e-3) / 1e12);
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  cudaFree(d);
+  *tflops_host = best;
   return SPH_OK;
 }
 

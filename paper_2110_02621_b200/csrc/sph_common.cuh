@@ -20,6 +20,7 @@ struct DP {
   float rc2;       // (2h)^2, contract neighbour test on float32 images (reading A24)
   float rc2m;      // candidate filter threshold on the centred images: rc2 + rounding margin
   int exact_filter;  // 1: margin too large for the expanded form, use the difference form
+  int subq;          // 1: sigma from separations that include the 10-bit residuals (k_pass_a<.., SUBQ>)
   float inv_h;       // float16 filter of k_build: coordinates in units of h
   unsigned thr_h2;   // its threshold on r^2 / h^2 (half2, both halves): 4.08 + the float32 image margin
   float qh;        // Q / h: q = r_Q * qh

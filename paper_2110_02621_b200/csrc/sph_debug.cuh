@@ -261,3 +261,45 @@ __global__ void k_dbg_ranges(int ncell, const int* __restrict__ lb, int* cs, int
   cs[c] = s;
   ce[c] = e;
 }
+
+// sph_debug_step_lists: the neighbour lists the pair passes and the second wall pass actually READ
+// (NL / NLW per fluid particle, NLF per wall particle), mapped to caller ids, for a host-side check
+// against the oracle's float32 contract.  mode 0: cnt[caller id] = entries; mode 1: ids at off[caller id]
+// (order of the lists: not sorted; the self entry of a fluid row is included).
+__global__ void __launch_bounds__(256)
+k_list_export(int n, int mode, const unsigned* __restrict__ IDrow,
+              const uint4* __restrict__ L1, const int* __restrict__ C1, int cap1, const unsigned* __restrict__ ID1,
+              const uint4* __restrict__ L2, const int* __restrict__ C2, int cap2, const unsigned* __restrict__ ID2,
+              int* __restrict__ cnt, const long long* __restrict__ off, int* __restrict__ ids, long long cap) {
+  const int s = blockIdx.x * 256 + threadIdx.x;
+  if (s >= n) return;
+  const unsigned me = IDrow[s];
+  const int n1 = C1[s], n2 = L2 ? C2[s] : 0;
+  if (!mode) { cnt[me] = n1 + n2; return; }
+  long long o = off[me];
+  const unsigned* c1 = reinterpret_cast<const unsigned*>(L1 + (size_t)(s >> 5) * (cap1 >> 2) * 32 + (s & 31));
+  for (int k = 0; k < n1; ++k, ++o)
+    if (o < cap) ids[o] = (int)ID1[c1[(size_t)(k >> 2) * 128 + (k & 3)]];
+  if (n2) {
+    const unsigned* c2 = reinterpret_cast<const unsigned*>(L2 + (size_t)(s >> 5) * (cap2 >> 2) * 32 + (s & 31));
+    for (int k = 0; k < n2; ++k, ++o)
+      if (o < cap) ids[o] = (int)ID2[c2[(size_t)(k >> 2) * 128 + (k & 3)]];
+  }
+}
+
+// sph_debug_fma_peak: register-resident FP32 FMA loop (8 independent chains per thread, no memory
+// traffic): the measured non-tensor FP32 peak that bench.py uses as the roofline denominator.
+__global__ void __launch_bounds__(256)
+k_fma_peak(float* __restrict__ out, int iters, float a, float b) {
+  float x0 = threadIdx.x, x1 = x0 + 1.f, x2 = x0 + 2.f, x3 = x0 + 3.f, x4 = x0 + 4.f, x5 = x0 + 5.f, x6 = x0 + 6.f, x7 = x0 + 7.f;
+#pragma unroll 1
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      x0 = fmaf(x0, a, b); x1 = fmaf(x1, a, b); x2 = fmaf(x2, a, b); x3 = fmaf(x3, a, b);
+      x4 = fmaf(x4, a, b); x5 = fmaf(x5, a, b); x6 = fmaf(x6, a, b); x7 = fmaf(x7, a, b);
+    }
+  }
+  const float s = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+  if (s == 12345.678f) out[0] = s;  // keeps the chains alive without a store in the common case
+}

@@ -212,7 +212,7 @@ __device__ __forceinline__ void walk_f(const DP& p, const float4* __restrict__ A
     if (++ry > 1) { ry = -1; ++rz; }
     const int smin = STAGE ? __reduce_min_sync(FULL, s) : 0, emax = STAGE ? __reduce_max_sync(FULL, e) : 0;
     bool staged = false;
-    if constexpr (STAGE) if (emax - smin <= TW) {  // warp-uniform; emax <= smin when no lane has a candidate in this row
+    if constexpr (STAGE) if (emax > smin && emax - smin <= TW) {  // warp-uniform; a row in which no lane has a candidate (emax <= smin) skips the tile
       const int t0 = smin, n = emax - smin;
       bool bad = hc.bad;
       __syncwarp();
@@ -515,13 +515,16 @@ k_wall(const DP p, SS* __restrict__ S, const int nw, const float4* __restrict__ 
   }
   if (!act) cnt = 0;
   float sW = 0, sp = 0, sWr = 0, srx = 0, sry = 0, srz = 0, svx = 0, svy = 0, svz = 0;
+  // multi-phase form of Eq. 2.12 (every fluid term divided by rho_f) unless the run asks for the
+  // wall model of Adami et al. (2012) without the paper's extensions (NEXT-4 ablation)
+  const bool mw = MULTI && !(p.flags & SPH_FLAG_WALL_ADAMI_ONLY);
   {
     auto body = make_body(R, [&](const uint4& xj, const float4& bj, const unsigned j) {
     const Geo g = geometry<DIM>(p, xi, xj);  // r_wf = r_w - r_f
     const int ph = MULTI ? phase_of(xj) : 0;
     const float rhof = p.rho0[ph] + bj.w, pf = p.c2[ph] * bj.w;
     sW += g.w;
-    if (MULTI) {
+    if (MULTI && mw) {
       const float ir = div_fast(g.w, rhof);
       sp = fmaf(pf, ir, sp);
       sWr += ir;
@@ -539,7 +542,7 @@ k_wall(const DP p, SS* __restrict__ S, const int nw, const float4* __restrict__ 
   float pwall = 0.f, vx = S->vwall[0], vy = S->vwall[1], vz = S->vwall[2];  // reading A7: v_w = v_wall
   if (sW > 0.f) {
     const float lever = p.Qf * (S->gw[0] * srx + S->gw[1] * sry + S->gw[2] * srz);  // (g - a_w) . sum
-    pwall = (sp + lever) / (MULTI ? sWr : sW);
+    pwall = (sp + lever) / (mw ? sWr : sW);
     if (WITH_VEL && (p.flags & SPH_FLAG_WALL_VEL_MIRROR)) {
       const float is = 1.0f / sW;  // reading A6: v_w = 2 v_wall - <v_f>
       vx = fmaf(2.0f, vx, -svx * is); vy = fmaf(2.0f, vy, -svy * is); vz = fmaf(2.0f, vz, -svz * is);
@@ -556,7 +559,10 @@ k_wall(const DP p, SS* __restrict__ S, const int nw, const float4* __restrict__ 
 // The self pair is a candidate like any other: it adds W(0) to sigma (reading A14) and, with
 // r = 0 and v_ij = 0, nothing to the continuity sum.
 // ------------------------------------------------------------------------------------------
-template <int DIM, bool MULTI, bool EXACT>
+// SUBQ: sigma_i from separations that include the 10-bit residuals of the master positions (units of
+// Q/1024): every multi-phase run, and single-phase runs whose quantum is coarse for their size (sph.cu:
+// DP::subq; the 1e-4 bar on a needs sigma to about 1e-6 h / H relative).
+template <int DIM, bool MULTI, bool SUBQ>
 __global__ void __launch_bounds__(PB, SPH_MINB)
 k_pass_a(const DP p, const SS* __restrict__ S, const int nf, const int init,
          const float4* __restrict__ A, const XB* __restrict__ R,
@@ -577,10 +583,13 @@ k_pass_a(const DP p, const SS* __restrict__ S, const int nf, const int init,
   const float rhoi = rho0i + bi.w, prsi = c2i * bi.w, ZL = rhoi * ci;
   double sig = 0.0;  // sum of W/alpha in float64 (DESIGN.md §4 "precision")
   float acc = 0.f;
+  // reading A13b: the number density of a free-surface (heavy) phase particle of a multi-phase
+  // run counts its own phase and the walls only; an internal-flow (light) phase particle counts every neighbour
+  const bool sig_all = !MULTI || !((p.fs_mask >> phi) & 1u);
   {
     auto body = make_body(R, [&](const uint4& xj, const float4& bj, const unsigned j) {
     const Geo g = geometry<DIM>(p, xi, xj);
-    sig += w64<DIM, MULTI>(p, xi, xj, g);
+    if (!MULTI || sig_all || phase_of(xj) == phi) sig += w64<DIM, SUBQ>(p, xi, xj, g);
     const float vd = fmaf(bi.z - bj.z, g.dz, fmaf(bi.y - bj.y, g.dy, (bi.x - bj.x) * g.dx));
     if (!MULTI) {
       // equal c: (U* - U_L)(Z_L + Z_R) = c (rho_j v_ij.e + c (rho_i - rho_j)) with p = c^2 (rho - rho0)
@@ -602,7 +611,7 @@ k_pass_a(const DP p, const SS* __restrict__ S, const int nf, const int init,
     {
       auto body = make_body(WR, [&](const uint4& xj, const float4& bj, const unsigned j) {  // (v_w, p_w)
       const Geo g = geometry<DIM>(p, xi, xj);
-      sig += w64<DIM, MULTI>(p, xi, xj, g);
+      sig += w64<DIM, SUBQ>(p, xi, xj, g);
       const float rhow = fmaf(bj.w, p.inv_c2[phi], rho0i);  // reading A5
       const float ZR = rhow * ci;
       const float vd = fmaf(bi.z - bj.z, g.dz, fmaf(bi.y - bj.y, g.dy, (bi.x - bj.x) * g.dx));

@@ -42,7 +42,7 @@ def _base(dim, dp, rho0, c0, g, lo, hi, **kw):
     cfg = dict(dim=dim, n_phases=len(rho0), dp=float(dp), h=1.3 * float(dp),
                rho0=[float(x) for x in rho0], c0=[float(x) for x in c0],
                g=[float(x) for x in g], g_osc_amp=[0.0, 0.0, 0.0], g_osc_period=0.0,
-               cfl=0.25, penalty_strength=1.0, penalty_phase_mask=1, free_surface_mask=1,
+               cfl=0.25, penalty_strength=1.0, penalty_phase_mask=0, free_surface_mask=1,
                flags=FLAG_REINIT | FLAG_WALL_VEL_MIRROR,
                domain_min=[float(x) for x in lo] + [0.0] * (3 - dim),
                domain_max=[float(x) for x in hi] + [0.0] * (3 - dim))
@@ -131,6 +131,34 @@ def two_phase_2d(dp=0.0125, tank=(5.366, 3.0), column=(2.0, 1.0), equal_c=False)
     return _finish(cfg, pos, tag, rho, pos_w)
 
 
+def hydrostatic_tank_x1(dp=0.01, L=1.0, H=0.5, c_rule="baseline"):
+    """The paper's two-phase hydrostatic tank, case X1 (section 4.1): 2-D tank of
+    length L = 2H = 1 m and height L, lower half water, upper half air (density ratio 1000), both at
+    rest on a Cartesian lattice, same speed of sound in both phases.  The paper's
+    spacings are dx = 0.01, 0.005, 0.0025, 0.00125 m.  c_rule: "baseline" = 10 sqrt(2 g H) (BASELINE.json,
+    reading A2), "paper" = 10 * 2 sqrt(g H).  Initial density hydrostatic in both phases."""
+    cfg = two_phase_2d(dp=dp, tank=(L, L), column=(L, H), equal_c=True)
+    cfg["name"] = "x1_hydrostatic_tank_dp%g" % dp
+    if c_rule == "paper":
+        c = 20.0 * math.sqrt(G0 * H)
+        pos, tag = cfg["pos"].astype(np.float64), cfg["tag"]
+        top = cfg["domain_max"][1] - NWALL * dp
+        p = np.where(tag == 0, G0 * (top - H) + 1000.0 * G0 * (H - pos[:, 1]), G0 * (top - pos[:, 1]))
+        rho = np.where(tag == 0, 1000.0, 1.0) + p / c ** 2
+        cfg["rho"] = np.where(tag < 0, 1000.0, rho).astype(np.float32)
+        cfg["c0"] = [c, c]
+    cfg["top"] = cfg["domain_max"][1] - NWALL * dp
+    return cfg
+
+
+def x1_analytic_pressure(cfg, y):
+    """Hydrostatic pressure of case X1 at height y (Fig. 4): p = rho_a g (top - y) above the
+    interface, + (rho_w - rho_a) g (H - y) below it (p = 0 at the lid, as the linear EOS has it)."""
+    y = np.asarray(y, np.float64)
+    ra, rw = cfg["rho0"][1], cfg["rho0"][0]
+    return ra * G0 * (cfg["top"] - y) + (rw - ra) * G0 * np.maximum(cfg["H"] - y, 0.0)
+
+
 def sloshing_spheres_3d(dp=0.004, tank=(2.0, 1.0, 1.0), fill=0.4, n_spheres=8, seed=211002621):
     """Config 3: 3-D sloshing box with spherical obstacles; walls = 3-layer band of the
     signed distance to union(tank walls, spheres); gravity tilted sinusoidally."""
@@ -194,7 +222,7 @@ def box_2d(n=24, dp=0.01, jitter=0.0, seed=7, two_phase=False):
     rho0 = [1000.0, 1.0] if two_phase else [1000.0]
     cfg = _base(2, dp, rho0, [c0] * len(rho0), [0.0, -G0, 0.0], [-NWALL * dp] * 2,
                 [H + NWALL * dp] * 2, name="box2d_%d" % n, H=H,
-                penalty_phase_mask=2 if two_phase else 1)
+                penalty_phase_mask=2 if two_phase else 0)
     rng = np.random.Generator(np.random.PCG64(seed))
     pos_f = _lattice((n, n), dp)
     pos_f = pos_f + rng.uniform(-jitter * dp, jitter * dp, pos_f.shape)

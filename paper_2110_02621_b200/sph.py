@@ -14,6 +14,7 @@ TAG_WALL = -1
 FLAG_REINIT = 1
 FLAG_WALL_VEL_MIRROR = 2
 FLAG_NO_GRAPH = 4
+FLAG_WALL_ADAMI_ONLY = 8
 STAGES = ("predict", "sort", "reorder", "wall", "pass_a", "pass_b", "build")
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -50,7 +51,7 @@ EXPORTS = (
     "sph_create", "sph_destroy", "sph_set_particles", "sph_set_particles_host", "sph_step",
     "sph_step_dt", "sph_get_fields", "sph_get_fields_host", "sph_get_stats", "sph_get_stats_ex", "sph_set_profiling",
     "sph_get_timings", "sph_num_cells", "sph_debug_cells", "sph_debug_neighbours", "sph_debug_list_check", "sph_probe_pressure", "sph_probe_gauge",
-    "sph_debug_normals", "sph_debug_sigma", "sph_launch_count", "sph_last_error",
+    "sph_debug_normals", "sph_debug_sigma", "sph_launch_count", "sph_last_error", "sph_debug_step_lists", "sph_debug_fma_peak",
 )
 
 _lib = None
@@ -81,6 +82,8 @@ def load():
     L.sph_num_cells.restype = i64; L.sph_num_cells.argtypes = [vp]
     L.sph_debug_cells.restype = C.c_int; L.sph_debug_cells.argtypes = [vp] * 6
     L.sph_debug_neighbours.restype = C.c_int; L.sph_debug_neighbours.argtypes = [vp, vp, vp, i64, vp, vp]
+    L.sph_debug_step_lists.restype = C.c_int; L.sph_debug_step_lists.argtypes = [vp, vp, vp, i64, vp, vp]
+    L.sph_debug_fma_peak.restype = C.c_int; L.sph_debug_fma_peak.argtypes = [vp, vp]
     L.sph_debug_normals.restype = C.c_int; L.sph_debug_normals.argtypes = [vp, vp, vp]
     L.sph_debug_list_check.restype = C.c_int; L.sph_debug_list_check.argtypes = [vp, vp, vp]
     L.sph_probe_pressure.restype = C.c_int; L.sph_probe_pressure.argtypes = [vp, C.c_int32, vp, vp, vp, vp]
@@ -240,6 +243,15 @@ class Sph:
         self._ck(self.L.sph_debug_neighbours(self.ctx, _hp(off), _hp(ids), tot.value, C.byref(tot), self._st()))
         return off, ids[:tot.value]
 
+    def debug_step_lists(self):
+        """The lists the passes read (caller ids, list order, self and filter extras included)."""
+        off = np.zeros(self.n + 1, np.int64)
+        tot = C.c_int64(0)
+        self._ck(self.L.sph_debug_step_lists(self.ctx, _hp(off), None, 0, C.byref(tot), self._st()))
+        ids = np.zeros(max(tot.value, 1), np.int32)
+        self._ck(self.L.sph_debug_step_lists(self.ctx, _hp(off), _hp(ids), tot.value, C.byref(tot), self._st()))
+        return off, ids[:tot.value]
+
     def probe_pressure(self, points):
         """Shepard-averaged fluid pressure at points (m,3) -> (p (m,), wsum (m,)); reading A29."""
         pts = np.ascontiguousarray(points, np.float32).reshape(-1, 3)
@@ -269,3 +281,15 @@ class Sph:
         buf = np.zeros(2 * max(self.n, 1), np.float32)
         self._ck(self.L.sph_debug_sigma(self.ctx, _hp(buf), self._st()))
         return buf[:self.n].copy(), buf[self.n:2 * self.n].copy()
+
+
+def fma_peak_tflops(stream=None):
+    """sph_debug_fma_peak: measured non-tensor FP32 peak of the current device in TFLOP/s."""
+    import torch
+    L = load()
+    out = C.c_double(0.0)
+    st = stream if stream is not None else torch.cuda.current_stream()
+    rc = L.sph_debug_fma_peak(C.byref(out), C.c_void_p(st.cuda_stream))
+    if rc != 0:
+        raise SphError("sph_debug_fma_peak failed with code %d" % rc)
+    return out.value

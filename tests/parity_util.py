@@ -21,18 +21,20 @@ def make_pair(cfg):
 
 
 def scales(cfg):
-    """Field scales S of reading A26: rho -> rho0 of the particle's phase, p -> rho0[0] |g| H,
-    a -> |g| rho0[0] / rho0[phase] (or that with |g| = 1 if g = 0), v -> sqrt(|g| H).
-    The acceleration scale is a force-density scale: a float32 pair term of a phase-k particle is
-    of size p / (rho0[k] h), so its rounding alone is 1e-7 rho0[0] g H / (rho0[k] h); for air next
-    to water (rho ratio 1000, H / h = 60) that is 6e-3 g: the bar 1e-4 is applied to
-    rho0[k] a / rho0[0], which for a single phase is a / |g| as before (A26)."""
+    """Field scales S of reading A26: rho -> rho0 of the particle's phase,
+    p -> rho0[0] |g| H, a -> |g| (1 if g = 0) for EVERY phase, v -> sqrt(|g| H), x -> H."""
     gm = float(np.linalg.norm(cfg["g"])) or 1.0
     H = float(cfg.get("H", 1.0))
     tag = cfg["tag"]
     rho0 = np.asarray(cfg["rho0"], np.float64)
     rs = np.where(tag >= 0, rho0[np.clip(tag, 0, None)], rho0[0])
-    return dict(rho=rs, p=rho0[0] * gm * H, acc=gm * rho0[0] / rs, vel=np.sqrt(gm * H), pos=H)
+    return dict(rho=rs, p=rho0[0] * gm * H, acc=gm, vel=np.sqrt(gm * H), pos=H)
+
+
+def acc_err_by_phase(cfg, o, g):
+    """max |a_gpu - f32(a_ref)| / max(|a_ref|, |g|) per fluid phase (reported by the two-phase tests)."""
+    fo, fg = o.fields(), g.get_fields(device=False, which=("acc",))
+    return {ph: rel_err(cfg, "acc", fg["acc"], fo["acc"], cfg["tag"] == ph) for ph in range(cfg["n_phases"])}
 
 
 def rel_err(cfg, name, x_gpu, x_ref, mask=None):

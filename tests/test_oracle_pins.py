@@ -606,3 +606,117 @@ def test_P22_fluid_moving_with_the_walls_feels_no_wall_motion():
     # with the walls at rest the same moving fluid is compressed against them (the pin is not vacuous)
     d2, _ = rates(dict(cfg0, vel=vel))
     assert np.max(np.abs(d2[fl] - d0[fl])) > 1e-2 * sd
+
+
+# ------------------------------------------------------------------ P23-P25: what round 1 left unpinned
+def _two_phase_lattice(n=24, dp=1.0 / 64, rho_w=1005.0, rho_a=1.3, **kw):
+    """Unperturbed two-phase box (water below y = H/2, air above), every particle given one
+    off-reference density per phase so that each formula leaves a distinct value."""
+    cfg = dict(inputs.box_2d(n=n, dp=dp, jitter=0.0, two_phase=True))
+    rho = np.where(cfg["tag"] == 0, rho_w, np.where(cfg["tag"] == 1, rho_a, 1000.0)).astype(np.float32)
+    cfg["rho"] = rho
+    cfg["g"] = [0.0, 0.0, 0.0]
+    cfg.update(kw)
+    return cfg
+
+
+def test_P23_two_phase_step_dispatch_reinit_and_density_update():
+    """Readings A13 / A13b / A15 inside orc.step (the dispatch, not the kernel): one step with dt = 0 on
+    the unperturbed two-phase lattice leaves the positions alone, so every density follows by hand from
+    the lattice constants of pin P2 (tests/golden/lattice_constants.txt, computed outside oracle/):
+      water, bulk          sigma (own phase + walls) = sigma0          -> Eq. 2.17 with rho_s = rho0 < rho*:
+                           rho = rho0 + (rho* - rho0) rho0 / rho*      (continuity adds dt * drho = 0)
+      water, interface row sigma = half-space sum (own row and below)  -> rho_s = rho0 * halfspace / sigma0
+      air (any)            sigma over every neighbour = sigma0         -> Eq. 2.4 / 2.18: rho = rho0_air,
+                           whatever rho* was (summation overwrites)
+    A wrong phase in either dispatch, the light phase counted in the water's sigma, or Eq. 2.18 on the water
+    changes one of these values by >= 0.5 %."""
+    gold = _gold("lattice_constants.txt")
+    n, dp = 24, 1.0 / 64
+    rw, ra = 1005.0, 1.3
+    cfg = _two_phase_lattice(n, dp, rw, ra)
+    o = run(cfg)
+    o.step(1, dts=[0.0])
+    f = o.fields()
+    y = cfg["pos"][:, 1].astype(np.float64)
+    tag = cfg["tag"]
+    H = n * dp
+    water, air = tag == 0, tag == 1
+    x = cfg["pos"][:, 0].astype(np.float64)
+    # interface row away from the side walls (the wall particles above the interface still count for a water particle)
+    top_row = water & (np.abs(y - (0.5 * H - 0.5 * dp)) < 1e-6) & (x > 3 * dp) & (x < H - 3 * dp)
+    bulk = water & (y < 0.5 * H - 3 * dp)
+    assert top_row.sum() == n - 6 and bulk.sum() == n * (n // 2 - 3)
+    want_bulk = 1000.0 + (rw - 1000.0) * 1000.0 / rw
+    assert np.max(np.abs(f["rho"][bulk] - want_bulk)) < 1e-6
+    rs = 1000.0 * gold["halfspace_2d"] / gold["sigma0_2d"]
+    want_top = rs + (rw - rs) * 1000.0 / rw
+    assert np.max(np.abs(f["rho"][top_row] - want_top)) < 1e-4     # golden constants carry 9 digits
+    assert np.max(np.abs(f["rho"][air] - 1.0)) < 2e-9              # sigma0 is a 20-neighbour sum
+    # Eq. 2.3 with each phase's own rho0 (c equal here)
+    c2 = cfg["c0"][0] ** 2
+    assert np.max(np.abs(f["p"][bulk] - c2 * (want_bulk - 1000.0))) < 1e-6 * c2
+    assert np.max(np.abs(f["p"][air])) < 1e-8 * c2
+    # the study-only variants really are the other readings (they must NOT reproduce the values above)
+    o2 = run(dict(cfg, oracle_variant=orc.VAR_SIGMA_ALL))
+    o2.step(1, dts=[0.0])
+    assert np.max(np.abs(o2.fields()["rho"][top_row] - want_bulk)) < 1e-6      # air counted: no deficiency
+    o3 = run(dict(cfg, oracle_variant=orc.VAR_SUM_RAW))
+    o3.step(1, dts=[0.0])
+    assert np.max(np.abs(o3.fields()["rho"][air] - gold["sigma0_2d"])) < 2e-9  # Eq. 2.4 raw: m sigma = rho0 V0 sigma0
+    o4 = run(dict(cfg, oracle_variant=orc.VAR_REINIT_LITERAL))
+    o4.step(1, dts=[0.0])
+    assert np.max(np.abs(o4.fields()["rho"][bulk] - 1000.0)) < 1e-6            # Eq. 2.18 on the water
+
+
+def test_P24_stats_kinetic_energy_and_front_closed_form():
+    """orc.stats: E_k = 1/2 M |v|^2 for a uniformly moving block, mass = N rho0 dp^d, x_front = the
+    largest x of the phase-0 particles within 3 dp of the floor: all closed forms of the generator's
+    lattice (config 0: column 20 x 40 sites of dp = 0.05 from the corner, PAPER.md:244 for the energy
+    definition)."""
+    cfg = dict(inputs.dam_break_2d())
+    v = np.array([0.3, -0.4, 0.0], np.float32)
+    vel = np.zeros_like(cfg["pos"])
+    vel[cfg["tag"] >= 0] = v
+    cfg["vel"] = vel
+    o = run(cfg)
+    s = o.stats()
+    nf, dp = cfg["n_fluid"], cfg["dp"]
+    M = nf * 1000.0 * dp * dp
+    assert nf == 800 and abs(s["mass"] - M) < 1e-9 * M
+    v64 = v.astype(np.float64)
+    assert abs(s["ek"] - 0.5 * M * float(v64 @ v64)) < 1e-12 * M
+    assert abs(s["x_front"] - (1.0 - 0.5 * dp)) < 1e-6          # float32 input positions
+    # a block that does not touch the floor band has no front
+    cfg2 = dict(inputs.dam_break_2d())
+    pos = cfg2["pos"].copy()
+    pos[cfg2["tag"] >= 0, 1] += 0.5
+    cfg2["pos"] = pos
+    assert run(cfg2).stats()["x_front"] < -1e100
+    # two phases: only phase 0 counts for the front, both for the energy
+    cfg3 = _two_phase_lattice(24, 1.0 / 64, 1000.0, 1.0)
+    vel3 = np.zeros_like(cfg3["pos"]); vel3[cfg3["tag"] >= 0] = (0.0, 2.0, 0.0)
+    cfg3["vel"] = vel3
+    s3 = run(cfg3).stats()
+    n = 24
+    M3 = (n * n // 2) * (1000.0 + 1.0) * (1.0 / 64) ** 2
+    assert abs(s3["ek"] - 0.5 * M3 * 4.0) < 1e-12 * M3 and abs(s3["mass"] - M3) < 1e-12 * M3
+    assert abs(s3["x_front"] - (n - 0.5) / 64.0) < 1e-6
+
+
+@pytest.mark.parametrize("dim", [2, 3])
+def test_P25_sigma_of_the_continuity_pass_on_the_lattice(dim):
+    """pass_continuity's own sigma (the one the reinitialisation of the next step reads) equals the
+    lattice constant of pin P2 for every particle of a closed, unperturbed single-phase box after a
+    step (dt = 0 keeps the lattice): sigma dp^d = 1.010473152 / 1.009500784, walls included."""
+    gold = _gold("lattice_constants.txt")
+    dp = 1.0 / 64
+    cfg = dict(inputs.box_2d(n=12, dp=dp)) if dim == 2 else dict(inputs.box_sweep_3d(n=9, dp=dp, jitter=0.0))
+    cfg["g"] = [0.0, 0.0, 0.0]
+    cfg["rho"] = np.full_like(cfg["rho"], 1000.0)
+    o = run(cfg)
+    o.step(1, dts=[0.0])
+    f = o.fields()
+    fl = cfg["tag"] >= 0
+    assert np.max(np.abs(f["sigma"][fl] * dp ** dim - gold["sigma0_%dd" % dim])) < 2e-9
+    assert np.max(np.abs(f["drho"][fl])) < 1e-6     # at rest with uniform rho and p: Eq. 2.9 gives 0
