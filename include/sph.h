@@ -85,7 +85,13 @@ typedef struct {
   double wall_osc_amp[3];        /* NEXT-1: all walls translate rigidly, x_w(t) = x_w(0) + wall_osc_amp *   */
   double wall_osc_freq;          /* sin(2 pi wall_osc_freq t); a_w enters Eq. 2.12,
                                     v_wall the mirror of reading A6; 0 = static walls.  The wall cell list is
-                                    then rebuilt every step; the domain box must contain the whole excursion */
+                                    then rebuilt with the lists; the domain box must contain the whole excursion */
+  double list_skin;              /* Verlet skin s: the cell list and the per-particle neighbour lists are built with radius
+                                    2h(1 + s) (cell edge 2h(1 + s)) and kept over the following steps until a pair
+                                    further apart than that could have come within 2h, i.e. until 2 sum_n max_i |dx_i^n|
+                                    (or that of fluid + walls) exceeds 2 h s; entries beyond 2h add exactly 0.  0 = rebuild
+                                    every step; < 0 = library default (0.1); at most 0.5.  Results do not depend on s
+                                    beyond the order of floating-point sums */
 } sph_params;
 
 typedef struct {
@@ -100,17 +106,19 @@ typedef struct {
   double x_front;    /* max x over phase-0 particles within 3 dp of the floor (floor = domain_min[dim-1] + 3 dp) */
   int64_t escaped;   /* fluid particles outside [domain_min, domain_max) at the last cell build */
   int64_t nonfinite; /* non-finite positions/velocities seen so far     */
+  int64_t rebuilds;  /* cell-list / neighbour-list builds since sph_set_particles (its own included) */
 } sph_stats;
 
 /* Stages timed by sph_set_profiling (indices into sph_get_timings' array). */
 enum sph_stage {
   SPH_STAGE_PREDICT = 0,   /* dt reduction + reinit (Eq. 2.17/2.18) + half kick + drift (Eq. 2.19-2.20) + cell hash */
-  SPH_STAGE_SORT = 1,      /* device radix sort of (cell id, index) */
-  SPH_STAGE_REORDER = 2,   /* gather into sorted SoA float4 + cell ranges */
+  SPH_STAGE_SORT = 1,      /* device radix sort of (cell id, index); only on steps that rebuild the lists */
+  SPH_STAGE_REORDER = 2,   /* gather into sorted SoA float4 + cell ranges; only on steps that rebuild */
   SPH_STAGE_WALL = 3,      /* wall extrapolation Eq. 2.12 (both calls of a step) */
   SPH_STAGE_PASS_A = 4,    /* sigma + continuity Eq. 2.9 + density update Eq. 2.21 / 2.4 + EOS */
   SPH_STAGE_PASS_B = 5,    /* momentum Eq. 2.10/2.11 + penalty Eq. 2.13 + second kick Eq. 2.22 */
-  SPH_STAGE_BUILD = 6,     /* neighbour-list build: the 27 / 9-cell candidate walk, once per step */
+  SPH_STAGE_BUILD = 6,     /* neighbour-list build: the 27 / 9-cell candidate walks (fluid and wall rows), on the
+                              steps that rebuild (every step when list_skin = 0) */
   SPH_STAGE_COUNT = 7
 };
 
@@ -157,9 +165,11 @@ int sph_get_stats_ex(sph_ctx* ctx, sph_stats* out, int32_t with_pairs, void* str
 
 /* Per-stage device times.  With profiling on, sph_step brackets every stage with CUDA events
  * on the caller's stream; sph_get_timings synchronises and returns the accumulated milliseconds
- * per stage since the last call (ms_host[SPH_STAGE_COUNT]) and the number of steps they cover. */
+ * per stage since the last call (ms_host[SPH_STAGE_COUNT]) and the number of steps they cover.  With profiling
+ * on the steps are issued as plain launches and the host reads the rebuild decision once per step. */
 int sph_set_profiling(sph_ctx* ctx, int32_t on);
-int sph_get_timings(sph_ctx* ctx, float* ms_host, int32_t* n_steps_host);
+int sph_get_timings(sph_ctx* ctx, float* ms_host, int32_t* n_steps_host, int32_t* n_rebuilds_host /* may be NULL:
+                    how many of those steps rebuilt the lists */);
 
 /* Number of cells of the grid (cell edge 2h(1+2^-10), reading A24). */
 int64_t sph_num_cells(const sph_ctx* ctx);
@@ -207,6 +217,14 @@ int sph_debug_list_check(sph_ctx* ctx, int64_t* out3_host, void* stream);
  * with the oracle's float32 contract lists (superset, every extra entry within the documented margin). */
 int sph_debug_step_lists(sph_ctx* ctx, int64_t* offsets_host, int32_t* ids_host, int64_t cap,
                          int64_t* total_host, void* stream);
+
+/* BASELINE.json config 4 asks for the density-reinitialisation kernel and the integrator to be timed on their own;
+ * the step runs them fused with the cell hash in one predictor launch (note under the step
+ * table).  This call times, on scratch outputs (the state is not changed), ms_host[0] = the stand-alone reinitialisation
+ * kernel (Eq. 2.17 / 2.18 from the stored sigma_i), ms_host[1] = the stand-alone integrator (first kick Eq. 2.19, drift
+ * Eq. 2.20, cell hash), ms_host[2] = the fused predictor; each the mean of 5 launches after one warm-up launch.
+ * HOST pointer to 3 floats; synchronises. */
+int sph_debug_time_pointwise(sph_ctx* ctx, float* ms_host, void* stream);
 
 /* Measured non-tensor FP32 peak of the current device: a register-resident FMA loop (8 independent chains per
  * thread, 2048 threads per SM, no memory traffic), best of 4 timed launches after 2 warm-up launches, in

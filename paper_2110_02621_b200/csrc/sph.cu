@@ -72,7 +72,6 @@ struct sph_ctx {
   double* dt_seq = nullptr;
   int64_t dt_seq_cap = 0;
   StatAcc* stat = nullptr;
-  int sort_passes = 1, sort_bits = 8;
   // NEXT-1 (moving walls): wall positions and caller ids in set-up order, sort buffers of the per-step re-sort
   int moving = 0;
   uint4* WX0 = nullptr;
@@ -92,8 +91,20 @@ struct sph_ctx {
   int* hidx = nullptr;     // caller indices of one class during sph_set_particles
   // one step captured as a CUDA graph (launch-bound small configurations); rebuilt after sph_set_particles
   cudaGraphExec_t gexec = nullptr;
-  cudaStream_t cap_stream = nullptr;
-  int64_t graph_launches = 0;  // kernel launches inside the captured step
+  cudaStream_t cap_stream = nullptr, cap_stream2 = nullptr;
+  int64_t graph_launches = 0;  // kernel launches of a captured step that keeps its lists
+  int64_t body_launches = 0;   // ... of its rebuild branch
+  int64_t direct_rebuilds = 0;          // rebuild branches issued by plain launches (already in `launches`)
+  int64_t graph_rebuilds_counted = 0;   // rebuild branches taken inside graph replays already added to `launches`
+  int cell_bits = 1;           // significant bits of a cell id of the step's grid
+  DP dpC;                      // the contract grid of reading A24 (cell edge 2h(1 + 2^-10)); = dp's grid when skin = 0
+  int64_t ncellC = 0;
+  uint4* WXB = nullptr;        // moving walls with kept lists: set-up positions in the current wall order
+  // scratch of contract_view (debug entry points with skin > 0)
+  unsigned *dKa = nullptr, *dVa = nullptr, *dKb = nullptr, *dVb = nullptr, *dID = nullptr, *dWID = nullptr;
+  float4 *dG = nullptr, *dWG = nullptr;
+  int *dlbF = nullptr, *dlbW = nullptr;
+  bool ev_rebuilt[64] = {};
   // profiling
   bool prof = false;
   std::vector<cudaEvent_t> ev;
@@ -118,10 +129,11 @@ namespace {
     c->launches++;                                         \
   } while (0)
 
-// Pair kernels are instantiated for DIM in {2,3} x MULTI x EXACT (filter form).
-#define PAIR_SEL(c) (((c)->prm.dim == 3 ? 4 : 0) | ((c)->multi ? 2 : 0) | ((c)->dp.exact_filter ? 1 : 0))
-#define PAIR_DISPATCH(KERN, grid, st, ...)                                            \
-  switch (PAIR_SEL(c)) {                                                              \
+// Pair kernels are instantiated for DIM in {2,3} x MULTI x a third flag: EXACT (filter form) for the list
+// builds, SUBQ (residuals in sigma) for pass A; pass B and the wall passes ignore it.
+#define SEL3(c, third) (((c)->prm.dim == 3 ? 4 : 0) | ((c)->multi ? 2 : 0) | ((third) ? 1 : 0))
+#define PAIR_DISPATCH(KERN, sel, grid, st, ...)                                       \
+  switch (sel) {                                                                      \
     case 0: LAUNCH((KERN<2, false, false>), grid, PB, st, __VA_ARGS__); break;        \
     case 1: LAUNCH((KERN<2, false, true>), grid, PB, st, __VA_ARGS__); break;         \
     case 2: LAUNCH((KERN<2, true, false>), grid, PB, st, __VA_ARGS__); break;         \
@@ -131,16 +143,13 @@ namespace {
     case 6: LAUNCH((KERN<3, true, false>), grid, PB, st, __VA_ARGS__); break;         \
     default: LAUNCH((KERN<3, true, true>), grid, PB, st, __VA_ARGS__); break;         \
   }
-#define WALL_DISPATCH(VEL, grid, st, ...)                                             \
-  switch (PAIR_SEL(c)) {                                                              \
-    case 0: LAUNCH((k_wall<2, false, false, VEL>), grid, PB, st, __VA_ARGS__); break; \
-    case 1: LAUNCH((k_wall<2, false, true, VEL>), grid, PB, st, __VA_ARGS__); break;  \
-    case 2: LAUNCH((k_wall<2, true, false, VEL>), grid, PB, st, __VA_ARGS__); break;  \
-    case 3: LAUNCH((k_wall<2, true, true, VEL>), grid, PB, st, __VA_ARGS__); break;   \
-    case 4: LAUNCH((k_wall<3, false, false, VEL>), grid, PB, st, __VA_ARGS__); break; \
-    case 5: LAUNCH((k_wall<3, false, true, VEL>), grid, PB, st, __VA_ARGS__); break;  \
-    case 6: LAUNCH((k_wall<3, true, false, VEL>), grid, PB, st, __VA_ARGS__); break;  \
-    default: LAUNCH((k_wall<3, true, true, VEL>), grid, PB, st, __VA_ARGS__); break;  \
+// list builds: DIM x EXACT
+#define BUILD_DISPATCH(KERN, grid, st, ...)                                           \
+  switch (((c)->prm.dim == 3 ? 2 : 0) | ((c)->dp.exact_filter ? 1 : 0)) {             \
+    case 0: LAUNCH((KERN<2, false>), grid, PB, st, __VA_ARGS__); break;               \
+    case 1: LAUNCH((KERN<2, true>), grid, PB, st, __VA_ARGS__); break;                \
+    case 2: LAUNCH((KERN<3, false>), grid, PB, st, __VA_ARGS__); break;               \
+    default: LAUNCH((KERN<3, true>), grid, PB, st, __VA_ARGS__); break;               \
   }
 
 inline int cdiv(int64_t a, int64_t b) { return (int)((a + b - 1) / b); }
@@ -165,34 +174,48 @@ void free_all(sph_ctx* c) {
                   c->keyA, c->valA, c->keyB, c->valB, c->hist, c->rowsum, c->lbF, c->lbW, c->WR,
                   c->WA, c->WN, c->WG, c->WK, c->WID, c->wnear, c->S, c->dt_seq, c->stat,
                   c->hpos, c->hvel, c->hrho, c->htagd, c->hout, c->hidx,
-                  c->WX0, c->WN0, c->WID0, c->WkeyA, c->WkeyB, c->WvalA, c->WvalB,
+                  c->WX0, c->WXB, c->WN0, c->WID0, c->dKa, c->dVa, c->dKb, c->dVb, c->dID, c->dWID, c->dG, c->dWG, c->dlbF, c->dlbW, c->WkeyA, c->WkeyB, c->WvalA, c->WvalB,
                   c->WTX, c->WTB, c->Whist, c->Wrowsum};
   for (void* p : ptrs)
     if (p) cudaFree(p);
   for (auto e : c->ev) cudaEventDestroy(e);
   if (c->gexec) cudaGraphExecDestroy(c->gexec);
   if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
+  if (c->cap_stream2) cudaStreamDestroy(c->cap_stream2);
   if (c->evFork) cudaEventDestroy(c->evFork);
   if (c->evJoin) cudaEventDestroy(c->evJoin);
   if (c->wstream) cudaStreamDestroy(c->wstream);
 }
 
-// Stable radix sort of (keys, vals); result pointers returned in *ko, *vo.
-int radix_sort(sph_ctx* c, cudaStream_t st, int n, unsigned* kA, unsigned* vA, unsigned* kB, unsigned* vB,
+// Digits of 9 bits when that saves a pass over 8-bit digits (sph_sort.cuh).
+inline void radix_plan(int bits, int* digit_bits, int* passes) {
+  *digit_bits = (bits + 8) / 9 < (bits + 7) / 8 ? 9 : 8;
+  *passes = (bits + *digit_bits - 1) / *digit_bits;
+}
+inline int bits_for(int64_t count) {
+  int bits = 1;
+  while ((1ll << bits) < count) ++bits;
+  return bits;
+}
+
+// Stable radix sort of (keys, vals) on keys of `bits` significant bits; result pointers returned in *ko, *vo.
+int radix_sort(sph_ctx* c, cudaStream_t st, int n, int bits, unsigned* kA, unsigned* vA, unsigned* kB, unsigned* vB,
                unsigned** ko, unsigned** vo, unsigned* hist = nullptr, unsigned* rowsum = nullptr) {
   if (!hist) { hist = c->hist; rowsum = c->rowsum; }
   unsigned *ki = kA, *vi = vA, *kt = kB, *vt = vB;
+  int dbits, passes;
+  radix_plan(bits, &dbits, &passes);
   if (n > 0) {
     const int items = rs_items((size_t)n), nblk = cdiv(n, RS_THREADS * items);
-    for (int pass = 0; pass < c->sort_passes; ++pass) {
-      int shift = c->sort_bits * pass;
+    for (int pass = 0; pass < passes; ++pass) {
+      int shift = dbits * pass;
 #define RS_PASS(ND, IT)                                                                                   \
   do {                                                                                                    \
     LAUNCH((k_radix_hist<ND, IT>), nblk, RS_THREADS, st, ki, n, shift, hist, nblk, rowsum);               \
     LAUNCH(k_scan_apply, ND, 256, st, hist, nblk, rowsum);                                                \
     LAUNCH((k_radix_scatter<ND, IT>), nblk, RS_THREADS, st, ki, vi, n, shift, hist, nblk, kt, vt, rowsum); \
   } while (0)
-      if (c->sort_bits == 9) { if (items == 4) RS_PASS(512, 4); else RS_PASS(512, 16); }
+      if (dbits == 9) { if (items == 4) RS_PASS(512, 4); else RS_PASS(512, 16); }
       else { if (items == 4) RS_PASS(256, 4); else RS_PASS(256, 16); }
 #undef RS_PASS
       std::swap(ki, kt);
@@ -208,98 +231,196 @@ int radix_sort(sph_ctx* c, cudaStream_t st, int n, unsigned* kA, unsigned* vA, u
 struct Prof {
   sph_ctx* c;
   cudaStream_t st;
-  int slot = 0;
   bool on;
   Prof(sph_ctx* c_, cudaStream_t s) : c(c_), st(s) {
     on = c->prof && c->ev_steps < sph_ctx::EV_MAX_STEPS;
   }
-  void mark() {
+  // marks: 0 start, 1 predict, 2 sort, 3 reorder, 4 list build (wall + fluid), 5 wall 1, 6 pass A, 7 wall 2, 8 pass B
+  void mark(int slot) {
     if (!on) return;
-    cudaEventRecord(c->ev[c->ev_steps * sph_ctx::EV_PER_STEP + slot++], st);
+    cudaEventRecord(c->ev[c->ev_steps * sph_ctx::EV_PER_STEP + slot], st);
   }
-  void done() {
-    if (on) c->ev_steps++;
+  void done(bool rebuilt) {
+    if (!on) return;
+    c->ev_rebuilt[c->ev_steps] = rebuilt;
+    c->ev_steps++;
   }
 };
 
-// wall extrapolation launcher (B = the fluid (v, rho - rho0) array the pressures are read from)
+// Eq. 2.12 for every wall particle from its wall-fluid list (R = the fluid records the pressures are read from)
 void launch_wall(sph_ctx* c, cudaStream_t st, bool with_vel, const XB* R) {
   if (c->nw == 0 || c->nf == 0) return;
   const int grid = cdiv(c->nw, PB), nw = (int)c->nw;
   if (with_vel) {
-    WALL_DISPATCH(true, grid, st, c->dp, c->S, nw, c->WA, c->WR, c->WK, c->A, R, c->lbF, c->NLF, c->NCF, c->capsw);
+    PAIR_DISPATCH(k_wall, SEL3(c, 1), grid, st, c->dp, c->S, nw, c->WR, R, c->NLF, c->NCF, c->capsw);
   } else {
-    WALL_DISPATCH(false, grid, st, c->dp, c->S, nw, c->WA, c->WR, c->WK, c->A, R, c->lbF, c->NLF, c->NCF, c->capsw);
+    PAIR_DISPATCH(k_wall, SEL3(c, 0), grid, st, c->dp, c->S, nw, c->WR, R, c->NLF, c->NCF, c->capsw);
   }
 }
 
 // NEXT-1 (moving walls): the walls at their positions of t^{n+1}, re-sorted into the cell grid (the
 // same kernels as the set-up, on scratch of their own: `st` is the wall stream, which runs beside the
-// fluid's predict / sort / reorder).
+// fluid's sort / reorder inside the rebuild branch).
 int wall_rebuild(sph_ctx* c, cudaStream_t st) {
   const int nw = (int)c->nw;
   if (nw == 0) return SPH_OK;
   LAUNCH(k_wall_shift, cdiv(nw, 256), 256, st, c->dp, c->S, nw, c->WX0, c->WTX, c->WTB, c->WkeyA, c->WvalA);
   unsigned *ks, *vs;
-  int rc = radix_sort(c, st, nw, c->WkeyA, c->WvalA, c->WkeyB, c->WvalB, &ks, &vs, c->Whist, c->Wrowsum);
+  int rc = radix_sort(c, st, nw, c->cell_bits, c->WkeyA, c->WvalA, c->WkeyB, c->WvalB, &ks, &vs, c->Whist, c->Wrowsum);
   if (rc) return rc;
   // gather + wall cell lower bounds in one launch, as for the fluid
   LAUNCH(k_reorder, std::max(cdiv(nw, 256), cdiv(c->ncell + 1, 256)), 256, st, c->dp, nw, vs, c->WTX, c->WTB, c->WID0,
          c->WR, c->WA, c->WID, ks, (int)c->ncell, c->lbW);
   CK(cudaMemcpyAsync(c->WK, ks, sizeof(unsigned) * nw, cudaMemcpyDeviceToDevice, st));
-  LAUNCH(k_image, cdiv(nw, 256), 256, st, c->dp, nw, c->WR, c->WG);
   LAUNCH(k_gather4, cdiv(nw, 256), 256, st, nw, vs, c->WN0, c->WN);  // normals: translation-invariant
+  LAUNCH(k_gatherx, cdiv(nw, 256), 256, st, nw, vs, c->WX0, c->WXB); // set-up positions in the new order (k_wall_move)
   LAUNCH(k_wnear, cdiv(c->ncell, 256), 256, st, c->dp, (int)c->ncell, c->lbW, c->wnear);
   return SPH_OK;
 }
 
-// Everything after the drift: sort, reorder, cell ranges, wall pass, pass A, wall pass, pass B.
-int pipeline_after_hash(sph_ctx* c, cudaStream_t st, int init, Prof& pf) {
+// The rebuild branch of a step (and the set-up): radix sort of the cell keys, gather into cell order with the
+// cell bounds, wall re-sort (moving walls, on the wall stream beside the fluid's), wall-fluid lists, fluid lists.
+// Input: TX / TB (positions, (v, rho - rho0)) and keyA / valA in the current order; output: R0, A, IDcur, lbF,
+// NL / NLW / NLF in the new order.
+int rebuild_body(sph_ctx* c, cudaStream_t st, int init, Prof& pf) {
   const int nf = (int)c->nf;
+  const bool wall_branch = c->moving && !init && c->nw > 0;
+  if (wall_branch) {
+    CK(cudaEventRecord(c->evFork, st));
+    CK(cudaStreamWaitEvent(c->wstream, c->evFork, 0));
+    int rcw = wall_rebuild(c, c->wstream);
+    if (rcw) return rcw;
+    CK(cudaEventRecord(c->evJoin, c->wstream));
+  }
   unsigned *ks, *vs;
-  int rc = radix_sort(c, st, nf, c->keyA, c->valA, c->keyB, c->valB, &ks, &vs);
+  int rc = radix_sort(c, st, nf, c->cell_bits, c->keyA, c->valA, c->keyB, c->valB, &ks, &vs);
   if (rc) return rc;
   c->K = ks;
-  pf.mark();  // end sort
+  pf.mark(2);  // end sort
   if (nf > 0) {
-    // reorder + cell lower bounds in one launch; no pointer ping-pong: every step issues the same launches
-    // with the same arguments (CUDA graph), k_build copies IDnext back to IDcur
+    // no pointer ping-pong: every rebuild issues the same launches with the same arguments (CUDA graph);
+    // k_build copies IDnext back to IDcur
     LAUNCH(k_reorder, std::max(cdiv(nf, 256), cdiv(c->ncell + 1, 256)), 256, st, c->dp, nf, vs, c->TX, c->TB, c->IDcur,
            c->R0, c->A, c->IDnext, ks, (int)c->ncell, c->lbF);
   } else {
     LAUNCH(k_cell_bounds, cdiv(c->ncell + 1, 256), 256, st, ks, nf, (int)c->ncell, c->lbF);
   }
-  if (c->moving && !init && c->nw > 0) CK(cudaStreamWaitEvent(st, c->evJoin, 0));  // join the wall branch of one_step
-  pf.mark();  // end reorder
-  launch_wall(c, st, true, c->R0);
-  pf.mark();  // end wall 1
-  if (nf > 0) {
-    switch (PAIR_SEL(c) & 5) {  // DIM x EXACT
-      case 0: LAUNCH((k_build<2, false>), cdiv(nf, PB), PB, st, c->dp, c->S, nf, c->A, c->K, c->lbF, c->NL, c->NC, c->caps, c->WA, c->lbW, c->wnear, c->NLW, c->NCW, c->capsw, c->IDcur, c->IDnext); break;
-      case 1: LAUNCH((k_build<2, true>), cdiv(nf, PB), PB, st, c->dp, c->S, nf, c->A, c->K, c->lbF, c->NL, c->NC, c->caps, c->WA, c->lbW, c->wnear, c->NLW, c->NCW, c->capsw, c->IDcur, c->IDnext); break;
-      case 4: LAUNCH((k_build<3, false>), cdiv(nf, PB), PB, st, c->dp, c->S, nf, c->A, c->K, c->lbF, c->NL, c->NC, c->caps, c->WA, c->lbW, c->wnear, c->NLW, c->NCW, c->capsw, c->IDcur, c->IDnext); break;
-      default: LAUNCH((k_build<3, true>), cdiv(nf, PB), PB, st, c->dp, c->S, nf, c->A, c->K, c->lbF, c->NL, c->NC, c->caps, c->WA, c->lbW, c->wnear, c->NLW, c->NCW, c->capsw, c->IDcur, c->IDnext); break;
-    }
-  }
-  pf.mark();  // end list build
-  if (nf > 0) {
-    // third template parameter of k_pass_a: SUBQ (residuals in sigma), not the filter form
-#undef PAIR_SEL
-#define PAIR_SEL(c) (((c)->prm.dim == 3 ? 4 : 0) | ((c)->multi ? 2 : 0) | ((c)->dp.subq ? 1 : 0))
-    PAIR_DISPATCH(k_pass_a, cdiv(nf, PB), st, c->dp, c->S, nf, init, c->A, c->R0, c->K, c->lbF, c->WA, c->WR,
-                  c->lbW, c->wnear, c->R1, c->SIG, c->DRHO, c->NL, c->NC, c->caps, c->NLW, c->NCW, c->capsw);
-  }
-#undef PAIR_SEL
-#define PAIR_SEL(c) (((c)->prm.dim == 3 ? 4 : 0) | ((c)->multi ? 2 : 0) | ((c)->dp.exact_filter ? 1 : 0))
-  pf.mark();  // end pass A
-  launch_wall(c, st, false, c->R1);
-  pf.mark();  // end wall 2
-  if (nf > 0) {
-    PAIR_DISPATCH(k_pass_b, cdiv(nf, PB), st, c->dp, c->S, nf, c->A, c->R1, c->K, c->lbF, c->WA, c->WR,
-                  c->WN, c->lbW, c->wnear, c->TB, c->ACC, c->NL, c->NC, c->caps, c->NLW, c->NCW, c->capsw);
-  }
-  pf.mark();  // end pass B
+  if (wall_branch) CK(cudaStreamWaitEvent(st, c->evJoin, 0));
+  pf.mark(3);  // end reorder
+  if (c->nw > 0 && nf > 0)
+    BUILD_DISPATCH(k_wall_build, cdiv(c->nw, PB), st, c->dp, c->S, (int)c->nw, c->WA, c->WK, c->A, c->lbF, c->NLF,
+                   c->NCF, c->capsw);
+  if (nf > 0)
+    BUILD_DISPATCH(k_build, cdiv(nf, PB), st, c->dp, c->S, nf, c->A, c->K, c->lbF, c->NL, c->NC, c->caps, c->WA,
+                   c->lbW, c->wnear, c->NLW, c->NCW, c->capsw, c->IDcur, c->IDnext);
+  pf.mark(4);  // end list build
   CK(cudaGetLastError());
+  return SPH_OK;
+}
+
+// The part of a step every step runs: wall pass, pass A, wall pass, pass B (R0 -> R1 -> TB, ACC).
+int pass_tail(sph_ctx* c, cudaStream_t st, int init, Prof& pf) {
+  const int nf = (int)c->nf;
+  if (c->moving && !init && c->nw > 0 && c->dp.skin > 0.0)  // kept lists: the walls move inside their cell order
+    LAUNCH(k_wall_move, cdiv(c->nw, 256), 256, st, c->dp, c->S, (int)c->nw, c->WXB, c->WR);
+  launch_wall(c, st, true, c->R0);
+  pf.mark(5);  // end wall 1
+  if (nf > 0) {
+    PAIR_DISPATCH(k_pass_a, SEL3(c, c->dp.subq), cdiv(nf, PB), st, c->dp, c->S, nf, init, c->R0, c->WR, c->R1, c->SIG,
+                  c->DRHO, c->NL, c->NC, c->caps, c->NLW, c->NCW, c->capsw);
+  }
+  pf.mark(6);  // end pass A
+  launch_wall(c, st, false, c->R1);
+  pf.mark(7);  // end wall 2
+  if (nf > 0) {
+    PAIR_DISPATCH(k_pass_b, SEL3(c, 0), cdiv(nf, PB), st, c->dp, c->S, nf, c->R1, c->WR, c->WN, c->TB, c->ACC, c->NL,
+                  c->NC, c->caps, c->NLW, c->NCW, c->capsw);
+  }
+  pf.mark(8);  // end pass B
+  CK(cudaGetLastError());
+  return SPH_OK;
+}
+
+// k_dt + k_predict: the head of a step.  cond / use_cond: the IF node of the step graph (0: plain launches).
+int step_head(sph_ctx* c, cudaStream_t q, const double* seq, int s, cudaGraphConditionalHandle cond, int use_cond) {
+  const int nf = (int)c->nf;
+  const int dt_grid = std::max(1, std::min(cdiv(nf, 256), 148 * 4));
+  LAUNCH(k_dt, dt_grid, 256, q, c->dp, c->S, nf, c->TB, seq, s);
+  if (nf > 0)
+    LAUNCH((k_predict<true, true>), cdiv(nf, 256), 256, q, c->dp, c->S, nf, c->R1, c->TB, c->ACC, c->SIG, c->TX, c->R0,
+           c->keyA, c->valA, cond, use_cond, 1);
+  CK(cudaGetLastError());
+  return SPH_OK;
+}
+
+// One step as a CUDA graph: head (k_dt, k_predict) -> IF node (rebuild branch, taken when k_predict's last
+// block says so through cudaGraphSetConditional) -> tail (wall, pass A, wall, pass B).
+int build_step_graph(sph_ctx* c) {
+  if (!c->cap_stream) CK(cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking));
+  if (!c->cap_stream2) CK(cudaStreamCreateWithFlags(&c->cap_stream2, cudaStreamNonBlocking));
+  const int64_t l0 = c->launches;
+  cudaGraph_t g = nullptr;
+  CK(cudaGraphCreate(&g, 0));
+  cudaGraphConditionalHandle cond = 0;
+  const bool use_cond = c->nf > 0;
+  int rc = SPH_OK;
+  cudaError_t e = cudaSuccess;
+  Prof pf(c, c->cap_stream);
+  pf.on = false;
+  do {
+    if (use_cond) {
+      e = cudaGraphConditionalHandleCreate(&cond, g, 0, cudaGraphCondAssignDefault);
+      if (e != cudaSuccess) break;
+    }
+    e = cudaStreamBeginCaptureToGraph(c->cap_stream, g, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal);
+    if (e != cudaSuccess) break;
+    rc = step_head(c, c->cap_stream, nullptr, 0, cond, use_cond ? 1 : 0);
+    const int64_t l_head = c->launches;
+    if (!rc && use_cond) {
+      cudaStreamCaptureStatus cs;
+      const cudaGraphNode_t* deps = nullptr;
+      size_t nd = 0;
+      e = cudaStreamGetCaptureInfo_v2(c->cap_stream, &cs, nullptr, nullptr, &deps, &nd);
+      if (e != cudaSuccess) break;
+      cudaGraphNodeParams np = {};
+      np.type = cudaGraphNodeTypeConditional;
+      np.conditional.handle = cond;
+      np.conditional.type = cudaGraphCondTypeIf;
+      np.conditional.size = 1;
+      cudaGraphNode_t cn;
+      e = cudaGraphAddNode(&cn, g, deps, nd, &np);
+      if (e != cudaSuccess) break;
+      cudaGraph_t body = np.conditional.phGraph_out[0];
+      e = cudaStreamBeginCaptureToGraph(c->cap_stream2, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal);
+      if (e != cudaSuccess) break;
+      pf.st = c->cap_stream2;
+      rc = rebuild_body(c, c->cap_stream2, 0, pf);
+      cudaError_t e2 = cudaStreamEndCapture(c->cap_stream2, nullptr);
+      c->body_launches = c->launches - l_head;
+      if (e2 != cudaSuccess) { e = e2; break; }
+      e = cudaStreamUpdateCaptureDependencies(c->cap_stream, &cn, 1, cudaStreamSetCaptureDependencies);
+      if (e != cudaSuccess) break;
+    }
+    pf.st = c->cap_stream;
+    if (!rc) rc = pass_tail(c, c->cap_stream, 0, pf);
+  } while (0);
+  cudaGraph_t gout = nullptr;
+  cudaStreamCaptureStatus cst = cudaStreamCaptureStatusNone;
+  cudaStreamIsCapturing(c->cap_stream, &cst);
+  if (cst != cudaStreamCaptureStatusNone) {
+    cudaError_t e3 = cudaStreamEndCapture(c->cap_stream, &gout);
+    if (e == cudaSuccess) e = e3;
+  }
+  c->graph_launches = c->launches - l0 - c->body_launches;  // launches of a step that keeps its lists
+  c->launches = l0;
+  if (rc || e != cudaSuccess) {
+    cudaGraphDestroy(g);
+    if (!rc) { c->err = std::string("step graph: ") + cudaGetErrorString(e); rc = SPH_ECUDA; }
+    return rc;
+  }
+  e = cudaGraphInstantiate(&c->gexec, g, 0);
+  cudaGraphDestroy(g);
+  if (e != cudaSuccess) { c->gexec = nullptr; c->err = std::string("graph instantiate: ") + cudaGetErrorString(e); return SPH_ECUDA; }
   return SPH_OK;
 }
 
@@ -315,57 +436,41 @@ int do_steps(sph_ctx* c, int32_t n_steps, const double* dt_host, cudaStream_t st
     CK(cudaMemcpyAsync(c->dt_seq, dt_host, sizeof(double) * n_steps, cudaMemcpyHostToDevice, st));
     CK(cudaStreamSynchronize(st));  // dt_host may be pageable; keep ownership rules simple
   }
-  const int nf = (int)c->nf;
-  const int dt_grid = std::max(1, std::min(cdiv(nf, 256), 148 * 4));
-  auto one_step = [&](cudaStream_t q, const double* seq, int s, Prof& pf) -> int {
-    pf.mark();  // start
-    LAUNCH(k_dt, dt_grid, 256, q, c->dp, c->S, nf, c->TB, seq, s);
-    if (c->moving && c->nw > 0) {
-      // NEXT-1: the wall re-sort needs the displacement of t^{n+1} (k_dt) and nothing of the fluid: fork
-      // it onto the wall stream; pipeline_after_hash joins before the first wall pass.  Under capture
-      // the events make it a parallel branch of the step graph.
-      CK(cudaEventRecord(c->evFork, q));
-      CK(cudaStreamWaitEvent(c->wstream, c->evFork, 0));
-      int rcw = wall_rebuild(c, c->wstream);
-      if (rcw) return rcw;
-      CK(cudaEventRecord(c->evJoin, c->wstream));
-    }
-    if (nf > 0)
-      LAUNCH(k_predict, cdiv(nf, 256), 256, q, c->dp, c->S, nf, c->R1, c->TB, c->ACC, c->SIG, c->TX, c->keyA, c->valA);
-    pf.mark();  // end predict
-    return pipeline_after_hash(c, q, 0, pf);
-  };
   // Device-computed dt, no per-stage events: every step is the same launch sequence with the same
-  // arguments, so it is captured once (on a private stream) and replayed as a CUDA graph.
+  // arguments, so it is captured once (on private streams) and replayed as a CUDA graph.
   const bool use_graph = !dt_host && !c->prof && !(c->prm.flags & SPH_FLAG_NO_GRAPH) && n_steps > 0;
   if (use_graph && !c->gexec) {
-    if (!c->cap_stream) CK(cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking));
-    CK(cudaStreamSynchronize(st));  // the capture stream is not ordered after st: drain st once
-    const int64_t l0 = c->launches;
-    CK(cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal));
-    Prof pf(c, c->cap_stream);
-    pf.on = false;
-    int rc = one_step(c->cap_stream, nullptr, 0, pf);
-    cudaGraph_t graph = nullptr;
-    cudaError_t e = cudaStreamEndCapture(c->cap_stream, &graph);
-    c->graph_launches = c->launches - l0;
-    c->launches = l0;
-    if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
-    if (e != cudaSuccess) { c->err = std::string("graph capture: ") + cudaGetErrorString(e); return SPH_ECUDA; }
-    e = cudaGraphInstantiate(&c->gexec, graph, 0);
-    cudaGraphDestroy(graph);
-    if (e != cudaSuccess) { c->gexec = nullptr; c->err = std::string("graph instantiate: ") + cudaGetErrorString(e); return SPH_ECUDA; }
+    CK(cudaStreamSynchronize(st));  // the capture streams are not ordered after st: drain st once
+    int rc = build_step_graph(c);
+    if (rc) return rc;
   }
   for (int s = 0; s < n_steps; ++s) {
     if (use_graph) {
       CK(cudaGraphLaunch(c->gexec, st));
-      c->launches += c->graph_launches;
+      c->launches += c->graph_launches;   // + body_launches on the steps that rebuild: added from S->rebuilds at the next stats read
       continue;
     }
+    // plain launches: the host reads the rebuild decision of k_predict (one 4-byte copy and a sync per step)
     Prof pf(c, st);
-    int rc = one_step(st, dt_host ? c->dt_seq : nullptr, s, pf);
+    pf.mark(0);
+    int rc = step_head(c, st, dt_host ? c->dt_seq : nullptr, s, 0, 0);
     if (rc) return rc;
-    pf.done();
+    pf.mark(1);
+    int rb = 1;
+    if (c->nf > 0 && c->dp.skin > 0.0) {
+      CK(cudaMemcpyAsync(&rb, (char*)c->S + offsetof(SS, rebuild), sizeof(int), cudaMemcpyDeviceToHost, st));
+      CK(cudaStreamSynchronize(st));
+    }
+    if (rb) {
+      rc = rebuild_body(c, st, 0, pf);
+      if (rc) return rc;
+      c->direct_rebuilds++;
+    } else {
+      pf.mark(2); pf.mark(3); pf.mark(4);
+    }
+    rc = pass_tail(c, st, 0, pf);
+    if (rc) return rc;
+    pf.done(rb != 0);
   }
   return SPH_OK;
 }
@@ -375,6 +480,61 @@ float4* fluid_images(sph_ctx* c, cudaStream_t st) {
   float4* G = reinterpret_cast<float4*>(c->TX);
   if (c->nf) LAUNCH(k_image, cdiv(c->nf, 256), 256, st, c->dp, (int)c->nf, c->R1, G);
   return G;
+}
+
+// What the integer-contract debug entry points walk: float32 images and caller ids of the fluid and wall
+// particles in the cell order of the CONTRACT grid (reading A24) at the current positions, with its cell bounds.
+// skin = 0: the step's own structures (its grid is the contract grid and it is rebuilt every step).
+// skin > 0: the step's grid has a larger cell edge and is only rebuilt now and then, so the contract order is
+// produced on demand with the step's sort kernels on scratch of its own: a stable sort by caller id, then by
+// contract cell id, i.e. the (unique) order the oracle's std::stable_sort from id order gives (reading A25).
+struct View {
+  DP dp;
+  const float4 *G = nullptr, *WG = nullptr;
+  const unsigned *ID = nullptr, *WID = nullptr;
+  const int *lb = nullptr, *lbW = nullptr;
+};
+
+int contract_order(sph_ctx* c, cudaStream_t st, int n, const float4* G, const unsigned* ID, float4* Gout,
+                   unsigned* IDout, int* lb) {
+  const int nc = (int)c->ncellC;
+  if (n == 0) {
+    LAUNCH(k_cell_bounds, cdiv(nc + 1, 256), 256, st, c->dKa, 0, nc, lb);
+    return SPH_OK;
+  }
+  unsigned *ks, *vs;
+  LAUNCH(k_dbg_idkeys, cdiv(n, 256), 256, st, n, ID, c->dKa, c->dVa);
+  int rc = radix_sort(c, st, n, bits_for(c->n), c->dKa, c->dVa, c->dKb, c->dVb, &ks, &vs);
+  if (rc) return rc;
+  unsigned *k2 = ks == c->dKa ? c->dKb : c->dKa, *v2 = vs == c->dVa ? c->dVb : c->dVa;
+  LAUNCH(k_dbg_cellkeys, cdiv(n, 256), 256, st, c->dpC, n, G, vs, ks);   // keys of the id-ordered sequence, in place of the ids
+  rc = radix_sort(c, st, n, bits_for(c->ncellC), ks, vs, k2, v2, &ks, &vs);
+  if (rc) return rc;
+  LAUNCH(k_dbg_gather, cdiv(n, 256), 256, st, n, vs, G, ID, Gout, IDout);
+  LAUNCH(k_cell_bounds, cdiv(nc + 1, 256), 256, st, ks, n, nc, lb);
+  return SPH_OK;
+}
+
+int contract_view(sph_ctx* c, cudaStream_t st, View* v) {
+  const float4* G = fluid_images(c, st);
+  if (c->moving && c->nw) LAUNCH(k_image, cdiv(c->nw, 256), 256, st, c->dp, (int)c->nw, c->WR, c->WG);
+  v->dp = c->dpC;
+  if (c->dp.skin <= 0.0) {
+    v->G = G; v->ID = c->IDcur; v->lb = c->lbF; v->WG = c->WG; v->WID = c->WID; v->lbW = c->lbW;
+    return SPH_OK;
+  }
+  const size_t cap = (size_t)std::max<int64_t>(std::max(c->nf, c->nw), 1);
+  int rc = dalloc(c, &c->dKa, cap) | dalloc(c, &c->dVa, cap) | dalloc(c, &c->dKb, cap) | dalloc(c, &c->dVb, cap) |
+           dalloc(c, &c->dG, (size_t)c->nf) | dalloc(c, &c->dID, (size_t)c->nf) | dalloc(c, &c->dWG, (size_t)c->nw) |
+           dalloc(c, &c->dWID, (size_t)c->nw) | dalloc(c, &c->dlbF, (size_t)c->ncellC + 1) |
+           dalloc(c, &c->dlbW, (size_t)c->ncellC + 1);
+  if (rc) return SPH_ENOMEM;
+  rc = contract_order(c, st, (int)c->nf, G, c->IDcur, c->dG, c->dID, c->dlbF);
+  if (rc) return rc;
+  rc = contract_order(c, st, (int)c->nw, c->WG, c->WID, c->dWG, c->dWID, c->dlbW);
+  if (rc) return rc;
+  v->G = c->dG; v->ID = c->dID; v->lb = c->dlbF; v->WG = c->dWG; v->WID = c->dWID; v->lbW = c->dlbW;
+  return SPH_OK;
 }
 
 }  // namespace
@@ -400,6 +560,12 @@ int sph_create(const sph_params* prm, sph_ctx** out) {
   memset(&d, 0, sizeof(d));
   const double PI = 3.14159265358979323846264338327950288;
   const double h = prm->h, dp = prm->dp, rc = 2.0 * h;
+  // Verlet skin: the step's lists hold every pair within 2h(1 + s) at the last build
+  double skin = prm->list_skin;
+  if (!(skin >= 0.0)) skin = 0.1;  // library default
+  if (getenv("SPH_SKIN")) skin = atof(getenv("SPH_SKIN"));   // measurement switch (profiles/): not part of the interface
+  if (!(skin >= 0.0) || skin > 0.5) { delete c; return SPH_EINVAL; }
+  const double rl = rc * (1.0 + skin);  // list radius
   d.dim = prm->dim; d.n_phases = prm->n_phases;
   d.rc2 = (float)(4.0 * h * h);
   const double alpha = prm->dim == 2 ? 7.0 / (4.0 * PI * h * h) : 21.0 / (16.0 * PI * h * h * h);
@@ -454,23 +620,33 @@ int sph_create(const sph_params* prm, sph_ctx** out) {
     d.sub_per_m = 1024.0 / d.Q;
     d.Qf = (float)d.Q; d.qh = (float)(d.Q / h); d.qhD = d.Q / h;
     d.mhqD[0] = -0.5 * d.qhD; d.mhqD[1] = d.mhqD[0] / 1024.0; d.tqD[0] = 2.0 * d.qhD; d.tqD[1] = d.tqD[0] / 1024.0;
-    // sigma from residual-exact separations (k_pass_a<.., SUBQ>) when the quantum is coarse for the case: the
-    // acceleration error from positions rounded to Q is about 15 (Q / h) (L / h) g (measured: 5.5e-4 g at
-    // config 4's 16.8 M size, Q / h = 1.4e-7, L / h = 200), so the 1e-4 bar needs (Q / h)(L / h) < 2e-6
-    d.subq = (prm->n_phases > 1 || (d.Q / h) * (Lmax / h) > 2e-6 || getenv("SPH_FORCE_SUBQ")) ? 1 : 0;
-    if (getenv("SPH_NO_SUBQ") && prm->n_phases == 1) d.subq = 0;
+    // sigma from residual-exact separations (k_pass_a<.., SUBQ>, +15 % on pass A) when the quantum is coarse for
+    // the case: positions rounded to Q leave about 15 (Q / h) (L_g / h) |g| in the acceleration, L_g the extent
+    // of the domain along gravity (measured: 5.5e-4 |g| at config 4's 16.8 M size, Q / h = 1.4e-7, L_g / h = 200;
+    // 5.5e-5 with the residuals in p); the 1e-4 bar decides.  Multi-phase runs always.
+    {
+      double gn = 0, Lg = 0;
+      for (int k = 0; k < prm->dim; ++k) gn += prm->g[k] * prm->g[k];
+      for (int k = 0; k < prm->dim; ++k)
+        Lg += (gn > 0 ? fabs(prm->g[k]) / sqrt(gn) : 0.0) * (prm->domain_max[k] - prm->domain_min[k]);
+      if (!(gn > 0)) Lg = Lmax;
+      d.subq = (prm->n_phases > 1 || 15.0 * (d.Q / h) * (Lg / h) > 1e-4) ? 1 : 0;
+      if (getenv("SPH_FORCE_SUBQ")) d.subq = 1;   // measurement switches (profiles/): not part of the interface
+      if (getenv("SPH_NO_SUBQ") && prm->n_phases == 1) d.subq = 0;
+    }
     d.gradcQ = (float)(-5.0 * alpha / (h * h) * d.Q);
     d.two_over_dp = (float)(2.0 * d.Q / dp);
     // candidate filter margin: rounding of the expanded form |xj|^2 - 2 xi.xj + |xi|^2 on images
     // of magnitude <= R, plus the rounding of the images themselves
     const double R = sqrt(R2), u = ldexp(1.0, -24);
-    const double err_expanded = 16.0 * u * R2 + 8.0 * u * R * rc;
-    const double err_diff = 16.0 * u * R * rc;
+    const double err_expanded = 16.0 * u * R2 + 8.0 * u * R * rl;
+    const double err_diff = 16.0 * u * R * rl;
     d.exact_filter = 2.0 * err_expanded > 0.08 * rc * rc ? 1 : 0;
-    d.rc2m = (float)(rc * rc + 2.0 * (d.exact_filter ? err_diff : err_expanded));
-    {  // float16 filter of k_build (sph_pair.cuh): threshold rounded up to the next half
+    d.rc2m = (float)(rl * rl + 2.0 * (d.exact_filter ? err_diff : err_expanded));
+    {  // float16 filter of k_build (sph_pair.cuh): threshold rounded up to the next half; the margin analysis
+       // there is relative to the radius, so the 4.08 of r = 2 becomes 4.08 (1 + s)^2 at the list radius
       d.inv_h = (float)(1.0 / h);
-      const double thr = 4.08 + 2.0 * err_diff / (h * h);
+      const double thr = 4.08 * (1.0 + skin) * (1.0 + skin) + 2.0 * err_diff / (h * h);
       __half th = __double2half(thr);
       if ((double)__half2float(th) < thr) th = __ushort_as_half((unsigned short)(__half_as_ushort(th) + 1));
       d.thr_h2 = (unsigned)__half_as_ushort(th) * 0x10001u;
@@ -478,28 +654,33 @@ int sph_create(const sph_params* prm, sph_ctx** out) {
   }
   d.gamma_p = (float)prm->penalty_strength;
   d.pen_mask = (prm->flags & SPH_FLAG_WALL_ADAMI_ONLY) ? 0u : prm->penalty_phase_mask; d.fs_mask = prm->free_surface_mask; d.flags = prm->flags;
-  const double edge = 2.0 * h * (1.0 + 1.0 / 1024.0);  // reading A24
-  d.inv_edge = (float)(1.0 / edge);
+  d.skin = skin;
+  d.skin_budget = 2.0 * h * skin * (1.0 - 1e-6);
+  // contract grid (reading A24: cell edge 2h(1 + 2^-10)) and the step's grid (cell edge that times 1 + s)
   d.ox = (float)prm->domain_min[0]; d.oy = (float)prm->domain_min[1]; d.oz = (float)prm->domain_min[2];
-  int nc[3] = {1, 1, 1};
-  for (int k = 0; k < prm->dim; ++k)
-    nc[k] = std::max(1, (int)ceil((prm->domain_max[k] - prm->domain_min[k]) / edge));
-  d.nx = nc[0]; d.ny = nc[1]; d.nz = nc[2];
   for (int k = 0; k < 3; ++k) {
     d.dmin[k] = (float)prm->domain_min[k]; d.dmax[k] = (float)prm->domain_max[k];
     d.g[k] = prm->g[k]; d.gamp[k] = prm->g_osc_amp[k];
   }
+  auto set_grid = [&](DP& q, double edge, int64_t* ncell) {
+    q.inv_edge = (float)(1.0 / edge);
+    int nc[3] = {1, 1, 1};
+    for (int k = 0; k < prm->dim; ++k)
+      nc[k] = std::max(1, (int)ceil((prm->domain_max[k] - prm->domain_min[k]) / edge));
+    q.nx = nc[0]; q.ny = nc[1]; q.nz = nc[2];
+    *ncell = (int64_t)nc[0] * nc[1] * nc[2];
+  };
+  const double edgeC = 2.0 * h * (1.0 + 1.0 / 1024.0);  // reading A24
+  set_grid(d, edgeC * (1.0 + skin), &c->ncell);
   for (int k = 0; k < 3; ++k) d.wamp[k] = k < prm->dim ? prm->wall_osc_amp[k] : 0.0;
   d.womega = 6.283185307179586476925286766559 * prm->wall_osc_freq;
   c->moving = prm->wall_osc_freq > 0.0 && (d.wamp[0] != 0.0 || d.wamp[1] != 0.0 || d.wamp[2] != 0.0);
   if (!c->moving) { d.womega = 0.0; d.wamp[0] = d.wamp[1] = d.wamp[2] = 0.0; }
   d.gperiod = prm->g_osc_period; d.cmax = cmax; d.cfl = prm->cfl; d.hD = h; d.dpD = dp;
-  c->ncell = (int64_t)nc[0] * nc[1] * nc[2];
-  if (c->ncell >= (1ll << 31) - 2) { delete c; return SPH_EINVAL; }
-  int bits = 1;
-  while ((1ll << bits) < c->ncell) ++bits;
-  c->sort_bits = (bits + 8) / 9 < (bits + 7) / 8 ? 9 : 8;
-  c->sort_passes = (bits + c->sort_bits - 1) / c->sort_bits;
+  c->dpC = d;
+  set_grid(c->dpC, edgeC, &c->ncellC);
+  if (c->ncell >= (1ll << 31) - 2 || c->ncellC >= (1ll << 31) - 2) { delete c; return SPH_EINVAL; }
+  c->cell_bits = bits_for(c->ncell);
   c->multi = prm->n_phases > 1;
   *out = c;
   return SPH_OK;
@@ -513,7 +694,7 @@ void sph_destroy(sph_ctx* c) {
 
 const char* sph_last_error(const sph_ctx* c) { return c ? c->err.c_str() : "null context"; }
 int64_t sph_launch_count(const sph_ctx* c) { return c ? c->launches : 0; }
-int64_t sph_num_cells(const sph_ctx* c) { return c ? c->ncell : 0; }
+int64_t sph_num_cells(const sph_ctx* c) { return c ? c->ncellC : 0; }
 
 int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel, const float* rho,
                       const int32_t* tag, void* stream) {
@@ -585,7 +766,7 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
     CK(cudaMemcpyAsync(idx, wid.data(), sizeof(int) * nw, cudaMemcpyHostToDevice, st));
     LAUNCH(k_load, cdiv(nw, 256), 256, st, c->dp, nw, 1, idx, pos, vel, rho, tag, c->TX, c->TB, c->ID0, c->keyA, c->valA);
     if (c->moving) {  // NEXT-1: keep the set-up order for the per-step re-sort
-      rc = dalloc(c, &c->WX0, nw) | dalloc(c, &c->WN0, nw) | dalloc(c, &c->WID0, nw) | dalloc(c, &c->WkeyA, nw) | dalloc(c, &c->WkeyB, nw) |
+      rc = dalloc(c, &c->WX0, nw) | dalloc(c, &c->WXB, nw) | dalloc(c, &c->WN0, nw) | dalloc(c, &c->WID0, nw) | dalloc(c, &c->WkeyA, nw) | dalloc(c, &c->WkeyB, nw) |
            dalloc(c, &c->WvalA, nw) | dalloc(c, &c->WvalB, nw) | dalloc(c, &c->WTX, nw) | dalloc(c, &c->WTB, nw) |
            dalloc(c, &c->Whist, (size_t)512 * cdiv(nw, RS_THREADS * rs_items((size_t)nw))) | dalloc(c, &c->Wrowsum, 512);
       if (rc) return rc;
@@ -597,7 +778,7 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
       CK(cudaMemcpyAsync(c->WID0, c->ID0, sizeof(unsigned) * nw, cudaMemcpyDeviceToDevice, st));
     }
     unsigned *ks, *vs;
-    rc = radix_sort(c, st, nw, c->keyA, c->valA, c->keyB, c->valB, &ks, &vs);
+    rc = radix_sort(c, st, nw, c->cell_bits, c->keyA, c->valA, c->keyB, c->valB, &ks, &vs);
     if (rc) return rc;
     LAUNCH(k_reorder, cdiv(nw, 256), 256, st, c->dp, nw, vs, c->TX, c->TB, c->ID0, c->WR, c->WA, c->WID,
            (const unsigned*)nullptr, -1, (int*)nullptr);
@@ -606,7 +787,10 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
     LAUNCH(k_cell_bounds, cdiv(c->ncell + 1, 256), 256, st, ks, nw, (int)c->ncell, c->lbW);
     if (c->prm.dim == 3) LAUNCH(k_normals<3>, cdiv(nw, 128), 128, st, c->dp, nw, c->WR, c->WK, c->lbW, c->WN);
     else LAUNCH(k_normals<2>, cdiv(nw, 128), 128, st, c->dp, nw, c->WR, c->WK, c->lbW, c->WN);
-    if (c->moving) LAUNCH(k_unsort4, cdiv(nw, 256), 256, st, nw, vs, c->WN, c->WN0);
+    if (c->moving) {
+      LAUNCH(k_unsort4, cdiv(nw, 256), 256, st, nw, vs, c->WN, c->WN0);
+      LAUNCH(k_gatherx, cdiv(nw, 256), 256, st, nw, vs, c->WX0, c->WXB);
+    }
   } else {
     LAUNCH(k_cell_bounds, cdiv(c->ncell + 1, 256), 256, st, c->keyA, 0, (int)c->ncell, c->lbW);
   }
@@ -619,7 +803,9 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
   }
   Prof pf(c, st);
   pf.on = false;
-  rc = pipeline_after_hash(c, st, 1, pf);
+  rc = rebuild_body(c, st, 1, pf);
+  if (!rc) rc = pass_tail(c, st, 1, pf);
+  c->direct_rebuilds = 0; c->graph_rebuilds_counted = 0;
   cudaError_t e = cudaStreamSynchronize(st);
   if (rc) return rc;
   if (e != cudaSuccess) { c->err = cudaGetErrorString(e); return SPH_ECUDA; }
@@ -712,9 +898,11 @@ int sph_get_stats_ex(sph_ctx* c, sph_stats* out, int32_t with_pairs, void* strea
   if (nf) {
     LAUNCH(k_stats, std::min(cdiv(nf, 256), 1184), 256, st, c->dp, nf, c->R1, c->TB, c->stat);
     if (with_pairs) {
-      const float4* G = fluid_images(c, st);
-      LAUNCH(k_neigh, cdiv(nf, PW), PW * 32, st, c->dp, nf, 0, 0, G, c->IDcur, G, c->IDcur, c->lbF, c->WG,
-             c->WID, c->lbW, (int*)nullptr, (const long long*)nullptr, (int*)nullptr, 0ll, &c->stat->pairs);
+      View v;
+      int rc = contract_view(c, st, &v);
+      if (rc) return rc;
+      LAUNCH(k_neigh, cdiv(nf, PW), PW * 32, st, v.dp, nf, 0, 0, v.G, v.ID, v.G, v.ID, v.lb, v.WG,
+             v.WID, v.lbW, (int*)nullptr, (const long long*)nullptr, (int*)nullptr, 0ll, &c->stat->pairs);
     }
   }
   SS hs;
@@ -733,6 +921,14 @@ int sph_get_stats_ex(sph_ctx* c, sph_stats* out, int32_t with_pairs, void* strea
     out->x_front = z.xfront_bits == 0 ? -INFINITY : (double)f;
   }
   out->escaped = (int64_t)hs.escaped; out->nonfinite = (int64_t)hs.nonfinite;
+  out->rebuilds = (int64_t)hs.rebuilds + 1;  // + the set-up's
+  {  // rebuild branches taken inside graph replays: their kernels were launched by the graph, count them now
+    const int64_t in_graph = (int64_t)hs.rebuilds - c->direct_rebuilds;
+    if (in_graph > c->graph_rebuilds_counted) {
+      c->launches += (in_graph - c->graph_rebuilds_counted) * c->body_launches;
+      c->graph_rebuilds_counted = in_graph;
+    }
+  }
   if (hs.nonfinite) { c->err = "non-finite particle state"; return SPH_ENONFINITE; }
   if (hs.list_overflow) {
     c->err = "a particle has " + std::to_string(hs.list_overflow) + " neighbours, the lists hold " +
@@ -755,21 +951,24 @@ int sph_set_profiling(sph_ctx* c, int32_t on) {
   return SPH_OK;
 }
 
-int sph_get_timings(sph_ctx* c, float* ms, int32_t* n_steps) {
+int sph_get_timings(sph_ctx* c, float* ms, int32_t* n_steps, int32_t* n_rebuilds) {
   if (!c || !ms || !n_steps) return SPH_EINVAL;
   for (int k = 0; k < SPH_STAGE_COUNT; ++k) ms[k] = 0.f;
   *n_steps = c->ev_steps;
+  if (n_rebuilds) *n_rebuilds = 0;
   if (c->ev_steps == 0) return SPH_OK;
   CK(cudaEventSynchronize(c->ev[(c->ev_steps - 1) * sph_ctx::EV_PER_STEP + 8]));
-  // marks per step: 0 start, 1 predict, 2 sort, 3 reorder, 4 wall1, 5 list build, 6 passA, 7 wall2, 8 passB
-  static const int stage_of[8] = {SPH_STAGE_PREDICT, SPH_STAGE_SORT, SPH_STAGE_REORDER, SPH_STAGE_WALL, SPH_STAGE_BUILD,
+  // marks per step: 0 start, 1 predict, 2 sort, 3 reorder, 4 list build, 5 wall 1, 6 pass A, 7 wall 2, 8 pass B
+  static const int stage_of[8] = {SPH_STAGE_PREDICT, SPH_STAGE_SORT, SPH_STAGE_REORDER, SPH_STAGE_BUILD, SPH_STAGE_WALL,
                                   SPH_STAGE_PASS_A, SPH_STAGE_WALL, SPH_STAGE_PASS_B};
-  for (int s = 0; s < c->ev_steps; ++s)
+  for (int s = 0; s < c->ev_steps; ++s) {
+    if (n_rebuilds && c->ev_rebuilt[s]) ++*n_rebuilds;
     for (int k = 0; k < 8; ++k) {
       float t = 0.f;
       CK(cudaEventElapsedTime(&t, c->ev[s * sph_ctx::EV_PER_STEP + k], c->ev[s * sph_ctx::EV_PER_STEP + k + 1]));
       ms[stage_of[k]] += t;
     }
+  }
   c->ev_steps = 0;
   return SPH_OK;
 }
@@ -778,15 +977,17 @@ int sph_debug_cells(sph_ctx* c, int32_t* cell_id, int32_t* perm, int32_t* cs, in
   if (!c) return SPH_EINVAL;
   if (!c->loaded) { c->err = "no particles"; return SPH_EINVAL; }
   cudaStream_t st = (cudaStream_t)stream;
-  const size_t n = (size_t)std::max<int64_t>(c->n, 1), nc = (size_t)c->ncell;
+  const size_t n = (size_t)std::max<int64_t>(c->n, 1), nc = (size_t)c->ncellC;
   int *dcid = nullptr, *dperm = nullptr, *dcs = nullptr, *dce = nullptr;
   CK(cudaMalloc((void**)&dcid, n * 4)); CK(cudaMalloc((void**)&dperm, n * 4));
   CK(cudaMalloc((void**)&dcs, 2 * nc * 4)); CK(cudaMalloc((void**)&dce, 2 * nc * 4));
-  const float4* G = fluid_images(c, st);
-  if (c->nf) LAUNCH(k_dbg_cells, cdiv(c->nf, 256), 256, st, c->dp, (int)c->nf, G, c->IDcur, dcid, dperm, 0);
-  if (c->nw) LAUNCH(k_dbg_cells, cdiv(c->nw, 256), 256, st, c->dp, (int)c->nw, c->WG, c->WID, dcid, dperm, (int)c->nf);
-  LAUNCH(k_dbg_ranges, cdiv(nc, 256), 256, st, (int)nc, c->lbF, dcs, dce);
-  LAUNCH(k_dbg_ranges, cdiv(nc, 256), 256, st, (int)nc, c->lbW, dcs + nc, dce + nc);
+  View v;
+  int rcv = contract_view(c, st, &v);
+  if (rcv) { cudaFree(dcid); cudaFree(dperm); cudaFree(dcs); cudaFree(dce); return rcv; }
+  if (c->nf) LAUNCH(k_dbg_cells, cdiv(c->nf, 256), 256, st, v.dp, (int)c->nf, v.G, v.ID, dcid, dperm, 0);
+  if (c->nw) LAUNCH(k_dbg_cells, cdiv(c->nw, 256), 256, st, v.dp, (int)c->nw, v.WG, v.WID, dcid, dperm, (int)c->nf);
+  LAUNCH(k_dbg_ranges, cdiv(nc, 256), 256, st, (int)nc, v.lb, dcs, dce);
+  LAUNCH(k_dbg_ranges, cdiv(nc, 256), 256, st, (int)nc, v.lbW, dcs + nc, dce + nc);
   cudaError_t e = cudaSuccess;
   if (cell_id && c->n) e = cudaMemcpyAsync(cell_id, dcid, c->n * 4, cudaMemcpyDeviceToHost, st);
   if (perm && c->n && e == cudaSuccess) e = cudaMemcpyAsync(perm, dperm, c->n * 4, cudaMemcpyDeviceToHost, st);
@@ -809,14 +1010,16 @@ int sph_debug_neighbours(sph_ctx* c, int64_t* offsets, int32_t* ids, int64_t cap
   int* dcnt = nullptr;
   CK(cudaMalloc((void**)&dcnt, std::max<int64_t>(n, 1) * 4));
   CK(cudaMemsetAsync(dcnt, 0, std::max<int64_t>(n, 1) * 4, st));
-  const float4* G = fluid_images(c, st);
+  View v;
+  int rcv = contract_view(c, st, &v);
+  if (rcv) { cudaFree(dcnt); return rcv; }
   auto run = [&](int mode, const long long* doff, int* dids, long long dcap) {
     if (c->nf)
-      LAUNCH(k_neigh, cdiv(c->nf, PW), PW * 32, st, c->dp, (int)c->nf, 0, mode, G, c->IDcur, G, c->IDcur, c->lbF,
-             c->WG, c->WID, c->lbW, dcnt, doff, dids, dcap, (unsigned long long*)nullptr);
+      LAUNCH(k_neigh, cdiv(c->nf, PW), PW * 32, st, v.dp, (int)c->nf, 0, mode, v.G, v.ID, v.G, v.ID, v.lb,
+             v.WG, v.WID, v.lbW, dcnt, doff, dids, dcap, (unsigned long long*)nullptr);
     if (c->nw && c->nf)
-      LAUNCH(k_neigh, cdiv(c->nw, PW), PW * 32, st, c->dp, (int)c->nw, 1, mode, c->WG, c->WID, G, c->IDcur, c->lbF,
-             c->WG, c->WID, c->lbW, dcnt, doff, dids, dcap, (unsigned long long*)nullptr);
+      LAUNCH(k_neigh, cdiv(c->nw, PW), PW * 32, st, v.dp, (int)c->nw, 1, mode, v.WG, v.WID, v.G, v.ID, v.lb,
+             v.WG, v.WID, v.lbW, dcnt, doff, dids, dcap, (unsigned long long*)nullptr);
   };
   run(0, nullptr, nullptr, 0);
   std::vector<int> hc((size_t)n);
@@ -935,6 +1138,42 @@ int sph_debug_step_lists(sph_ctx* c, int64_t* offsets, int32_t* ids, int64_t cap
   }
   cudaFree(dcnt);
   return rc;
+}
+
+int sph_debug_time_pointwise(sph_ctx* c, float* ms, void* stream) {
+  if (!c || !ms) return SPH_EINVAL;
+  if (!c->loaded) { c->err = "no particles"; return SPH_EINVAL; }
+  cudaStream_t st = (cudaStream_t)stream;
+  ms[0] = ms[1] = ms[2] = 0.f;
+  const int nf = (int)c->nf;
+  if (!nf) return SPH_OK;
+  // scratch outputs: the state (R1, TB, ACC, SIG, R0, keyA / valA of the step) is read, never written
+  float4* B2 = nullptr; uint4* X2 = nullptr; XB* R2 = nullptr; unsigned *k2 = nullptr, *v2 = nullptr;
+  CK(cudaMalloc((void**)&B2, sizeof(float4) * nf)); CK(cudaMalloc((void**)&X2, sizeof(uint4) * nf));
+  CK(cudaMalloc((void**)&R2, sizeof(XB) * nf)); CK(cudaMalloc((void**)&k2, 4 * (size_t)nf)); CK(cudaMalloc((void**)&v2, 4 * (size_t)nf));
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  const int grid = cdiv(nf, 256);
+  for (int which = 0; which < 3; ++which) {
+    float tot = 0.f;
+    for (int rep = 0; rep < 6; ++rep) {
+      CK(cudaMemcpyAsync(B2, c->TB, sizeof(float4) * nf, cudaMemcpyDeviceToDevice, st));  // the kernels update (v, rho) in place
+      cudaEventRecord(e0, st);
+      if (which == 0) LAUNCH((k_predict<true, false>), grid, 256, st, c->dp, c->S, nf, c->R1, B2, c->ACC, c->SIG, X2, R2, k2, v2, 0ull, 0, 0);
+      else if (which == 1) LAUNCH((k_predict<false, true>), grid, 256, st, c->dp, c->S, nf, c->R1, B2, c->ACC, c->SIG, X2, R2, k2, v2, 0ull, 0, 0);
+      else LAUNCH((k_predict<true, true>), grid, 256, st, c->dp, c->S, nf, c->R1, B2, c->ACC, c->SIG, X2, R2, k2, v2, 0ull, 0, 0);
+      cudaEventRecord(e1, st);
+      cudaError_t e = cudaEventSynchronize(e1);
+      if (e != cudaSuccess) { c->err = cudaGetErrorString(e); return SPH_ECUDA; }
+      float t = 0.f;
+      cudaEventElapsedTime(&t, e0, e1);
+      if (rep) tot += t;
+    }
+    ms[which] = tot / 5.f;
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  cudaFree(B2); cudaFree(X2); cudaFree(R2); cudaFree(k2); cudaFree(v2);
+  return SPH_OK;
 }
 
 int sph_debug_fma_peak(double* tflops_host, void* stream) {

@@ -48,6 +48,12 @@ k_gather4(int n, const unsigned* __restrict__ vals, const float4* __restrict__ i
   if (s < n) out[s] = in[vals[s]];
 }
 
+__global__ void __launch_bounds__(256)
+k_gatherx(int n, const unsigned* __restrict__ vals, const uint4* __restrict__ in, uint4* __restrict__ out) {
+  const int s = blockIdx.x * 256 + threadIdx.x;
+  if (s < n) out[s] = in[vals[s]];
+}
+
 // NEXT-1 (moving walls): wall particles in set-up order at their displaced positions X0 + sq, with the
 // cell hash of the new position; input of the per-step wall re-sort.
 __global__ void __launch_bounds__(256)
@@ -167,48 +173,109 @@ __device__ __forceinline__ unsigned drift_axis(unsigned X, unsigned& res, double
 
 // Predictor: density reinitialisation Eq. 2.17 / 2.18 from the sigma_i of the last pass A
 // (same positions, reading A13), first half kick Eq. 2.19, drift Eq. 2.20,
-// cell hash of the new position.  In place on (v, rho) ; the new position goes to TX.
+// cell hash of the new position.  In place on (v, rho); the new record goes to Rout (the input of the
+// pair passes when the lists are kept) and the new position to TX (the input of the reorder when
+// they are rebuilt).
+// Verlet skin: the block maxima of |dx_i|^2 are combined with atomicMax and the last block to finish
+// adds this step's largest displacement to S->disp, decides whether the lists (built with radius
+// 2h(1 + skin)) still hold every pair within 2h, and publishes the decision: S->rebuild and, when
+// the step runs as a CUDA graph, the condition of the IF node that holds the rebuild branch.
+// DO_REINIT / DO_MOVE = false give the stand-alone "density reinitialisation kernel" and "integrator"
+// that BASELINE.json's config 4 asks to be timed separately (sph_debug_time_pointwise); the step
+// itself runs the fused <true, true> form.
+template <bool DO_REINIT, bool DO_MOVE>
 __global__ void __launch_bounds__(256)
 k_predict(DP p, SS* __restrict__ S, int nf, const XB* __restrict__ R, float4* __restrict__ B,
           const float4* __restrict__ ACC, const float* __restrict__ SIG, uint4* __restrict__ TX,
-          unsigned* __restrict__ keys, unsigned* __restrict__ vals) {
+          XB* __restrict__ Rout, unsigned* __restrict__ keys, unsigned* __restrict__ vals,
+          cudaGraphConditionalHandle cond, int use_cond, int decide) {
+  __shared__ float smax[8];
   const int i = blockIdx.x * 256 + threadIdx.x;
-  if (i >= nf) return;
-  uint4 x = R[i].x;
-  float4 b = B[i];
-  const float4 a = ACC[i];
-  const int ph = phase_of(x);
-  if (p.flags & SPH_FLAG_REINIT) {
-    const float rho0 = p.rho0[ph];
-    const float ds = rho0 * SIG[i];  // rho0 sigma/sigma0 - rho0; SIG holds sigma/sigma0 - 1
-    float d = ds;
-    // Eq. 2.17 for rho* > rho_s: rho - rho0 = rho_s (rho* - rho0) / rho*  (same value as
-    // rho_s + (rho* - rho_s) rho0 / rho*, without the cancellation of two O(rho0) terms)
-    if (((p.fs_mask >> ph) & 1u) && b.w > ds) d = b.w * ((rho0 + ds) / (rho0 + b.w));
-    b.w = d;
+  float d2 = 0.f;
+  if (i < nf) {
+    uint4 x = R[i].x;
+    float4 b = B[i];
+    const int ph = phase_of(x);
+    if (DO_REINIT && (p.flags & SPH_FLAG_REINIT)) {
+      const float rho0 = p.rho0[ph];
+      const float ds = rho0 * SIG[i];  // rho0 sigma/sigma0 - rho0; SIG holds sigma/sigma0 - 1
+      float d = ds;
+      // Eq. 2.17 for rho* > rho_s: rho - rho0 = rho_s (rho* - rho0) / rho*  (same value as
+      // rho_s + (rho* - rho_s) rho0 / rho*, without the cancellation of two O(rho0) terms)
+      if (((p.fs_mask >> ph) & 1u) && b.w > ds) d = b.w * ((rho0 + ds) / (rho0 + b.w));
+      b.w = d;
+    }
+    if (DO_MOVE) {
+      const float4 a = ACC[i];
+      const float hdt = 0.5f * S->dt;
+      b.x = fmaf(hdt, a.x, b.x); b.y = fmaf(hdt, a.y, b.y); b.z = fmaf(hdt, a.z, b.z);  // Eq. 2.19
+      const bool fin = isfinite(b.x) && isfinite(b.y) && isfinite(b.z);
+      if (fin) {
+        const double k = S->dt_d * p.sub_per_m;
+        unsigned rx = (x.w >> 22) & 1023u, ry = (x.w >> 12) & 1023u, rz = (x.w >> 2) & 1023u;
+        x.x = drift_axis(x.x, rx, k * (double)b.x);
+        x.y = drift_axis(x.y, ry, k * (double)b.y);
+        if (p.dim == 3) x.z = drift_axis(x.z, rz, k * (double)b.z);
+        x.w = (rx << 22) | (ry << 12) | (rz << 2) | (unsigned)ph;
+        // this step's displacement, rounded up: |dx| <= dt |v| (1 + 2^-20) + one sub-quantum per axis
+        const float dtf = S->dt * 1.000001f;
+        d2 = dtf * dtf * fmaf(b.z, b.z, fmaf(b.y, b.y, b.x * b.x));
+      } else {
+        atomicAdd(&S->nonfinite, 1ull);
+      }
+      TX[i] = x;
+      const float gx = fx_image(x.x, p.O[0], p.Q), gy = fx_image(x.y, p.O[1], p.Q);
+      const float gz = p.dim == 3 ? fx_image(x.z, p.O[2], p.Q) : 0.0f;
+      bool out = gx < p.dmin[0] || gx >= p.dmax[0] || gy < p.dmin[1] || gy >= p.dmax[1];
+      if (p.dim == 3) out = out || gz < p.dmin[2] || gz >= p.dmax[2];
+      if (out || !fin) atomicAdd(&S->escaped, 1ull);
+      keys[i] = cell_key(p, gx, gy, gz);
+      vals[i] = (unsigned)i;
+    }
+    B[i] = b;
+    Rout[i] = XB{x, b};
   }
-  const float hdt = 0.5f * S->dt;
-  b.x = fmaf(hdt, a.x, b.x); b.y = fmaf(hdt, a.y, b.y); b.z = fmaf(hdt, a.z, b.z);  // Eq. 2.19
-  const bool fin = isfinite(b.x) && isfinite(b.y) && isfinite(b.z);
-  if (fin) {
-    const double k = S->dt_d * p.sub_per_m;
-    unsigned rx = (x.w >> 22) & 1023u, ry = (x.w >> 12) & 1023u, rz = (x.w >> 2) & 1023u;
-    x.x = drift_axis(x.x, rx, k * (double)b.x);
-    x.y = drift_axis(x.y, ry, k * (double)b.y);
-    if (p.dim == 3) x.z = drift_axis(x.z, rz, k * (double)b.z);
-    x.w = (rx << 22) | (ry << 12) | (rz << 2) | (unsigned)ph;
-  } else {
-    atomicAdd(&S->nonfinite, 1ull);
+  if (!decide) return;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) d2 = fmaxf(d2, __shfl_xor_sync(FULL, d2, o));
+  if ((threadIdx.x & 31) == 0) smax[threadIdx.x >> 5] = d2;
+  __syncthreads();
+  if (threadIdx.x != 0) return;
+  for (int w = 1; w < 8; ++w) d2 = fmaxf(d2, smax[w]);
+  if (d2 > 0.f) atomicMax(&S->dmax2_bits, __float_as_uint(d2));
+  __threadfence();
+  if (atomicAdd(&S->blocks_done2, 1u) != gridDim.x - 1) return;
+  __threadfence();
+  const double dstep = sqrt((double)__uint_as_float(atomicMax(&S->dmax2_bits, 0u))) + 2.0 * p.Q;
+  double disp = S->disp + dstep;
+  double dw2 = 0.0;
+  for (int k = 0; k < 3; ++k) {
+    const double d = p.Q * (double)(S->sq[k] - S->sq_build[k]);
+    dw2 += d * d;
   }
-  TX[i] = x;
-  B[i] = b;
-  const float gx = fx_image(x.x, p.O[0], p.Q), gy = fx_image(x.y, p.O[1], p.Q);
-  const float gz = p.dim == 3 ? fx_image(x.z, p.O[2], p.Q) : 0.0f;
-  bool out = gx < p.dmin[0] || gx >= p.dmax[0] || gy < p.dmin[1] || gy >= p.dmax[1];
-  if (p.dim == 3) out = out || gz < p.dmin[2] || gz >= p.dmax[2];
-  if (out || !fin) atomicAdd(&S->escaped, 1ull);
-  keys[i] = cell_key(p, gx, gy, gz);
-  vals[i] = (unsigned)i;
+  const int rb = (p.skin <= 0.0 || 2.0 * disp > p.skin_budget || disp + sqrt(dw2) > p.skin_budget) ? 1 : 0;
+  if (rb) {
+    disp = 0.0;
+    for (int k = 0; k < 3; ++k) S->sq_build[k] = S->sq[k];
+    S->rebuilds += 1;
+  }
+  S->disp = disp;
+  S->rebuild = rb;
+  S->dmax2_bits = 0u;
+  S->blocks_done2 = 0u;
+  if (use_cond) cudaGraphSetConditional(cond, (unsigned)rb);
+}
+
+// NEXT-1 with kept lists: the wall records in their cell order of the last list build, at the displacement of
+// t^{n+1} (WXB: the positions of sph_set_particles in that order).
+__global__ void __launch_bounds__(256)
+k_wall_move(DP p, const SS* __restrict__ S, int nw, const uint4* __restrict__ WXB, XB* __restrict__ WR) {
+  const int i = blockIdx.x * 256 + threadIdx.x;
+  if (i >= nw) return;
+  uint4 x = WXB[i];
+  x.x += (unsigned)S->sq[0]; x.y += (unsigned)S->sq[1];
+  if (p.dim == 3) x.z += (unsigned)S->sq[2];
+  WR[i].x = x;
 }
 
 // Wall normals, Eq. 2.16, once, in float64 (reading A10).

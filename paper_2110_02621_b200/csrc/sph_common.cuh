@@ -41,6 +41,10 @@ struct DP {
   double a_over_s0;
   double g[3], gamp[3], gperiod;
   double wamp[3], womega;  // NEXT-1: wall motion x_w(t) = x_w(0) + wamp sin(womega t); womega = 0: static walls
+  // Verlet skin: the lists are built with radius 2h(1 + skin) on a cell grid of that edge
+  // and kept while 2 * (fluid displacement bound) and (fluid + wall displacement) stay below skin_budget
+  double skin;         // s >= 0; 0: the lists are rebuilt every step
+  double skin_budget;  // 2 h s (1 - 1e-6) in metres
 };
 
 // Per-particle record gathered by the pair bodies: one 32-byte sector, one 256-bit load.
@@ -72,6 +76,14 @@ struct SS {
   unsigned long long escaped, nonfinite;
   int dt_underflow;
   int list_overflow;     // largest neighbour count seen above the list capacity (0 = none); sticky
+  // Verlet skin: written by k_predict's last block
+  double disp;             // sum over the steps since the last list build of max_i |dx_i| (metres): a bound on
+                           // every fluid particle's displacement since then
+  int sq_build[3];         // wall displacement (units of Q) at the last list build
+  int rebuild;             // 1: this step rebuilds the cell list and the neighbour lists
+  unsigned dmax2_bits;     // max_i |dx_i|^2 of this step (float bits)
+  unsigned blocks_done2;
+  long long rebuilds;      // list builds since sph_set_particles (the set-up's included)
 };
 
 #define FULL 0xffffffffu

@@ -253,6 +253,29 @@ __global__ void k_dbg_cells(DP p, int n, const float4* __restrict__ P, const uns
   if (perm) perm[perm_base + i] = (int)ID[i];
 }
 
+// contract_view (sph.cu): sort keys of the on-demand contract order
+__global__ void k_dbg_idkeys(int n, const unsigned* __restrict__ ID, unsigned* __restrict__ keys, unsigned* __restrict__ vals) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  keys[i] = ID[i];
+  vals[i] = (unsigned)i;
+}
+__global__ void k_dbg_cellkeys(DP p, int n, const float4* __restrict__ G, const unsigned* __restrict__ vals,
+                               unsigned* __restrict__ keys) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= n) return;
+  const float4 r = G[vals[k]];
+  keys[k] = cell_key(p, r.x, r.y, r.z);
+}
+__global__ void k_dbg_gather(int n, const unsigned* __restrict__ vals, const float4* __restrict__ G,
+                             const unsigned* __restrict__ ID, float4* __restrict__ Gout, unsigned* __restrict__ IDout) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= n) return;
+  const unsigned v = vals[k];
+  Gout[k] = G[v];
+  IDout[k] = ID[v];
+}
+
 __global__ void k_dbg_ranges(int ncell, const int* __restrict__ lb, int* cs, int* ce) {
   int c = blockIdx.x * blockDim.x + threadIdx.x;
   if (c >= ncell) return;

@@ -483,37 +483,41 @@ k_build(const DP p, SS* __restrict__ S, const int nf, const float4* __restrict__
 // Wall extrapolation, Eq. 2.12 (readings A4-A7); a_w = 0, v_wall = 0.
 // One thread per wall dummy particle, summing over its fluid neighbours.  WB = (v_w, p_w).
 // ------------------------------------------------------------------------------------------
-template <int DIM, bool MULTI, bool EXACT, bool WITH_VEL>
+// k_wall_build (list build only, in the rebuild branch of a step): the float32 filter walk of every wall
+// particle over the fluid arrays, survivors written to its wall-fluid neighbour list NLF / NCF.
+template <int DIM, bool EXACT>
 __global__ void __launch_bounds__(PB)
-k_wall(const DP p, SS* __restrict__ S, const int nw, const float4* __restrict__ WA,
-       XB* __restrict__ WR, const unsigned* __restrict__ WK,
-       const float4* __restrict__ A, const XB* __restrict__ R, const int* __restrict__ lbF,
-       uint4* __restrict__ NLF, int* __restrict__ NCF, const int capsf) {
-  // The first wall pass of a step (WITH_VEL) filters the fluid candidates of every wall particle
-  // into a wall-fluid neighbour list; the second one (after pass A, same positions) only reads it.
+k_wall_build(const DP p, SS* __restrict__ S, const int nw, const float4* __restrict__ WA,
+             const unsigned* __restrict__ WK, const float4* __restrict__ A, const int* __restrict__ lbF,
+             uint4* __restrict__ NLF, int* __restrict__ NCF, const int capsf) {
+  __shared__ unsigned qs[QCAP * PB];
+  const int w0 = blockIdx.x * PB + threadIdx.x;
+  const bool act = w0 < nw;
+  const int w = act ? w0 : nw - 1;
+  uint4* col = NLF + (size_t)(w0 >> 5) * (capsf >> 2) * 32 + (threadIdx.x & 31);
+  const float4 ai = WA[w];
+  int cx, cy, cz;
+  cell_of_key(p, WK[w], cx, cy, cz);
+  ListSink sink(qs + threadIdx.x, col, capsf >> 2);
+  walk_f<DIM, EXACT, false>(p, A, lbF, act, ai, cx, cy, cz, nullptr, HCtx{}, sink);
+  if (act) {
+    NCF[w] = min(sink.n, capsf);
+    if (sink.n > capsf) atomicMax(&S->list_overflow, sink.n);
+  }
+}
+
+// k_wall: Eq. 2.12 for every wall particle from its wall-fluid neighbour list; WITH_VEL: pressure and the
+// velocity of reading A6 (first wall pass of a step), else the pressure only (second pass, after pass A).
+template <int DIM, bool MULTI, bool WITH_VEL>
+__global__ void __launch_bounds__(PB)
+k_wall(const DP p, const SS* __restrict__ S, const int nw, XB* __restrict__ WR, const XB* __restrict__ R,
+       const uint4* __restrict__ NLF, const int* __restrict__ NCF, const int capsf) {
   const int w0 = blockIdx.x * PB + threadIdx.x;
   const bool act = w0 < nw;
   const int w = act ? w0 : nw - 1;
   const uint4 xi = WR[w].x;
-  uint4* col = NLF + (size_t)(w0 >> 5) * (capsf >> 2) * 32 + (threadIdx.x & 31);
-  int cnt;
-  if (WITH_VEL) {
-    __shared__ unsigned qs[QCAP * PB];
-    const float4 ai = WA[w];
-    int cx, cy, cz;
-    cell_of_key(p, WK[w], cx, cy, cz);
-    ListSink sink(qs + threadIdx.x, col, capsf >> 2);
-    walk_f<DIM, EXACT, false>(p, A, lbF, act, ai, cx, cy, cz, nullptr, HCtx{}, sink);
-    cnt = min(sink.n, capsf);
-    if (act) {
-      NCF[w] = cnt;
-      if (sink.n > capsf) atomicMax(&S->list_overflow, sink.n);
-    }
-    __syncwarp();  // the list walk below reads what this lane wrote (same thread: program order suffices)
-  } else {
-    cnt = act ? NCF[w] : 0;
-  }
-  if (!act) cnt = 0;
+  const uint4* col = NLF + (size_t)(w0 >> 5) * (capsf >> 2) * 32 + (threadIdx.x & 31);
+  const int cnt = act ? NCF[w] : 0;
   float sW = 0, sp = 0, sWr = 0, srx = 0, sry = 0, srz = 0, svx = 0, svy = 0, svz = 0;
   // multi-phase form of Eq. 2.12 (every fluid term divided by rho_f) unless the run asks for the
   // wall model of Adami et al. (2012) without the paper's extensions (NEXT-4 ablation)
@@ -536,7 +540,7 @@ k_wall(const DP p, SS* __restrict__ S, const int nw, const float4* __restrict__ 
     }
     if (WITH_VEL) { svx = fmaf(bj.x, g.w, svx); svy = fmaf(bj.y, g.w, svy); svz = fmaf(bj.z, g.w, svz); }
     });
-    walk_l<!WITH_VEL>(col, cnt, body);
+    walk_l(col, cnt, body);
   }
   if (!act) return;
   float pwall = 0.f, vx = S->vwall[0], vy = S->vwall[1], vz = S->vwall[2];  // reading A7: v_w = v_wall
@@ -565,10 +569,7 @@ k_wall(const DP p, SS* __restrict__ S, const int nw, const float4* __restrict__ 
 template <int DIM, bool MULTI, bool SUBQ>
 __global__ void __launch_bounds__(PB, SPH_MINB)
 k_pass_a(const DP p, const SS* __restrict__ S, const int nf, const int init,
-         const float4* __restrict__ A, const XB* __restrict__ R,
-         const unsigned* __restrict__ K, const int* __restrict__ lbF,
-         const float4* __restrict__ WA, const XB* __restrict__ WR,
-         const int* __restrict__ lbW, const unsigned char* __restrict__ wnear,
+         const XB* __restrict__ R, const XB* __restrict__ WR,
          XB* __restrict__ Rout, float* __restrict__ SIG, float* __restrict__ DRHO,
          const uint4* __restrict__ NL, const int* __restrict__ NC, const int caps,
          const uint4* __restrict__ NLW, const int* __restrict__ NCW, const int capsw) {
@@ -577,7 +578,7 @@ k_pass_a(const DP p, const SS* __restrict__ S, const int nf, const int init,
   const int i = act ? i0 : nf - 1;
   const uint4 xi = R[i].x;
   const float4 bi = R[i].b;
-  const unsigned key = K[i];
+  const int ncw = act ? NCW[i] : 0;
   const int phi = MULTI ? phase_of(xi) : 0;
   const float rho0i = p.rho0[phi], c2i = p.c2[phi], ci = p.c0[phi];
   const float rhoi = rho0i + bi.w, prsi = c2i * bi.w, ZL = rhoi * ci;
@@ -607,7 +608,7 @@ k_pass_a(const DP p, const SS* __restrict__ S, const int nf, const int init,
     walk_l(NL + (size_t)(i0 >> 5) * (caps >> 2) * 32 + (threadIdx.x & 31), act ? NC[i] : 0, body);
   }
   float accw = 0.f;
-  if (__any_sync(FULL, act && wnear[key])) {
+  if (__any_sync(FULL, ncw > 0)) {
     {
       auto body = make_body(WR, [&](const uint4& xj, const float4& bj, const unsigned j) {  // (v_w, p_w)
       const Geo g = geometry<DIM>(p, xi, xj);
@@ -618,7 +619,7 @@ k_pass_a(const DP p, const SS* __restrict__ S, const int nf, const int init,
       const float num = fmaf(ZR, vd, (prsi - bj.w) * g.r);
       accw = fmaf(g.f, div_fast(num, ZL + ZR), accw);
       });
-      walk_l(NLW + (size_t)(i0 >> 5) * (capsw >> 2) * 32 + (threadIdx.x & 31), act ? NCW[i] : 0, body);
+      walk_l(NLW + (size_t)(i0 >> 5) * (capsw >> 2) * 32 + (threadIdx.x & 31), ncw, body);
     }
   }
   if (!act) return;
@@ -644,11 +645,8 @@ k_pass_a(const DP p, const SS* __restrict__ S, const int nf, const int init,
 template <int DIM, bool MULTI, bool EXACT>
 __global__ void __launch_bounds__(PB, SPH_MINB)
 k_pass_b(const DP p, const SS* __restrict__ S, const int nf,
-         const float4* __restrict__ A, const XB* __restrict__ R,
-         const unsigned* __restrict__ K, const int* __restrict__ lbF,
-         const float4* __restrict__ WA, const XB* __restrict__ WR,
-         const float4* __restrict__ WN, const int* __restrict__ lbW,
-         const unsigned char* __restrict__ wnear, float4* __restrict__ Bout, float4* __restrict__ ACC,
+         const XB* __restrict__ R, const XB* __restrict__ WR,
+         const float4* __restrict__ WN, float4* __restrict__ Bout, float4* __restrict__ ACC,
          const uint4* __restrict__ NL, const int* __restrict__ NC, const int caps,
          const uint4* __restrict__ NLW, const int* __restrict__ NCW, const int capsw) {
   const int i0 = blockIdx.x * PB + threadIdx.x;
@@ -656,7 +654,7 @@ k_pass_b(const DP p, const SS* __restrict__ S, const int nf,
   const int i = act ? i0 : nf - 1;
   const uint4 xi = R[i].x;
   const float4 bi = R[i].b;
-  const unsigned key = K[i];
+  const int ncw = act ? NCW[i] : 0;
   const int phi = MULTI ? phase_of(xi) : 0;
   const float rho0i = p.rho0[phi], c2i = p.c2[phi], ci = p.c0[phi];
   const float rhoi = rho0i + bi.w, prsi = c2i * bi.w, ZL = rhoi * ci;
@@ -688,7 +686,7 @@ k_pass_b(const DP p, const SS* __restrict__ S, const int nf,
     walk_l(NL + (size_t)(i0 >> 5) * (caps >> 2) * 32 + (threadIdx.x & 31), act ? NC[i] : 0, body);
   }
   KSum wx, wy, wz;
-  if (__any_sync(FULL, act && wnear[key])) {
+  if (__any_sync(FULL, ncw > 0)) {
     const bool pen = (p.pen_mask >> phi) & 1u;
     {
       auto body = make_body(WR, [&](const uint4& xj, const float4& bj, const unsigned j) {
@@ -714,7 +712,7 @@ k_pass_b(const DP p, const SS* __restrict__ S, const int nf,
         }
       }
       });
-      walk_l(NLW + (size_t)(i0 >> 5) * (capsw >> 2) * 32 + (threadIdx.x & 31), act ? NCW[i] : 0, body);
+      walk_l(NLW + (size_t)(i0 >> 5) * (capsw >> 2) * 32 + (threadIdx.x & 31), ncw, body);
     }
   }
   if (!act) return;

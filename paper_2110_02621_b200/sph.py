@@ -15,6 +15,7 @@ FLAG_REINIT = 1
 FLAG_WALL_VEL_MIRROR = 2
 FLAG_NO_GRAPH = 4
 FLAG_WALL_ADAMI_ONLY = 8
+DEFAULT_LIST_SKIN = 0.1   # what sph_create takes for list_skin < 0 (include/sph.h)
 STAGES = ("predict", "sort", "reorder", "wall", "pass_a", "pass_b", "build")
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -35,7 +36,7 @@ class SphParams(C.Structure):
         ("penalty_phase_mask", C.c_uint32), ("free_surface_mask", C.c_uint32),
         ("flags", C.c_uint32), ("max_neighbours", C.c_uint32),
         ("domain_min", C.c_double * 3), ("domain_max", C.c_double * 3),
-        ("wall_osc_amp", C.c_double * 3), ("wall_osc_freq", C.c_double),
+        ("wall_osc_amp", C.c_double * 3), ("wall_osc_freq", C.c_double), ("list_skin", C.c_double),
     ]
 
 
@@ -43,7 +44,7 @@ class SphStats(C.Structure):
     _fields_ = [
         ("t", C.c_double), ("dt", C.c_double), ("steps", C.c_int64), ("n_fluid", C.c_int64),
         ("n_wall", C.c_int64), ("n_pairs", C.c_int64), ("e_kin", C.c_double), ("mass", C.c_double),
-        ("x_front", C.c_double), ("escaped", C.c_int64), ("nonfinite", C.c_int64),
+        ("x_front", C.c_double), ("escaped", C.c_int64), ("nonfinite", C.c_int64), ("rebuilds", C.c_int64),
     ]
 
 
@@ -51,7 +52,7 @@ EXPORTS = (
     "sph_create", "sph_destroy", "sph_set_particles", "sph_set_particles_host", "sph_step",
     "sph_step_dt", "sph_get_fields", "sph_get_fields_host", "sph_get_stats", "sph_get_stats_ex", "sph_set_profiling",
     "sph_get_timings", "sph_num_cells", "sph_debug_cells", "sph_debug_neighbours", "sph_debug_list_check", "sph_probe_pressure", "sph_probe_gauge",
-    "sph_debug_normals", "sph_debug_sigma", "sph_launch_count", "sph_last_error", "sph_debug_step_lists", "sph_debug_fma_peak",
+    "sph_debug_normals", "sph_debug_sigma", "sph_launch_count", "sph_last_error", "sph_debug_step_lists", "sph_debug_fma_peak", "sph_debug_time_pointwise",
 )
 
 _lib = None
@@ -78,11 +79,12 @@ def load():
     L.sph_get_stats.restype = C.c_int; L.sph_get_stats.argtypes = [vp, C.POINTER(SphStats), vp]
     L.sph_get_stats_ex.restype = C.c_int; L.sph_get_stats_ex.argtypes = [vp, C.POINTER(SphStats), i32, vp]
     L.sph_set_profiling.restype = C.c_int; L.sph_set_profiling.argtypes = [vp, i32]
-    L.sph_get_timings.restype = C.c_int; L.sph_get_timings.argtypes = [vp, vp, vp]
+    L.sph_get_timings.restype = C.c_int; L.sph_get_timings.argtypes = [vp, vp, vp, vp]
     L.sph_num_cells.restype = i64; L.sph_num_cells.argtypes = [vp]
     L.sph_debug_cells.restype = C.c_int; L.sph_debug_cells.argtypes = [vp] * 6
     L.sph_debug_neighbours.restype = C.c_int; L.sph_debug_neighbours.argtypes = [vp, vp, vp, i64, vp, vp]
     L.sph_debug_step_lists.restype = C.c_int; L.sph_debug_step_lists.argtypes = [vp, vp, vp, i64, vp, vp]
+    L.sph_debug_time_pointwise.restype = C.c_int; L.sph_debug_time_pointwise.argtypes = [vp, vp, vp]
     L.sph_debug_fma_peak.restype = C.c_int; L.sph_debug_fma_peak.argtypes = [vp, vp]
     L.sph_debug_normals.restype = C.c_int; L.sph_debug_normals.argtypes = [vp, vp, vp]
     L.sph_debug_list_check.restype = C.c_int; L.sph_debug_list_check.argtypes = [vp, vp, vp]
@@ -116,6 +118,7 @@ def make_params(cfg: dict) -> SphParams:
     P.free_surface_mask = cfg.get("free_surface_mask", 1)
     P.flags = cfg.get("flags", FLAG_REINIT | FLAG_WALL_VEL_MIRROR)
     P.max_neighbours = cfg.get("max_neighbours", 0)
+    P.list_skin = cfg.get("list_skin", -1.0)   # < 0: library default
     return P
 
 
@@ -209,7 +212,8 @@ class Sph:
         if check:
             self._ck(rc)
         return dict(t=s.t, dt=s.dt, steps=s.steps, n_fluid=s.n_fluid, n_wall=s.n_wall, npairs=s.n_pairs,
-                    ek=s.e_kin, mass=s.mass, x_front=s.x_front, escaped=s.escaped, nonfinite=s.nonfinite, rc=rc)
+                    ek=s.e_kin, mass=s.mass, x_front=s.x_front, escaped=s.escaped, nonfinite=s.nonfinite,
+                    rebuilds=s.rebuilds, rc=rc)
 
     # -- profiling ---------------------------------------------------------------------------------
     def set_profiling(self, on=True):
@@ -217,9 +221,17 @@ class Sph:
 
     def get_timings(self):
         ms = np.zeros(len(STAGES), np.float32)
-        ns = C.c_int32(0)
-        self._ck(self.L.sph_get_timings(self.ctx, _hp(ms), C.byref(ns)))
+        ns, nr = C.c_int32(0), C.c_int32(0)
+        self._ck(self.L.sph_get_timings(self.ctx, _hp(ms), C.byref(ns), C.byref(nr)))
+        self.last_timing_rebuilds = nr.value
         return dict(zip(STAGES, ms.tolist())), ns.value
+
+    def time_pointwise(self):
+        """sph_debug_time_pointwise: stand-alone density-reinitialisation kernel, integrator kernel (kick + drift +
+        cell hash) and the fused predictor the step runs, ms per launch (state untouched)."""
+        ms = np.zeros(3, np.float32)
+        self._ck(self.L.sph_debug_time_pointwise(self.ctx, _hp(ms), self._st()))
+        return dict(reinit=float(ms[0]), integrator=float(ms[1]), fused_predict=float(ms[2]))
 
     def launch_count(self):
         return self.L.sph_launch_count(self.ctx)

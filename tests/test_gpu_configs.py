@@ -10,7 +10,7 @@ import pytest
 from oracle import orc
 from paper_2110_02621_b200 import inputs, sph
 
-from parity_util import TOL, compare_fields, make_pair
+from parity_util import TOL, acc_tol, compare_fields, extra_bound, make_pair
 
 pytestmark = pytest.mark.gpu
 
@@ -36,6 +36,8 @@ def _steps_and_compare(cfg, nsteps, names=("rho", "p", "acc", "vel", "pos"), lig
     if light_acc_tol is not None:
         assert ph[0] < TOL and max(ph.values()) < light_acc_tol, ("after %d steps" % nsteps, ph)
         e.pop("acc")
+    elif acc_tol(cfg) > TOL:       # declared deviation for H / h > 66 (parity_util.acc_tol)
+        assert e.pop("acc") < acc_tol(cfg), ("after %d steps" % nsteps, ph, acc_tol(cfg))
     assert max(e.values()) < TOL, ("after %d steps" % nsteps, e, ph)
     so, sg = o.stats(), g.get_stats()
     # after steps the two position sets differ in the last bits: pairs at r = 2h to rounding may flip
@@ -46,7 +48,7 @@ def _steps_and_compare(cfg, nsteps, names=("rho", "p", "acc", "vel", "pos"), lig
     assert abs(sg["ek"] - so["ek"]) <= 1e-3 * so["ek"] + 1e-12
     # the lists the passes read hold every float32-contract neighbour (k_build's float16 filter)
     missing, extra, total = g.debug_list_check()
-    assert missing == 0 and extra <= 0.06 * total
+    assert missing == 0 and extra <= extra_bound(cfg) * total
     # probes (readings A29 / A30) on the oracle's own state, sampled points
     from oracle import probes
     fo = o.fields()
@@ -95,7 +97,7 @@ def test_cfg1_moving_walls_full_size():
     sg = g.get_stats()
     assert sg["escaped"] == 0 and sg["nonfinite"] == 0
     missing, extra, total = g.debug_list_check()
-    assert missing == 0 and extra <= 0.06 * total
+    assert missing == 0 and extra <= extra_bound(cfg) * total
 
 
 def test_cfg1_cells_bit_exact_full_size():
