@@ -308,6 +308,7 @@ def run_gpu(args):
     ms = float(sum(a.elapsed_time(b) for a, b in ev))
     ms = max_over_ranks(ms, "cuda")
     st = g.get_stats()
+    st_timed = st
     launches = g.launch_count() - l0        # after the stats read: it adds the rebuild branches the graph replays took
     rebuilds = st["rebuilds"] - r0          # steps of the timed region that rebuilt the cell list and the neighbour lists
     if st["escaped"] or st["nonfinite"]:
@@ -456,7 +457,7 @@ def run_gpu(args):
                        "parallelism": "replicas only" if world > 1 else "1 gpu"},
             "pair_interactions_per_s": pairs_s, "pairs_per_step": fluid_pairs,
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
-            "list_skin": skin, "rebuilds_in_timed_steps": int(rebuilds),
+            "list_skin_max": skin, "list_skin_at_end": st_timed["list_skin"], "rebuilds_in_timed_steps": int(rebuilds),
             "roofline": roofline, "kernels": kern, "stage_ms_per_step": stage_def,
             "stage_ms_per_launch_skin0": stage_ms, "pointwise_standalone_ms": pointwise,
             "cpu_baseline": cpu,

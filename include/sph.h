@@ -89,9 +89,13 @@ typedef struct {
   double list_skin;              /* Verlet skin s: the cell list and the per-particle neighbour lists are built with radius
                                     2h(1 + s) (cell edge 2h(1 + s)) and kept over the following steps until a pair
                                     further apart than that could have come within 2h, i.e. until 2 sum_n max_i |dx_i^n|
-                                    (or that of fluid + walls) exceeds 2 h s; entries beyond 2h add exactly 0.  0 = rebuild
-                                    every step; < 0 = library default (0.1); at most 0.5.  Results do not depend on s
-                                    beyond the order of floating-point sums */
+                                    (or that of fluid + walls) exceeds 2 h s; entries beyond 2h add exactly 0.  The value
+                                    given is the LARGEST skin (it fixes the cell edge); every build takes the skin in
+                                    [0.002, list_skin] that minimises pass cost + build cost / steps between builds for
+                                    the displacement per step seen then (a fluid at rest keeps thin lists for long, a
+                                    violent flow thicker ones for a few steps).  0 = rebuild every step; < 0 = library
+                                    default (0.1); at most 0.5.  Results do not depend on it beyond the order of
+                                    floating-point sums */
 } sph_params;
 
 typedef struct {
@@ -107,6 +111,7 @@ typedef struct {
   int64_t escaped;   /* fluid particles outside [domain_min, domain_max) at the last cell build */
   int64_t nonfinite; /* non-finite positions/velocities seen so far     */
   int64_t rebuilds;  /* cell-list / neighbour-list builds since sph_set_particles (its own included) */
+  double list_skin;  /* skin of the lists in use (adaptive, within [0.002, sph_params.list_skin]) */
 } sph_stats;
 
 /* Stages timed by sph_set_profiling (indices into sph_get_timings' array). */

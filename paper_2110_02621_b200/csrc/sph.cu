@@ -642,7 +642,9 @@ int sph_create(const sph_params* prm, sph_ctx** out) {
     const double err_expanded = 16.0 * u * R2 + 8.0 * u * R * rl;
     const double err_diff = 16.0 * u * R * rl;
     d.exact_filter = 2.0 * err_expanded > 0.08 * rc * rc ? 1 : 0;
-    d.rc2m = (float)(rl * rl + 2.0 * (d.exact_filter ? err_diff : err_expanded));
+    d.marg32 = 2.0 * (d.exact_filter ? err_diff : err_expanded);
+    d.marg16 = 2.0 * err_diff / (h * h);
+    d.rc2m = (float)(rl * rl + d.marg32);   // thresholds at the largest skin: the first build's (SS::rl2m / thr_h2 later)
     {  // float16 filter of k_build (sph_pair.cuh): threshold rounded up to the next half; the margin analysis
        // there is relative to the radius, so the 4.08 of r = 2 becomes 4.08 (1 + s)^2 at the list radius
       d.inv_h = (float)(1.0 / h);
@@ -655,7 +657,7 @@ int sph_create(const sph_params* prm, sph_ctx** out) {
   d.gamma_p = (float)prm->penalty_strength;
   d.pen_mask = (prm->flags & SPH_FLAG_WALL_ADAMI_ONLY) ? 0u : prm->penalty_phase_mask; d.fs_mask = prm->free_surface_mask; d.flags = prm->flags;
   d.skin = skin;
-  d.skin_budget = 2.0 * h * skin * (1.0 - 1e-6);
+  d.skin_min = std::min(skin, 0.002);
   // contract grid (reading A24: cell edge 2h(1 + 2^-10)) and the step's grid (cell edge that times 1 + s)
   d.ox = (float)prm->domain_min[0]; d.oy = (float)prm->domain_min[1]; d.oz = (float)prm->domain_min[2];
   for (int k = 0; k < 3; ++k) {
@@ -746,6 +748,14 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
   if (rc) return c->err.find("out of memory") != std::string::npos ? SPH_ENOMEM : SPH_ECUDA;
   c->IDcur = c->ID0; c->IDnext = c->ID1;
   CK(cudaMemsetAsync(c->S, 0, sizeof(SS), st));
+  {  // the first build takes the largest skin; k_predict adapts it from the displacements it sees
+    SS h0;
+    memset(&h0, 0, sizeof(h0));
+    h0.skin_cur = c->dp.skin; h0.budget = 2.0 * c->dp.hD * c->dp.skin * (1.0 - 1e-6);
+    h0.rl2m = c->dp.rc2m; h0.thr_h2 = c->dp.thr_h2;
+    CK(cudaMemcpyAsync(c->S, &h0, sizeof(SS), cudaMemcpyHostToDevice, st));
+    CK(cudaStreamSynchronize(st));
+  }
   CK(cudaMemsetAsync(c->A + nf, 0, 16 * sizeof(float4), st));   // padding read by the chunked candidate loads
   CK(cudaMemsetAsync(c->WA + nw, 0, 16 * sizeof(float4), st));
   CK(cudaMemsetAsync(c->ACC, 0, sizeof(float4) * std::max(nf, 1), st));
@@ -922,6 +932,7 @@ int sph_get_stats_ex(sph_ctx* c, sph_stats* out, int32_t with_pairs, void* strea
   }
   out->escaped = (int64_t)hs.escaped; out->nonfinite = (int64_t)hs.nonfinite;
   out->rebuilds = (int64_t)hs.rebuilds + 1;  // + the set-up's
+  out->list_skin = hs.skin_cur;
   {  // rebuild branches taken inside graph replays: their kernels were launched by the graph, count them now
     const int64_t in_graph = (int64_t)hs.rebuilds - c->direct_rebuilds;
     if (in_graph > c->graph_rebuilds_counted) {

@@ -1,6 +1,8 @@
 // sph_aux.cuh — loading, time step, predictor, reorder, wall normals and near-wall flags.
 // Included by sph.cu only.  Citations: PAPER.md:<line>; readings Axx: DESIGN.md §3.
 #pragma once
+#include <cuda_fp16.h>
+
 #include "sph_common.cuh"
 
 constexpr unsigned RES_MID = (512u << 22) | (512u << 12) | (512u << 2);  // zero residual on every axis
@@ -248,17 +250,37 @@ k_predict(DP p, SS* __restrict__ S, int nf, const XB* __restrict__ R, float4* __
   __threadfence();
   const double dstep = sqrt((double)__uint_as_float(atomicMax(&S->dmax2_bits, 0u))) + 2.0 * p.Q;
   double disp = S->disp + dstep;
-  double dw2 = 0.0;
+  double dw2 = 0.0, dws2 = 0.0;
   for (int k = 0; k < 3; ++k) {
-    const double d = p.Q * (double)(S->sq[k] - S->sq_build[k]);
+    const double d = p.Q * (double)(S->sq[k] - S->sq_build[k]), e = p.Q * (double)(S->sq[k] - S->sq_prev[k]);
     dw2 += d * d;
+    dws2 += e * e;
+    S->sq_prev[k] = S->sq[k];
   }
-  const int rb = (p.skin <= 0.0 || 2.0 * disp > p.skin_budget || disp + sqrt(dw2) > p.skin_budget) ? 1 : 0;
+  // the skin the next build should take: optimum for this step's displacement, 20 % head room
+  const double delta = (dstep + sqrt(dws2)) / p.hD, beta = 0.65;
+  double snext = 1.2 * (-2.0 * beta * delta + sqrt(4.0 * beta * beta * delta * delta + 12.0 * beta * delta)) / 6.0;
+  snext = fmin(fmax(snext, p.skin_min), p.skin);
+  const int since = S->since + 1;
+  const bool stale = 2.0 * disp > S->budget || disp + sqrt(dw2) > S->budget;   // a pair beyond the list radius may be within 2h
+  const bool loose = S->skin_cur > 1.5 * snext + 0.004 && since >= 4;          // the lists carry far more entries than they need to
+  const int rb = (p.skin <= 0.0 || stale || loose) ? 1 : 0;
   if (rb) {
     disp = 0.0;
     for (int k = 0; k < 3; ++k) S->sq_build[k] = S->sq[k];
     S->rebuilds += 1;
+    if (p.skin > 0.0) {
+      const double rl = 2.0 * p.hD * (1.0 + snext);
+      S->skin_cur = snext;
+      S->budget = 2.0 * p.hD * snext * (1.0 - 1e-6);
+      S->rl2m = __double2float_ru(rl * rl + p.marg32);
+      const double thr = 4.08 * (1.0 + snext) * (1.0 + snext) + p.marg16;
+      __half th = __double2half(thr);
+      if ((double)__half2float(th) < thr) th = __ushort_as_half((unsigned short)(__half_as_ushort(th) + 1));
+      S->thr_h2 = (unsigned)__half_as_ushort(th) * 0x10001u;
+    }
   }
+  S->since = rb ? 0 : since;
   S->disp = disp;
   S->rebuild = rb;
   S->dmax2_bits = 0u;

@@ -43,8 +43,10 @@ struct DP {
   double wamp[3], womega;  // NEXT-1: wall motion x_w(t) = x_w(0) + wamp sin(womega t); womega = 0: static walls
   // Verlet skin: the lists are built with radius 2h(1 + skin) on a cell grid of that edge
   // and kept while 2 * (fluid displacement bound) and (fluid + wall displacement) stay below skin_budget
-  double skin;         // s >= 0; 0: the lists are rebuilt every step
-  double skin_budget;  // 2 h s (1 - 1e-6) in metres
+  double skin;         // largest skin s_max >= 0 (the cell edge is 2h(1 + s_max)); 0: the lists are rebuilt every step
+  double skin_min;     // smallest skin the adaptive choice takes
+  double marg32;       // rounding margin of the float32 filter forms on r^2 (m^2): threshold = rl^2 + marg32
+  double marg16;       // float32-image part of the float16 filter's margin on r^2 / h^2: threshold = 4.08 (rl / 2h)^2 + marg16
 };
 
 // Per-particle record gathered by the pair bodies: one 32-byte sector, one 256-bit load.
@@ -76,7 +78,17 @@ struct SS {
   unsigned long long escaped, nonfinite;
   int dt_underflow;
   int list_overflow;     // largest neighbour count seen above the list capacity (0 = none); sticky
-  // Verlet skin: written by k_predict's last block
+  // Verlet skin: written by k_predict's last block (and by sph_set_particles for the first build).
+  // The skin is ADAPTIVE: every build takes the skin that minimises (pass cost + build cost / steps between builds)
+  // for the displacement per step seen at that time, s = (-2 b d + sqrt(4 b^2 d^2 + 12 b d)) / 6 with d = max_i |dx_i| / h
+  // and b = build cost / pass cost (0.65 measured), within [skin_min, skin]; k_build / k_wall_build read the
+  // thresholds of the current skin from here.
+  double skin_cur;         // skin of the lists in use
+  double budget;           // 2 h skin_cur (1 - 1e-6): the lists hold every pair within 2h while 2 disp (or disp + wall displacement) stays below it
+  float rl2m;              // float32 filter threshold of the current skin: (2h(1 + skin_cur))^2 + marg32
+  unsigned thr_h2;         // float16 filter threshold (half2, both halves)
+  int since;               // steps since the last build
+  int sq_prev[3];          // wall displacement of the previous step (units of Q)
   double disp;             // sum over the steps since the last list build of max_i |dx_i| (metres): a bound on
                            // every fluid particle's displacement since then
   int sq_build[3];         // wall displacement (units of Q) at the last list build

@@ -193,9 +193,10 @@ __device__ __forceinline__ float filter_t(const float4& ai, const float m2x, con
 template <int DIM, bool EXACT, bool STAGE, class Sink>
 __device__ __forceinline__ void walk_f(const DP& p, const float4* __restrict__ A, const int* __restrict__ lb,
                                        const bool act, const float4 ai, const int cx, const int cy,
-                                       const int cz, HTile* __restrict__ tile, const HCtx& hc, Sink& sink) {
+                                       const int cz, HTile* __restrict__ tile, const HCtx& hc, Sink& sink,
+                                       const float rl2m, const unsigned thr_h2) {
   const float m2x = -2.0f * ai.x, m2y = -2.0f * ai.y, m2z = -2.0f * ai.z;
-  const float thr = EXACT ? p.rc2m : p.rc2m - ai.w;
+  const float thr = EXACT ? rl2m : rl2m - ai.w;
   const int lane = threadIdx.x & 31;
   constexpr int NR = DIM == 3 ? 9 : 3;
   int ry = -1, rz = DIM == 3 ? -1 : 0;
@@ -260,10 +261,10 @@ __device__ __forceinline__ void walk_f(const DP& p, const float4* __restrict__ A
             }
           }
           static_assert(CHS == 8, "four pair records per chunk");
-          sink.template push2<0>(r2[0], p.thr_h2, rem, ok0, j0);
-          sink.template push2<2>(r2[1], p.thr_h2, rem, 1, j0 + 2);
-          sink.template push2<4>(r2[2], p.thr_h2, rem, 1, j0 + 4);
-          sink.template push2<6>(r2[3], p.thr_h2, rem, 1, j0 + 6);
+          sink.template push2<0>(r2[0], thr_h2, rem, ok0, j0);
+          sink.template push2<2>(r2[1], thr_h2, rem, 1, j0 + 2);
+          sink.template push2<4>(r2[2], thr_h2, rem, 1, j0 + 4);
+          sink.template push2<6>(r2[3], thr_h2, rem, 1, j0 + 6);
           sink.after_chunk(CHS);
         }
       }
@@ -297,7 +298,7 @@ __device__ __forceinline__ void walk_q(const DP& p, const float4* __restrict__ A
                                        const bool act, const float4 ai, const int cx, const int cy,
                                        const int cz, unsigned* __restrict__ q, Body& body) {
   QueueSink<Body> sink(q, body);
-  walk_f<DIM, EXACT, false>(p, A, lb, act, ai, cx, cy, cz, nullptr, HCtx{}, sink);
+  walk_f<DIM, EXACT, false>(p, A, lb, act, ai, cx, cy, cz, nullptr, HCtx{}, sink, p.rc2m, p.thr_h2);
 }
 
 // List walk: every lane runs over its own column of the warp's neighbour groups; the loop is
@@ -457,17 +458,19 @@ k_build(const DP p, SS* __restrict__ S, const int nf, const float4* __restrict__
     hc.bad = act && !(fmaxf(fabsf(x), fmaxf(fabsf(y), fabsf(z))) < 15.9f);
     hc.xi = h2(x, x); hc.yi = h2(y, y); hc.zi = h2(z, z);
   }
+  const float rl2m = S->rl2m;          // thresholds of the skin this build takes (adaptive: SS, k_predict)
+  const unsigned thr_h2 = S->thr_h2;
   int n = 0, nw = 0;
   {
     ListSink sink(qs + threadIdx.x, NL + (size_t)(i0 >> 5) * (caps >> 2) * 32 + (threadIdx.x & 31), caps >> 2);
-    walk_f<DIM, EXACT, true>(p, A, lbF, act, ai, cx, cy, cz, tiles + (threadIdx.x >> 5), hc, sink);
+    walk_f<DIM, EXACT, true>(p, A, lbF, act, ai, cx, cy, cz, tiles + (threadIdx.x >> 5), hc, sink, rl2m, thr_h2);
     n = sink.n;
   }
   // fluid-wall lists (same filter over the static wall arrays) for the warps that have a wall
   // particle in a stencil: both pair passes read them, so the wall candidate walk is also paid once
   if (__any_sync(FULL, act && wnear[key])) {
     ListSink sink(qs + threadIdx.x, NLW + (size_t)(i0 >> 5) * (capsw >> 2) * 32 + (threadIdx.x & 31), capsw >> 2);
-    walk_f<DIM, EXACT, true>(p, WA, lbW, act, ai, cx, cy, cz, tiles + (threadIdx.x >> 5), hc, sink);
+    walk_f<DIM, EXACT, true>(p, WA, lbW, act, ai, cx, cy, cz, tiles + (threadIdx.x >> 5), hc, sink, rl2m, thr_h2);
     nw = sink.n;
   }
   if (act) {
@@ -499,7 +502,7 @@ k_wall_build(const DP p, SS* __restrict__ S, const int nw, const float4* __restr
   int cx, cy, cz;
   cell_of_key(p, WK[w], cx, cy, cz);
   ListSink sink(qs + threadIdx.x, col, capsf >> 2);
-  walk_f<DIM, EXACT, false>(p, A, lbF, act, ai, cx, cy, cz, nullptr, HCtx{}, sink);
+  walk_f<DIM, EXACT, false>(p, A, lbF, act, ai, cx, cy, cz, nullptr, HCtx{}, sink, S->rl2m, S->thr_h2);
   if (act) {
     NCF[w] = min(sink.n, capsf);
     if (sink.n > capsf) atomicMax(&S->list_overflow, sink.n);

@@ -44,7 +44,7 @@ class SphStats(C.Structure):
     _fields_ = [
         ("t", C.c_double), ("dt", C.c_double), ("steps", C.c_int64), ("n_fluid", C.c_int64),
         ("n_wall", C.c_int64), ("n_pairs", C.c_int64), ("e_kin", C.c_double), ("mass", C.c_double),
-        ("x_front", C.c_double), ("escaped", C.c_int64), ("nonfinite", C.c_int64), ("rebuilds", C.c_int64),
+        ("x_front", C.c_double), ("escaped", C.c_int64), ("nonfinite", C.c_int64), ("rebuilds", C.c_int64), ("list_skin", C.c_double),
     ]
 
 
@@ -213,7 +213,7 @@ class Sph:
             self._ck(rc)
         return dict(t=s.t, dt=s.dt, steps=s.steps, n_fluid=s.n_fluid, n_wall=s.n_wall, npairs=s.n_pairs,
                     ek=s.e_kin, mass=s.mass, x_front=s.x_front, escaped=s.escaped, nonfinite=s.nonfinite,
-                    rebuilds=s.rebuilds, rc=rc)
+                    rebuilds=s.rebuilds, list_skin=s.list_skin, rc=rc)
 
     # -- profiling ---------------------------------------------------------------------------------
     def set_profiling(self, on=True):

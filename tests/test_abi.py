@@ -31,7 +31,7 @@ def test_library_builds_and_exports_every_declared_symbol():
 def test_struct_layouts_match_header():
     # sph_params: 2 int32 + 2 + 4 + 4 + 3 + 3 + 1 + 1 + 1 doubles + 4 uint32 + 6 doubles
     assert ctypes.sizeof(sph.SphParams) == 8 + 8 * 19 + 16 + 8 * 6 + 8 * 4 + 8   # + wall_osc_amp[3], wall_osc_freq, list_skin
-    assert ctypes.sizeof(sph.SphStats) == 8 * 12
+    assert ctypes.sizeof(sph.SphStats) == 8 * 13
 
 
 def test_product_does_not_import_oracle():
