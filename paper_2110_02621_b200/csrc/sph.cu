@@ -303,7 +303,7 @@ int rebuild_body(sph_ctx* c, cudaStream_t st, int init, Prof& pf) {
     LAUNCH(k_reorder, std::max(cdiv(nf, 256), cdiv(c->ncell + 1, 256)), 256, st, c->dp, nf, vs, c->TX, c->TB, c->IDcur,
            c->R0, c->A, c->IDnext, ks, (int)c->ncell, c->lbF);
   } else {
-    LAUNCH(k_cell_bounds, cdiv(c->ncell + 1, 256), 256, st, ks, nf, (int)c->ncell, c->lbF);
+    LAUNCH(k_cell_bounds, cdiv(c->ncell + 1, 256), 256, st, ks, nf, (int)c->ncell, c->lbF, c->dp.sub_bits);
   }
   if (wall_branch) CK(cudaStreamWaitEvent(st, c->evJoin, 0));
   pf.mark(3);  // end reorder
@@ -499,7 +499,7 @@ int contract_order(sph_ctx* c, cudaStream_t st, int n, const float4* G, const un
                    unsigned* IDout, int* lb) {
   const int nc = (int)c->ncellC;
   if (n == 0) {
-    LAUNCH(k_cell_bounds, cdiv(nc + 1, 256), 256, st, c->dKa, 0, nc, lb);
+    LAUNCH(k_cell_bounds, cdiv(nc + 1, 256), 256, st, c->dKa, 0, nc, lb, 0);
     return SPH_OK;
   }
   unsigned *ks, *vs;
@@ -511,7 +511,7 @@ int contract_order(sph_ctx* c, cudaStream_t st, int n, const float4* G, const un
   rc = radix_sort(c, st, n, bits_for(c->ncellC), ks, vs, k2, v2, &ks, &vs);
   if (rc) return rc;
   LAUNCH(k_dbg_gather, cdiv(n, 256), 256, st, n, vs, G, ID, Gout, IDout);
-  LAUNCH(k_cell_bounds, cdiv(nc + 1, 256), 256, st, ks, n, nc, lb);
+  LAUNCH(k_cell_bounds, cdiv(nc + 1, 256), 256, st, ks, n, nc, lb, 0);
   return SPH_OK;
 }
 
@@ -682,7 +682,18 @@ int sph_create(const sph_params* prm, sph_ctx** out) {
   c->dpC = d;
   set_grid(c->dpC, edgeC, &c->ncellC);
   if (c->ncell >= (1ll << 31) - 2 || c->ncellC >= (1ll << 31) - 2) { delete c; return SPH_EINVAL; }
-  c->cell_bits = bits_for(c->ncell);
+  // sub-cell Morton bits in the sort key (possible when the lists are kept, skin > 0: the contract's id order inside
+  // a cell is then produced on demand by contract_view).  Measured (profiles/r02_README.md): 1 or 2 bits per axis
+  // change the pair passes by less than 1 % and cost a radix pass, so the default is 0.
+  d.sub_bits = 0;
+  if (skin > 0.0) {
+    int b = 0;
+    if (getenv("SPH_SUB_BITS")) b = atoi(getenv("SPH_SUB_BITS"));   // measurement switch (profiles/): not part of the interface
+    while (b > 0 && bits_for(c->ncell) + b * prm->dim > 31) --b;
+    d.sub_bits = b * prm->dim;
+  }
+  c->dpC.sub_bits = 0;
+  c->cell_bits = bits_for(c->ncell) + d.sub_bits;
   c->multi = prm->n_phases > 1;
   *out = c;
   return SPH_OK;
@@ -794,7 +805,7 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
            (const unsigned*)nullptr, -1, (int*)nullptr);
     CK(cudaMemcpyAsync(c->WK, ks, sizeof(unsigned) * nw, cudaMemcpyDeviceToDevice, st));
     LAUNCH(k_image, cdiv(nw, 256), 256, st, c->dp, nw, c->WR, c->WG);
-    LAUNCH(k_cell_bounds, cdiv(c->ncell + 1, 256), 256, st, ks, nw, (int)c->ncell, c->lbW);
+    LAUNCH(k_cell_bounds, cdiv(c->ncell + 1, 256), 256, st, ks, nw, (int)c->ncell, c->lbW, c->dp.sub_bits);
     if (c->prm.dim == 3) LAUNCH(k_normals<3>, cdiv(nw, 128), 128, st, c->dp, nw, c->WR, c->WK, c->lbW, c->WN);
     else LAUNCH(k_normals<2>, cdiv(nw, 128), 128, st, c->dp, nw, c->WR, c->WK, c->lbW, c->WN);
     if (c->moving) {
@@ -802,7 +813,7 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
       LAUNCH(k_gatherx, cdiv(nw, 256), 256, st, nw, vs, c->WX0, c->WXB);
     }
   } else {
-    LAUNCH(k_cell_bounds, cdiv(c->ncell + 1, 256), 256, st, c->keyA, 0, (int)c->ncell, c->lbW);
+    LAUNCH(k_cell_bounds, cdiv(c->ncell + 1, 256), 256, st, c->keyA, 0, (int)c->ncell, c->lbW, 0);
   }
   LAUNCH(k_wnear, cdiv(c->ncell, 256), 256, st, c->dp, (int)c->ncell, c->lbW, c->wnear);
   CK(cudaStreamSynchronize(st));  // wid host buffer / idx reuse

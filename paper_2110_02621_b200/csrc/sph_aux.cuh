@@ -32,7 +32,7 @@ __global__ void k_load(DP p, int n, int is_wall, const int* __restrict__ idx, co
     TB[i] = make_float4(vel[3 * o], vel[3 * o + 1], p.dim == 3 ? vel[3 * o + 2] : 0.0f, drho);
   }
   ID[i] = (unsigned)o;
-  keys[i] = cell_key(p, fx_image(x.x, p.O[0], p.Q), fx_image(x.y, p.O[1], p.Q),
+  keys[i] = sort_key(p, fx_image(x.x, p.O[0], p.Q), fx_image(x.y, p.O[1], p.Q),
                      p.dim == 3 ? fx_image(x.z, p.O[2], p.Q) : 0.0f);
   vals[i] = (unsigned)i;
 }
@@ -68,7 +68,7 @@ k_wall_shift(DP p, const SS* __restrict__ S, int nw, const uint4* __restrict__ X
   if (p.dim == 3) x.z += (unsigned)S->sq[2];
   TX[i] = x;
   TB[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-  keys[i] = cell_key(p, fx_image(x.x, p.O[0], p.Q), fx_image(x.y, p.O[1], p.Q),
+  keys[i] = sort_key(p, fx_image(x.x, p.O[0], p.Q), fx_image(x.y, p.O[1], p.Q),
                      p.dim == 3 ? fx_image(x.z, p.O[2], p.Q) : 0.0f);
   vals[i] = (unsigned)i;
 }
@@ -88,7 +88,7 @@ k_reorder(DP p, int n, const unsigned* __restrict__ vals, const uint4* __restric
     int lo = 0, hi = n;
     while (lo < hi) {
       const int mid = (lo + hi) >> 1;
-      if (keys[mid] < (unsigned)s) lo = mid + 1; else hi = mid;
+      if ((keys[mid] >> p.sub_bits) < (unsigned)s) lo = mid + 1; else hi = mid;
     }
     lb[s] = lo;
   }
@@ -231,7 +231,7 @@ k_predict(DP p, SS* __restrict__ S, int nf, const XB* __restrict__ R, float4* __
       bool out = gx < p.dmin[0] || gx >= p.dmax[0] || gy < p.dmin[1] || gy >= p.dmax[1];
       if (p.dim == 3) out = out || gz < p.dmin[2] || gz >= p.dmax[2];
       if (out || !fin) atomicAdd(&S->escaped, 1ull);
-      keys[i] = cell_key(p, gx, gy, gz);
+      keys[i] = sort_key(p, gx, gy, gz);
       vals[i] = (unsigned)i;
     }
     B[i] = b;
@@ -307,7 +307,7 @@ __global__ void k_normals(DP p, int nw, const XB* __restrict__ WR, const unsigne
   const int w = blockIdx.x * blockDim.x + threadIdx.x;
   if (w >= nw) return;
   const uint4 xi = WR[w].x;
-  const unsigned key = WK[w];
+  const unsigned key = WK[w] >> p.sub_bits;
   const unsigned row = key / (unsigned)p.nx;
   const int cx = (int)(key - row * (unsigned)p.nx), cz = (int)(row / (unsigned)p.ny),
             cy = (int)(row - (unsigned)cz * (unsigned)p.ny);

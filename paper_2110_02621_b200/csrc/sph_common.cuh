@@ -43,6 +43,8 @@ struct DP {
   double wamp[3], womega;  // NEXT-1: wall motion x_w(t) = x_w(0) + wamp sin(womega t); womega = 0: static walls
   // Verlet skin: the lists are built with radius 2h(1 + skin) on a cell grid of that edge
   // and kept while 2 * (fluid displacement bound) and (fluid + wall displacement) stay below skin_budget
+  int sub_bits;        // sort key = (cell id << sub_bits) | Morton code of the position inside the cell (sub_bits / dim bits
+                       // per axis; 0 when skin = 0, where the order inside a cell is the contract's id order, reading A25)
   double skin;         // largest skin s_max >= 0 (the cell edge is 2h(1 + s_max)); 0: the lists are rebuilt every step
   double skin_min;     // smallest skin the adaptive choice takes
   double marg32;       // rounding margin of the float32 filter forms on r^2 (m^2): threshold = rl^2 + marg32
@@ -144,6 +146,28 @@ __device__ __forceinline__ float4 centred_image(const DP& p, const uint4& x) {
   const float b = (float)(fx_to_double(x.y, p.O[1], p.Q) - p.C[1]);
   const float c = p.dim == 3 ? (float)(fx_to_double(x.z, p.O[2], p.Q) - p.C[2]) : 0.0f;
   return make_float4(a, b, c, fmaf(c, c, fmaf(b, b, a * a)));
+}
+
+// Sort key of the step's cell list: the cell id of reading A24's hash on the step's grid, and below it the Morton code
+// of the position inside the cell, so that particles that are neighbours in memory are neighbours in space: the
+// lanes of a warp then gather from few cache lines at a time (profiles/r02).
+__device__ __forceinline__ unsigned spread_bits(unsigned v, const int dim) {  // v < 8: bit k -> bit k * dim
+  return dim == 3 ? ((v & 1u) | ((v & 2u) << 2) | ((v & 4u) << 4)) : ((v & 1u) | ((v & 2u) << 1) | ((v & 4u) << 2));
+}
+__device__ __forceinline__ unsigned sort_key(const DP& p, float x, float y, float z) {
+  const float ux = __fmul_rn(__fsub_rn(x, p.ox), p.inv_edge), uy = __fmul_rn(__fsub_rn(y, p.oy), p.inv_edge);
+  const float uz = p.dim == 3 ? __fmul_rn(__fsub_rn(z, p.oz), p.inv_edge) : 0.0f;
+  const float fx = fminf(fmaxf(floorf(ux), 0.0f), (float)(p.nx - 1)), fy = fminf(fmaxf(floorf(uy), 0.0f), (float)(p.ny - 1));
+  const float fz = p.dim == 3 ? fminf(fmaxf(floorf(uz), 0.0f), (float)(p.nz - 1)) : 0.0f;
+  unsigned key = (unsigned)(((int)fz * p.ny + (int)fy) * p.nx + (int)fx);
+  if (p.sub_bits) {
+    const int b = p.sub_bits / p.dim;
+    const float sc = (float)(1 << b), top = sc - 1.0f;
+    const unsigned sx = (unsigned)fminf(fmaxf((ux - fx) * sc, 0.0f), top), sy = (unsigned)fminf(fmaxf((uy - fy) * sc, 0.0f), top);
+    const unsigned sz = p.dim == 3 ? (unsigned)fminf(fmaxf((uz - fz) * sc, 0.0f), top) : 0u;
+    key = (key << p.sub_bits) | spread_bits(sx, p.dim) | (spread_bits(sy, p.dim) << 1) | (p.dim == 3 ? spread_bits(sz, 3) << 2 : 0u);
+  }
+  return key;
 }
 
 __device__ __forceinline__ unsigned cell_key(const DP& p, float x, float y, float z) {

@@ -139,13 +139,13 @@ k_radix_scatter(const unsigned* __restrict__ keys, const unsigned* __restrict__ 
 // cells of an x-row of the stencil are one contiguous range [lb[c0], lb[c1+1])).  One thread per
 // cell, binary search in the sorted keys (the tank may be mostly dry: no serial gap filling).
 __global__ void __launch_bounds__(256)
-k_cell_bounds(const unsigned* __restrict__ keys, int n, int ncell, int* __restrict__ lb) {
+k_cell_bounds(const unsigned* __restrict__ keys, int n, int ncell, int* __restrict__ lb, int sub_bits) {
   const int c = blockIdx.x * 256 + threadIdx.x;
   if (c > ncell) return;
   int lo = 0, hi = n;
   while (lo < hi) {
     const int mid = (lo + hi) >> 1;
-    if (keys[mid] < (unsigned)c) lo = mid + 1; else hi = mid;
+    if ((keys[mid] >> sub_bits) < (unsigned)c) lo = mid + 1; else hi = mid;
   }
   lb[c] = lo;
 }
