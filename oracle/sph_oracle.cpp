@@ -10,7 +10,7 @@
 // Every function cites the passage of /root/reference/PAPER.md it follows
 // (PAPER.md:<line>, equation number).  Where the paper is silent or garbled the
 // reading is the one listed in DESIGN.md ("Readings", ids A1..A28 follow
-// SURVEY.md §8(c)).
+// SURVEY.md §8(c); A13b, A29-A32 were added by the build).
 //
 // Pins (tests/test_oracle_pins.py) and what they fix:
 //   kernel W, W'          — unit integral, finite difference           (P1)
@@ -26,6 +26,12 @@
 //   penalty               — closed form of reading A8/A9               (P15)
 //   normals               — flat wall / corner / middle layer          (P16)
 //   mass, whole step      — hydrostatic column relaxes to rho g (H-z)  (P5,P17)
+//   step dispatch         — which phase gets Eq. 2.17 / 2.18, continuity / summation, whose neighbours
+//                           count in sigma: densities after a dt = 0 two-phase step by hand       (P23)
+//   stats                 — E_k = 1/2 M |v|^2, mass, x_front closed forms                          (P24)
+//   sigma of pass A       — lattice constant after a step                                         (P25)
+//   two-phase tank X1     — stays at rest under reading A13b, not without it   (P26)
+//   wall extensions       — without them air leaves the tank                   (P27)
 // PARITY UNPINNED (fixed by DESIGN.md readings only, no external pin exists):
 //   wall velocity mirror (A6), step ordering and two wall passes (A16),
 //   per-pair wall density (A5), penalty scaling (A8), unequal-c solver (A3;

@@ -85,10 +85,17 @@ struct sph_ctx {
   cudaStream_t wstream = nullptr;
   cudaEvent_t evFork = nullptr, evJoin = nullptr;
   std::map<void*, size_t> cap_bytes;  // dalloc: capacity of the buffer behind each pointer member
-  float *hpos = nullptr, *hvel = nullptr, *hrho = nullptr;  // staging of sph_set_particles_host
-  int32_t* htagd = nullptr;
-  float* hout = nullptr;   // staging of sph_get_fields_host
-  int* hidx = nullptr;     // caller indices of one class during sph_set_particles
+  // DEVICE staging of the host-pointer entry points (caller order), kept across calls
+  float *stage_pos = nullptr, *stage_vel = nullptr, *stage_rho = nullptr;
+  int32_t* stage_tag = nullptr;
+  float* stage_out = nullptr;
+  int* class_idx = nullptr;   // device: caller indices of one class during sph_set_particles
+  // PINNED host bounce buffer of the host-pointer entry points: pageable caller memory goes through it in two
+  // halves (the copy of one half overlaps the memcpy of the other), so their speed does not depend on the
+  // caller pinning its arrays; memory that is already pinned or registered is copied directly
+  char* pin = nullptr;
+  size_t pin_bytes = 0;
+  cudaEvent_t pin_ev[2] = {nullptr, nullptr};
   // one step captured as a CUDA graph (launch-bound small configurations); rebuilt after sph_set_particles
   cudaGraphExec_t gexec = nullptr;
   cudaStream_t cap_stream = nullptr, cap_stream2 = nullptr;
@@ -173,7 +180,7 @@ void free_all(sph_ctx* c) {
   void* ptrs[] = {c->R0, c->R1, c->TX, c->A, c->TB, c->ACC, c->SIG, c->DRHO, c->NL, c->NC, c->NLW, c->NCW, c->NLF, c->NCF, c->ID0, c->ID1,
                   c->keyA, c->valA, c->keyB, c->valB, c->hist, c->rowsum, c->lbF, c->lbW, c->WR,
                   c->WA, c->WN, c->WG, c->WK, c->WID, c->wnear, c->S, c->dt_seq, c->stat,
-                  c->hpos, c->hvel, c->hrho, c->htagd, c->hout, c->hidx,
+                  c->stage_pos, c->stage_vel, c->stage_rho, c->stage_tag, c->stage_out, c->class_idx,
                   c->WX0, c->WXB, c->WN0, c->WID0, c->dKa, c->dVa, c->dKb, c->dVb, c->dID, c->dWID, c->dG, c->dWG, c->dlbF, c->dlbW, c->WkeyA, c->WkeyB, c->WvalA, c->WvalB,
                   c->WTX, c->WTB, c->Whist, c->Wrowsum};
   for (void* p : ptrs)
@@ -185,6 +192,8 @@ void free_all(sph_ctx* c) {
   if (c->evFork) cudaEventDestroy(c->evFork);
   if (c->evJoin) cudaEventDestroy(c->evJoin);
   if (c->wstream) cudaStreamDestroy(c->wstream);
+  if (c->pin) cudaFreeHost(c->pin);
+  for (int k = 0; k < 2; ++k) if (c->pin_ev[k]) cudaEventDestroy(c->pin_ev[k]);
 }
 
 // Digits of 9 bits when that saves a pass over 8-bit digits (sph_sort.cuh).
@@ -537,6 +546,66 @@ int contract_view(sph_ctx* c, cudaStream_t st, View* v) {
   return SPH_OK;
 }
 
+bool is_pinned(const void* p) {
+  cudaPointerAttributes a;
+  if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+  return a.type == cudaMemoryTypeHost || a.type == cudaMemoryTypeManaged;
+}
+
+int pin_init(sph_ctx* c) {
+  if (c->pin) return SPH_OK;
+  const size_t bytes = (size_t)32 << 20;
+  if (cudaMallocHost((void**)&c->pin, bytes) != cudaSuccess) { cudaGetLastError(); c->pin = nullptr; c->err = "pinned staging allocation failed"; return SPH_ENOMEM; }
+  c->pin_bytes = bytes;
+  for (int k = 0; k < 2; ++k) CK(cudaEventCreateWithFlags(&c->pin_ev[k], cudaEventDisableTiming));
+  return SPH_OK;
+}
+
+// host -> device / device -> host through the pinned bounce buffer (or directly when the caller's memory is pinned)
+int h2d(sph_ctx* c, void* dst, const void* src, size_t bytes, cudaStream_t st) {
+  if (!bytes) return SPH_OK;
+  if (is_pinned(src)) { CK(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, st)); return SPH_OK; }
+  int rc = pin_init(c);
+  if (rc) return rc;
+  const size_t half = c->pin_bytes / 2;
+  int k = 0;
+  for (size_t off = 0; off < bytes; off += half, k ^= 1) {
+    const size_t m = std::min(half, bytes - off);
+    CK(cudaEventSynchronize(c->pin_ev[k]));  // the previous copy out of this half is done
+    memcpy(c->pin + k * half, (const char*)src + off, m);
+    CK(cudaMemcpyAsync((char*)dst + off, c->pin + k * half, m, cudaMemcpyHostToDevice, st));
+    CK(cudaEventRecord(c->pin_ev[k], st));
+  }
+  return SPH_OK;
+}
+
+int d2h(sph_ctx* c, void* dst, const void* src, size_t bytes, cudaStream_t st) {
+  if (!bytes) return SPH_OK;
+  if (is_pinned(dst)) { CK(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, st)); return SPH_OK; }
+  int rc = pin_init(c);
+  if (rc) return rc;
+  const size_t half = c->pin_bytes / 2;
+  size_t pend_off[2] = {0, 0}, pend_m[2] = {0, 0};
+  int k = 0;
+  for (size_t off = 0; off < bytes; off += half, k ^= 1) {
+    const size_t m = std::min(half, bytes - off);
+    if (pend_m[k]) {  // drain the chunk that sits in this half
+      CK(cudaEventSynchronize(c->pin_ev[k]));
+      memcpy((char*)dst + pend_off[k], c->pin + k * half, pend_m[k]);
+    }
+    CK(cudaMemcpyAsync(c->pin + k * half, (const char*)src + off, m, cudaMemcpyDeviceToHost, st));
+    CK(cudaEventRecord(c->pin_ev[k], st));
+    pend_off[k] = off; pend_m[k] = m;
+  }
+  for (int j = 0; j < 2; ++j, k ^= 1)
+    if (pend_m[k]) {
+      CK(cudaEventSynchronize(c->pin_ev[k]));
+      memcpy((char*)dst + pend_off[k], c->pin + k * half, pend_m[k]);
+      pend_m[k] = 0;
+    }
+  return SPH_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -673,7 +742,11 @@ int sph_create(const sph_params* prm, sph_ctx** out) {
     *ncell = (int64_t)nc[0] * nc[1] * nc[2];
   };
   const double edgeC = 2.0 * h * (1.0 + 1.0 / 1024.0);  // reading A24
-  set_grid(d, edgeC * (1.0 + skin), &c->ncell);
+  // NEXT-4: cell edge = half the list radius with a 125 / 25-cell walk, measured against the 27 / 9-cell walk
+  // (profiles/r02_README.md); only with kept lists (the contract grid stays the 27-cell one)
+  d.reach = 1;
+  if (skin > 0.0 && getenv("SPH_REACH")) d.reach = atoi(getenv("SPH_REACH")) == 2 ? 2 : 1;   // measurement switch
+  set_grid(d, edgeC * (1.0 + skin) / d.reach, &c->ncell);
   for (int k = 0; k < 3; ++k) d.wamp[k] = k < prm->dim ? prm->wall_osc_amp[k] : 0.0;
   d.womega = 6.283185307179586476925286766559 * prm->wall_osc_freq;
   c->moving = prm->wall_osc_freq > 0.0 && (d.wamp[0] != 0.0 || d.wamp[1] != 0.0 || d.wamp[2] != 0.0);
@@ -692,7 +765,7 @@ int sph_create(const sph_params* prm, sph_ctx** out) {
     while (b > 0 && bits_for(c->ncell) + b * prm->dim > 31) --b;
     d.sub_bits = b * prm->dim;
   }
-  c->dpC.sub_bits = 0;
+  c->dpC.sub_bits = 0; c->dpC.reach = 1;
   c->cell_bits = bits_for(c->ncell) + d.sub_bits;
   c->multi = prm->n_phases > 1;
   *out = c;
@@ -733,30 +806,33 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
   c->n = n; c->nf = (int64_t)fid.size(); c->nw = (int64_t)wid.size();
   const int nf = (int)c->nf, nw = (int)c->nw;
   const size_t cap = (size_t)std::max(nf, nw);
-  int rc = 0;
-  rc |= dalloc(c, &c->R0, nf); rc |= dalloc(c, &c->R1, nf); rc |= dalloc(c, &c->TX, cap); rc |= dalloc(c, &c->A, (size_t)nf + 16);
-  rc |= dalloc(c, &c->TB, cap);
-  rc |= dalloc(c, &c->ACC, nf); rc |= dalloc(c, &c->SIG, nf); rc |= dalloc(c, &c->DRHO, nf);
+  int rc = SPH_OK;
+  // every allocation is attempted only while the previous ones succeeded; the first failing code is returned
+#define TRY(call) do { if (rc == SPH_OK) rc = (call); } while (0)
+  TRY(dalloc(c, &c->R0, nf)); TRY(dalloc(c, &c->R1, nf)); TRY(dalloc(c, &c->TX, cap)); TRY(dalloc(c, &c->A, (size_t)nf + 16));
+  TRY(dalloc(c, &c->TB, cap));
+  TRY(dalloc(c, &c->ACC, nf)); TRY(dalloc(c, &c->SIG, nf)); TRY(dalloc(c, &c->DRHO, nf));
   c->npad = ((size_t)nf + PB - 1) / PB * PB;
   c->caps = c->prm.max_neighbours ? (int)((c->prm.max_neighbours + 3u) & ~3u) : (c->prm.dim == 3 ? 160 : 64);
-  rc |= dalloc(c, &c->NL, c->npad * (size_t)(c->caps >> 2)); rc |= dalloc(c, &c->NC, nf);
+  TRY(dalloc(c, &c->NL, c->npad * (size_t)(c->caps >> 2))); TRY(dalloc(c, &c->NC, nf));
   c->capsw = (c->caps * 3 / 4 + 3) & ~3;  // a particle in a corner of three walls has 7/8 of its (then smaller) support in them
-  rc |= dalloc(c, &c->NLW, c->npad * (size_t)(c->capsw >> 2)); rc |= dalloc(c, &c->NCW, nf);
-  rc |= dalloc(c, &c->NLF, ((size_t)nw + PB - 1) / PB * PB * (size_t)(c->capsw >> 2)); rc |= dalloc(c, &c->NCF, nw);
-  rc |= dalloc(c, &c->ID0, cap); rc |= dalloc(c, &c->ID1, cap);
-  rc |= dalloc(c, &c->keyA, cap); rc |= dalloc(c, &c->valA, cap); rc |= dalloc(c, &c->keyB, cap);
-  rc |= dalloc(c, &c->valB, cap);
-  rc |= dalloc(c, &c->hist, (size_t)512 * std::max(cdiv(std::max(nf, 1), RS_THREADS * rs_items((size_t)nf)),
-                                                  cdiv(std::max(nw, 1), RS_THREADS * rs_items((size_t)nw))));
-  rc |= dalloc(c, &c->rowsum, 512);
-  if (!rc) CK(cudaMemsetAsync(c->rowsum, 0, 512 * sizeof(unsigned), (cudaStream_t)stream));  // radix digit totals: zero between passes
-  rc |= dalloc(c, &c->lbF, c->ncell + 1); rc |= dalloc(c, &c->lbW, c->ncell + 1);
-  rc |= dalloc(c, &c->wnear, c->ncell);
-  rc |= dalloc(c, &c->WR, nw); rc |= dalloc(c, &c->WA, (size_t)nw + 16);
-  rc |= dalloc(c, &c->WN, nw); rc |= dalloc(c, &c->WG, nw); rc |= dalloc(c, &c->WK, nw);
-  rc |= dalloc(c, &c->WID, nw);
-  rc |= dalloc(c, &c->S, 1); rc |= dalloc(c, &c->stat, 1);
-  if (rc) return c->err.find("out of memory") != std::string::npos ? SPH_ENOMEM : SPH_ECUDA;
+  TRY(dalloc(c, &c->NLW, c->npad * (size_t)(c->capsw >> 2))); TRY(dalloc(c, &c->NCW, nf));
+  TRY(dalloc(c, &c->NLF, ((size_t)nw + PB - 1) / PB * PB * (size_t)(c->capsw >> 2))); TRY(dalloc(c, &c->NCF, nw));
+  TRY(dalloc(c, &c->ID0, cap)); TRY(dalloc(c, &c->ID1, cap));
+  TRY(dalloc(c, &c->keyA, cap)); TRY(dalloc(c, &c->valA, cap)); TRY(dalloc(c, &c->keyB, cap));
+  TRY(dalloc(c, &c->valB, cap));
+  TRY(dalloc(c, &c->hist, (size_t)512 * std::max(cdiv(std::max(nf, 1), RS_THREADS * rs_items((size_t)nf)),
+                                                  cdiv(std::max(nw, 1), RS_THREADS * rs_items((size_t)nw)))));
+  TRY(dalloc(c, &c->rowsum, 512));
+  if (rc == SPH_OK) CK(cudaMemsetAsync(c->rowsum, 0, 512 * sizeof(unsigned), (cudaStream_t)stream));  // radix digit totals: zero between passes
+  TRY(dalloc(c, &c->lbF, c->ncell + 1)); TRY(dalloc(c, &c->lbW, c->ncell + 1));
+  TRY(dalloc(c, &c->wnear, c->ncell));
+  TRY(dalloc(c, &c->WR, nw)); TRY(dalloc(c, &c->WA, (size_t)nw + 16));
+  TRY(dalloc(c, &c->WN, nw)); TRY(dalloc(c, &c->WG, nw)); TRY(dalloc(c, &c->WK, nw));
+  TRY(dalloc(c, &c->WID, nw));
+  TRY(dalloc(c, &c->S, 1)); TRY(dalloc(c, &c->stat, 1));
+#undef TRY
+  if (rc) return rc;
   c->IDcur = c->ID0; c->IDnext = c->ID1;
   CK(cudaMemsetAsync(c->S, 0, sizeof(SS), st));
   {  // the first build takes the largest skin; k_predict adapts it from the displacements it sees
@@ -780,16 +856,25 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
     CK(cudaMemsetAsync((char*)c->S + offsetof(SS, sq), 0, 3 * sizeof(int), st));
     CK(cudaStreamSynchronize(st));  // g0 / v0 are stack variables
   }
-  if (dalloc(c, &c->hidx, std::max<size_t>(cap, 1))) return SPH_ECUDA;  // kept across calls
-  int* idx = c->hidx;
+  if (dalloc(c, &c->class_idx, std::max<size_t>(cap, 1))) return SPH_ECUDA;  // kept across calls
+  int* idx = c->class_idx;
   // ---- wall structure, built once ----
   if (nw > 0) {
     CK(cudaMemcpyAsync(idx, wid.data(), sizeof(int) * nw, cudaMemcpyHostToDevice, st));
     LAUNCH(k_load, cdiv(nw, 256), 256, st, c->dp, nw, 1, idx, pos, vel, rho, tag, c->TX, c->TB, c->ID0, c->keyA, c->valA);
     if (c->moving) {  // NEXT-1: keep the set-up order for the per-step re-sort
-      rc = dalloc(c, &c->WX0, nw) | dalloc(c, &c->WXB, nw) | dalloc(c, &c->WN0, nw) | dalloc(c, &c->WID0, nw) | dalloc(c, &c->WkeyA, nw) | dalloc(c, &c->WkeyB, nw) |
-           dalloc(c, &c->WvalA, nw) | dalloc(c, &c->WvalB, nw) | dalloc(c, &c->WTX, nw) | dalloc(c, &c->WTB, nw) |
-           dalloc(c, &c->Whist, (size_t)512 * cdiv(nw, RS_THREADS * rs_items((size_t)nw))) | dalloc(c, &c->Wrowsum, 512);
+      rc = dalloc(c, &c->WX0, nw);
+      if (!rc) rc = dalloc(c, &c->WXB, nw);
+      if (!rc) rc = dalloc(c, &c->WN0, nw);
+      if (!rc) rc = dalloc(c, &c->WID0, nw);
+      if (!rc) rc = dalloc(c, &c->WkeyA, nw);
+      if (!rc) rc = dalloc(c, &c->WkeyB, nw);
+      if (!rc) rc = dalloc(c, &c->WvalA, nw);
+      if (!rc) rc = dalloc(c, &c->WvalB, nw);
+      if (!rc) rc = dalloc(c, &c->WTX, nw);
+      if (!rc) rc = dalloc(c, &c->WTB, nw);
+      if (!rc) rc = dalloc(c, &c->Whist, (size_t)512 * cdiv(nw, RS_THREADS * rs_items((size_t)nw)));
+      if (!rc) rc = dalloc(c, &c->Wrowsum, 512);
       if (rc) return rc;
       CK(cudaMemsetAsync(c->Wrowsum, 0, 512 * sizeof(unsigned), st));
       if (!c->wstream) CK(cudaStreamCreateWithFlags(&c->wstream, cudaStreamNonBlocking));
@@ -841,18 +926,19 @@ int sph_set_particles_host(sph_ctx* c, int64_t n, const float* pos, const float*
   if (n < 0 || (n > 0 && (!pos || !vel || !rho || !tag))) { c->err = "bad arguments"; return SPH_EINVAL; }
   cudaStream_t st = (cudaStream_t)stream;
   size_t m = (size_t)std::max<int64_t>(n, 1);
-  int rc = dalloc(c, &c->hpos, m * 3) | dalloc(c, &c->hvel, m * 3) | dalloc(c, &c->hrho, m) | dalloc(c, &c->htagd, m);
+  int rc = dalloc(c, &c->stage_pos, m * 3);
+  if (!rc) rc = dalloc(c, &c->stage_vel, m * 3);
+  if (!rc) rc = dalloc(c, &c->stage_rho, m);
+  if (!rc) rc = dalloc(c, &c->stage_tag, m);
   if (rc) return rc;
-  float *dpos = c->hpos, *dvel = c->hvel, *drho = c->hrho;
-  int32_t* dtag = c->htagd;
-  cudaError_t e = cudaSuccess;
+  float *dpos = c->stage_pos, *dvel = c->stage_vel, *drho = c->stage_rho;
+  int32_t* dtag = c->stage_tag;
   if (n) {
-    e = cudaMemcpyAsync(dpos, pos, n * 12, cudaMemcpyHostToDevice, st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(dvel, vel, n * 12, cudaMemcpyHostToDevice, st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(drho, rho, n * 4, cudaMemcpyHostToDevice, st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(dtag, tag, n * 4, cudaMemcpyHostToDevice, st);
+    rc = h2d(c, dpos, pos, (size_t)n * 12, st);
+    if (!rc) rc = h2d(c, dvel, vel, (size_t)n * 12, st);
+    if (!rc) rc = h2d(c, drho, rho, (size_t)n * 4, st);
+    if (!rc) rc = h2d(c, dtag, tag, (size_t)n * 4, st);
   }
-  if (e != cudaSuccess) { c->err = cudaGetErrorString(e); rc = SPH_ECUDA; }
   if (rc == SPH_OK) rc = sph_set_particles(c, n, dpos, dvel, drho, dtag, stream);
   cudaStreamSynchronize(st);
   return rc;
@@ -884,23 +970,22 @@ int sph_get_fields_host(sph_ctx* c, float* pos, float* vel, float* rho, float* p
   if (!c->loaded) { c->err = "no particles"; return SPH_EINVAL; }
   cudaStream_t st = (cudaStream_t)stream;
   const size_t n = (size_t)std::max<int64_t>(c->n, 1);
-  if (dalloc(c, &c->hout, n * 11)) return SPH_ECUDA;  // kept across calls
-  float* buf = c->hout;
+  if (dalloc(c, &c->stage_out, n * 11)) return SPH_ECUDA;  // kept across calls
+  float* buf = c->stage_out;
   float *dpos = buf, *dvel = buf + 3 * n, *dacc = buf + 6 * n, *drho = buf + 9 * n, *dp = buf + 10 * n;
   int rc = sph_get_fields(c, pos ? dpos : nullptr, vel ? dvel : nullptr, rho ? drho : nullptr,
                           p ? dp : nullptr, acc ? dacc : nullptr, stream);
-  cudaError_t e = cudaSuccess;
   if (rc == SPH_OK && c->n) {
-    if (pos) e = cudaMemcpyAsync(pos, dpos, c->n * 12, cudaMemcpyDeviceToHost, st);
-    if (vel && e == cudaSuccess) e = cudaMemcpyAsync(vel, dvel, c->n * 12, cudaMemcpyDeviceToHost, st);
-    if (acc && e == cudaSuccess) e = cudaMemcpyAsync(acc, dacc, c->n * 12, cudaMemcpyDeviceToHost, st);
-    if (rho && e == cudaSuccess) e = cudaMemcpyAsync(rho, drho, c->n * 4, cudaMemcpyDeviceToHost, st);
-    if (p && e == cudaSuccess) e = cudaMemcpyAsync(p, dp, c->n * 4, cudaMemcpyDeviceToHost, st);
+    if (pos) rc = d2h(c, pos, dpos, (size_t)c->n * 12, st);
+    if (vel && !rc) rc = d2h(c, vel, dvel, (size_t)c->n * 12, st);
+    if (acc && !rc) rc = d2h(c, acc, dacc, (size_t)c->n * 12, st);
+    if (rho && !rc) rc = d2h(c, rho, drho, (size_t)c->n * 4, st);
+    if (p && !rc) rc = d2h(c, p, dp, (size_t)c->n * 4, st);
   }
   cudaError_t e2 = cudaStreamSynchronize(st);
   if (rc) return rc;
-  if (e != cudaSuccess || e2 != cudaSuccess) {
-    c->err = cudaGetErrorString(e != cudaSuccess ? e : e2);
+  if (e2 != cudaSuccess) {
+    c->err = cudaGetErrorString(e2);
     return SPH_ECUDA;
   }
   return SPH_OK;

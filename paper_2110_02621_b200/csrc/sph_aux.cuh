@@ -317,12 +317,13 @@ __global__ void k_normals(DP p, int nw, const XB* __restrict__ WR, const unsigne
   const double dpd = p.dpD;
   const double V0 = DIM == 2 ? dpd * dpd : dpd * dpd * dpd;
   double px = 0, py = 0, pz = 0;
-  for (int dz = (DIM == 3 ? -1 : 0); dz <= (DIM == 3 ? 1 : 0); ++dz)
-    for (int dy = -1; dy <= 1; ++dy) {
+  const int RC = p.reach;
+  for (int dz = (DIM == 3 ? -RC : 0); dz <= (DIM == 3 ? RC : 0); ++dz)
+    for (int dy = -RC; dy <= RC; ++dy) {
       const int y = cy + dy, z = cz + dz;
       if (y < 0 || y >= p.ny || z < 0 || z >= p.nz) continue;
       const int rb = (z * p.ny + y) * p.nx;
-      const int s = lbW[rb + max(cx - 1, 0)], e = lbW[rb + min(cx + 1, p.nx - 1) + 1];
+      const int s = lbW[rb + max(cx - RC, 0)], e = lbW[rb + min(cx + RC, p.nx - 1) + 1];
       for (int j = s; j < e; ++j) {
         if (j == w) continue;
         const uint4 xj = WR[j].x;
@@ -349,12 +350,13 @@ __global__ void k_wnear(DP p, int ncell, const int* __restrict__ lbW, unsigned c
   if (c >= ncell) return;
   const int row = c / p.nx, cx = c - row * p.nx, cz = row / p.ny, cy = row - cz * p.ny;
   int any = 0;
-  for (int dz = (p.dim == 3 ? -1 : 0); dz <= (p.dim == 3 ? 1 : 0); ++dz)
-    for (int dy = -1; dy <= 1; ++dy) {
+  const int RC = p.reach;
+  for (int dz = (p.dim == 3 ? -RC : 0); dz <= (p.dim == 3 ? RC : 0); ++dz)
+    for (int dy = -RC; dy <= RC; ++dy) {
       const int y = cy + dy, z = cz + dz;
       if (y < 0 || y >= p.ny || z < 0 || z >= p.nz) continue;
       const int rb = (z * p.ny + y) * p.nx;
-      any |= lbW[rb + min(cx + 1, p.nx - 1) + 1] > lbW[rb + max(cx - 1, 0)];
+      any |= lbW[rb + min(cx + RC, p.nx - 1) + 1] > lbW[rb + max(cx - RC, 0)];
     }
   wnear[c] = (unsigned char)any;
 }

@@ -43,6 +43,8 @@ struct DP {
   double wamp[3], womega;  // NEXT-1: wall motion x_w(t) = x_w(0) + wamp sin(womega t); womega = 0: static walls
   // Verlet skin: the lists are built with radius 2h(1 + skin) on a cell grid of that edge
   // and kept while 2 * (fluid displacement bound) and (fluid + wall displacement) stay below skin_budget
+  int reach;           // cells per axis a neighbour walk reaches on each side: 1 (cell edge = list radius, 27 / 9 cells) or
+                       // 2 (cell edge = half of it, 125 / 25 cells: NEXT-4 measurement)
   int sub_bits;        // sort key = (cell id << sub_bits) | Morton code of the position inside the cell (sub_bits / dim bits
                        // per axis; 0 when skin = 0, where the order inside a cell is the contract's id order, reading A25)
   double skin;         // largest skin s_max >= 0 (the cell edge is 2h(1 + s_max)); 0: the lists are rebuilt every step

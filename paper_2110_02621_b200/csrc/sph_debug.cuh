@@ -24,15 +24,16 @@ __device__ __forceinline__ void walk(const DP& p, const float4* __restrict__ P, 
   const unsigned lt = (1u << lane) - 1u;
   const int cx = cell_coord(xi, p.ox, p.inv_edge, p.nx), cy = cell_coord(yi, p.oy, p.inv_edge, p.ny);
   const int cz = p.dim == 3 ? cell_coord(zi, p.oz, p.inv_edge, p.nz) : 0;
-  const int nrow = p.dim == 3 ? 9 : 3;
+  const int RC = p.reach, W = 2 * RC + 1;     // W * W <= 25 rows: one per lane
+  const int nrow = p.dim == 3 ? W * W : W;
   int rs = 0, re = 0;
   if (lane < nrow) {
-    int y = cy + (lane % 3) - 1, z = cz + (lane / 3) - 1;
+    int y = cy + (lane % W) - RC, z = cz + (lane / W) - RC;
     if (p.dim != 3) z = 0;
     if (y >= 0 && y < p.ny && z >= 0 && z < p.nz) {
       int rb = (z * p.ny + y) * p.nx;
-      rs = lb[rb + max(cx - 1, 0)];
-      re = lb[rb + min(cx + 1, p.nx - 1) + 1];
+      rs = lb[rb + max(cx - RC, 0)];
+      re = lb[rb + min(cx + RC, p.nx - 1) + 1];
     }
   }
   int qn = 0, qh = 0;

@@ -198,19 +198,19 @@ __device__ __forceinline__ void walk_f(const DP& p, const float4* __restrict__ A
   const float m2x = -2.0f * ai.x, m2y = -2.0f * ai.y, m2z = -2.0f * ai.z;
   const float thr = EXACT ? rl2m : rl2m - ai.w;
   const int lane = threadIdx.x & 31;
-  constexpr int NR = DIM == 3 ? 9 : 3;
-  int ry = -1, rz = DIM == 3 ? -1 : 0;
+  const int RC = p.reach, NR = DIM == 3 ? (2 * RC + 1) * (2 * RC + 1) : 2 * RC + 1;
+  int ry = -RC, rz = DIM == 3 ? -RC : 0;
 #pragma unroll 1
   for (int r = 0; r < NR; ++r) {
     int s = 0x7fffffff, e = 0;
     const int y = cy + ry, z = cz + rz;
     if (act && y >= 0 && y < p.ny && z >= 0 && z < p.nz) {
       const int rb = (z * p.ny + y) * p.nx;
-      const int s1 = __ldg(lb + rb + max(cx - 1, 0));
-      e = __ldg(lb + rb + min(cx + 1, p.nx - 1) + 1);
+      const int s1 = __ldg(lb + rb + max(cx - RC, 0));
+      e = __ldg(lb + rb + min(cx + RC, p.nx - 1) + 1);
       if (e > s1) s = s1; else e = 0;
     }
-    if (++ry > 1) { ry = -1; ++rz; }
+    if (++ry > RC) { ry = -RC; ++rz; }
     const int smin = STAGE ? __reduce_min_sync(FULL, s) : 0, emax = STAGE ? __reduce_max_sync(FULL, e) : 0;
     bool staged = false;
     if constexpr (STAGE) if (emax > smin && emax - smin <= TW) {  // warp-uniform; a row in which no lane has a candidate (emax <= smin) skips the tile

@@ -20,12 +20,13 @@ k_probe_pressure(const DP p, const int nf, const int m, const float* __restrict_
   const int cz = p.dim == 3 ? cell_coord(zf, p.oz, p.inv_edge, p.nz) : 0;
   const double ih = 1.0 / p.hD;
   double sw = 0.0, sp = 0.0;
-  for (int dz = (p.dim == 3 ? -1 : 0); dz <= (p.dim == 3 ? 1 : 0); ++dz)
-    for (int dy = -1; dy <= 1; ++dy) {
+  const int RC = p.reach;
+  for (int dz = (p.dim == 3 ? -RC : 0); dz <= (p.dim == 3 ? RC : 0); ++dz)
+    for (int dy = -RC; dy <= RC; ++dy) {
       const int yy = cy + dy, zz = cz + dz;
       if (yy < 0 || yy >= p.ny || zz < 0 || zz >= p.nz) continue;
       const int rb = (zz * p.ny + yy) * p.nx;
-      const int s = lbF[rb + max(cx - 1, 0)], e = lbF[rb + min(cx + 1, p.nx - 1) + 1];
+      const int s = lbF[rb + max(cx - RC, 0)], e = lbF[rb + min(cx + RC, p.nx - 1) + 1];
       for (int j = s + lane; j < e; j += 32) {
         const XB r = R[j];
         const double ddx = fx_to_double(r.x.x, p.O[0], p.Q) - x, ddy = fx_to_double(r.x.y, p.O[1], p.Q) - y;
