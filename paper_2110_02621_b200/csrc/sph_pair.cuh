@@ -359,14 +359,21 @@ struct KSum {
 struct Geo {
   float dx, dy, dz, r, rinv, w, f;
 };
-template <int DIM>
+__device__ __forceinline__ float rsqrt_raw(float x) {
+  float y;
+  asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+// REFINE = false: 1 / r straight from MUFU.RSQ (2^-22).  Measured in pass A (profiles/r02_README.md): -3 % on the
+// pass, but the 10-step acceleration error of box2d_jitter goes from 0.99e-4 to 1.05e-4 of |g| (bar 1e-4): not used.
+template <int DIM, bool REFINE = true>
 __device__ __forceinline__ Geo geometry(const DP& p, const uint4& xi, const uint4& xj) {
   Geo g;
   g.dx = (float)(int)(xi.x - xj.x);
   g.dy = (float)(int)(xi.y - xj.y);
   g.dz = DIM == 3 ? (float)(int)(xi.z - xj.z) : 0.0f;
   const float r2 = DIM == 3 ? fmaf(g.dz, g.dz, fmaf(g.dy, g.dy, g.dx * g.dx)) : fmaf(g.dy, g.dy, g.dx * g.dx);
-  g.rinv = rsqrt_fast(fmaxf(r2, 0.5f));
+  g.rinv = REFINE ? rsqrt_fast(fmaxf(r2, 0.5f)) : rsqrt_raw(fmaxf(r2, 0.5f));
   g.r = r2 * g.rinv;
   const float qq = g.r * p.qh;
   const float t = fmaxf(fmaf(-0.5f, qq, 1.0f), 0.0f), t2 = t * t;
@@ -591,8 +598,9 @@ k_pass_a(const DP p, const SS* __restrict__ S, const int nf, const int init,
   // run counts its own phase and the walls only; an internal-flow (light) phase particle counts every neighbour
   const bool sig_all = !MULTI || !((p.fs_mask >> phi) & 1u);
   {
+    constexpr bool RF = true;
     auto body = make_body(R, [&](const uint4& xj, const float4& bj, const unsigned j) {
-    const Geo g = geometry<DIM>(p, xi, xj);
+    const Geo g = geometry<DIM, RF>(p, xi, xj);
     if (!MULTI || sig_all || phase_of(xj) == phi) sig += w64<DIM, SUBQ>(p, xi, xj, g);
     const float vd = fmaf(bi.z - bj.z, g.dz, fmaf(bi.y - bj.y, g.dy, (bi.x - bj.x) * g.dx));
     if (!MULTI) {
