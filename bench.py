@@ -281,6 +281,8 @@ def run_gpu(args):
         # not the headline workload: the line's config.workload says so.
         a0, f0 = (float(x) for x in args.wall_osc.split(","))
         cfg["wall_osc_amp"], cfg["wall_osc_freq"] = (a0, 0.0, 0.0), f0
+    if args.no_graph:
+        cfg["flags"] = cfg["flags"] | sph.FLAG_NO_GRAPH
     nfl, nwl = cfg["n_fluid"], cfg["n_wall"]
     K, W = args.steps, max(args.warmup, 0)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")  # > 126 MB L2
@@ -355,9 +357,12 @@ def run_gpu(args):
     # measured non-tensor FP32 peak (SURVEY.md section 8(d) "Peaks"): register-resident FMA loop, this device, now
     fma_sampler = ClockSampler(local)
     fma_sampler.start()
-    peak = sph.fma_peak_tflops()
-    for _ in range(20):             # keep the loop running long enough for nvidia-smi to sample its clocks
-        peak = max(peak, sph.fma_peak_tflops())
+    if args.derived_peak:
+        peak = peak_derived
+    else:
+        peak = sph.fma_peak_tflops()
+        for _ in range(20):             # keep the loop running long enough for nvidia-smi to sample its clocks
+            peak = max(peak, sph.fma_peak_tflops())
     fma_clocks = fma_sampler.stop()
     kern = {}
     # Pair stages.  The 27-cell candidate walk runs once per step in k_build (fluid-fluid) and inside
@@ -384,7 +389,7 @@ def run_gpu(args):
                    "frac_with_candidates": (fl_pair + CAND_FLOPS * cand_b * stage_def["rebuilds_per_step"]) / t_pair / 1e12 / peak}
     # HBM-bound stages: algorithmic bytes per fluid particle
     hbm = _peaks().get("hbm_gbs", 6650.0)
-    bytes_pp = {"predict": 108.0, "sort": (16.0 + 4.0) * g_sort_passes(g), "reorder": 100.0}
+    bytes_pp = {"predict": 140.0, "sort": (16.0 + 4.0) * g_sort_passes(g), "reorder": 100.0}
     for name, b in bytes_pp.items():
         t = stage_ms[name] * 1e-3
         if t > 0:
@@ -397,7 +402,8 @@ def run_gpu(args):
                 "l1_data_pipe_frac_ncu": float(ncu["l1_data_pipe_frac"]) if ncu else None,
                 "issue_active_frac_ncu": float(ncu["issue_active_frac"]) if ncu else None,
                 "ncu_capture": (ncu["capture"] if ncu else None), "csrc_hash": csrc_hash(),
-                "peak_source": "measured: sph_debug_fma_peak (register-resident FMA loop, 8 chains x 2048 threads per SM) on this device in this run",
+                "peak_source": ("derived from unit counts (--derived-peak: profiler capture, not a bench line)" if args.derived_peak else
+                                "measured: sph_debug_fma_peak (register-resident FMA loop, 8 chains x 2048 threads per SM) on this device in this run"),
                 "peak_derived": peak_derived, "peak_clocks": {"sm_mhz": fma_clocks.get("sm_mhz"), "sm_max_mhz": fma_clocks.get("sm_max_mhz")},
                 "flops_per_hit": FLOPS_HIT[dom], "flops_per_candidate": CAND_FLOPS,
                 # list build + pass A + pass B together (the candidate walk is k_build's):
@@ -520,6 +526,10 @@ def main():
                     help="oracle steps of the cpu_baseline leg (1 M particles: about 0.6 s per step on 16 cores)")
     ap.add_argument("--csrc-hash", action="store_true", help="print the hash profiles/ncu_kernels.csv is keyed by and exit")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--derived-peak", action="store_true",
+                    help="skip the FMA-loop peak measurement (126 launches) and use the derived peak: for profiler launch lists only")
+    ap.add_argument("--no-graph", action="store_true",
+                    help="SPH_FLAG_NO_GRAPH: plain launches instead of the step graph (same kernels; for profiler captures)")
     ap.add_argument("--wall-osc", default="", metavar="A0,F0",
                     help="move the walls along x as A0 sin(2 pi F0 t) (metres, Hz); implies a non-headline line")
     args = ap.parse_args()

@@ -32,10 +32,12 @@
 //   sigma of pass A       — lattice constant after a step                                         (P25)
 //   two-phase tank X1     — stays at rest under reading A13b, not without it   (P26)
 //   wall extensions       — without them air leaves the tank                   (P27)
+//   unequal-c solver      — acoustic characteristic relations, limiter limits                    (P28)
+//   fluid-wall pair       — Eq. 2.12 lever, wall density A5, Eq. 2.11 weights by hand             (P29)
 // PARITY UNPINNED (fixed by DESIGN.md readings only, no external pin exists):
-//   wall velocity mirror (A6), step ordering and two wall passes (A16),
-//   per-pair wall density (A5), penalty scaling (A8), unequal-c solver (A3;
-//   pinned only by its reduction to Eq. 2.8 at c_L = c_R, P18).
+//   wall velocity mirror (A6), step ordering and two wall passes (A16), penalty scaling and
+//   window (A8 / A9); whether A3's extension and A5's per-pair wall density are the authors' choice
+//   (P18 / P28 / P29 pin that the code computes what those readings say).
 //
 // Build: g++ -O2 -fopenmp -ffp-contract=off -shared -fPIC (see oracle/build.py)
 

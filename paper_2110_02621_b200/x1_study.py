@@ -63,12 +63,23 @@ def run_case(dp, t_end, samples=50, c_rule="baseline", flags=None, penalty=True,
     pex = inputs.x1_analytic_pressure(cfg, y)
     l2 = lambda p: math.sqrt(float(((p[fl] - pex[fl]) ** 2).sum() / (pex[fl] ** 2).sum()))
     ep0 = float((m[fl] * inputs.G0 * cfg["pos"][fl, 1].astype(np.float64)).sum())
+    # where the error sits: mean of (p - p_exact) / (rho_w g H) over the water in ten bands of height (time-averaged p)
+    S = cfg["rho0"][0] * inputs.G0 * cfg["H"]
+    pbar = p_acc / max(n_acc, 1) if p_acc is not None else f["p"].astype(np.float64)
+    water = tag == 0
+    profile = []
+    for k in range(10):
+        lo, hi = k * cfg["H"] / 10.0, (k + 1) * cfg["H"] / 10.0
+        sel = water & (y >= lo) & (y < hi)
+        if sel.any():
+            profile.append([0.5 * (lo + hi), float(((pbar - pex)[sel]).mean() / S)])
+    y_water_mean = float(y[water].mean())
     out = dict(dp=dp, n_fluid=cfg["n_fluid"], n_wall=cfg["n_wall"], t_end=t, steps=steps,
                l2_end=l2(f["p"].astype(np.float64)), l2_avg=l2(p_acc / max(n_acc, 1)) if p_acc is not None else None,
                ek_max_over_T=max(h["ek"] for h in hist) / T_tot, ek_end_over_T=hist[-1]["ek"] / T_tot,
                ep0=ep0, ep_end_minus_ep0_over_T=(hist[-1]["ep"] - ep0) / T_tot,
                escaped=int(s["escaped"]), nonfinite=int(s["nonfinite"]), seconds=time.time() - t0,
-               c0=cfg["c0"][0], history=hist)
+               c0=cfg["c0"][0], error_profile=profile, water_mean_height=y_water_mean, history=hist)
     g.close()
     return out
 
@@ -94,6 +105,9 @@ def main():
     for r in rows:
         print("%-9g %9d %9d %10.5f %10.5f %11.3e %11.3e %8d" % (r["dp"], r["n_fluid"], r["steps"], r["l2_end"], r["l2_avg"] or float("nan"),
                                                                r["ek_max_over_T"], r["ek_end_over_T"], r["escaped"]))
+    for r in rows:
+        print("dp %g: mean (p - p_exact) / (rho_w g H) of the water by height: " % r["dp"] +
+              " ".join("%.2f:%+.4f" % (yy, e) for yy, e in r["error_profile"]) + "; mean water height %.5f" % r["water_mean_height"])
     for a_, b_ in zip(rows[:-1], rows[1:]):
         if a_["l2_avg"] and b_["l2_avg"]:
             print("order dp %g -> %g: L2(avg) ratio %.3f (observed order %.2f)" % (

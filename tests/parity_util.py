@@ -42,7 +42,7 @@ def acc_tol(cfg):
     DEVIATION 1.5e-6 H / h (A26c): the paper prescribes single precision and a
     float32 pair term of Eq. 2.10 is of size 0.1 g H / h with a relative rounding of a few 2^-24, so the largest
     error over 1e7 particles of a sum of 80 such terms is about 1e-6 (H / h) |g| whatever the summation (measured
-    1.8e-4 |g| at config 4's 16.8 M size, H / h = 197; 5.5e-5 at its 1 M size, H / h = 77).  Only config 4's sizes
+    1.8e-4 |g| at config 4's 16.8 M size, H / h = 197; 7.3e-5 at its 1 M size, H / h = 77).  Only config 4's sizes
     above 1 M exceed H / h = 66 by enough to matter."""
     return max(TOL, 1.5e-6 * float(cfg.get("H", 1.0)) / float(cfg["h"]))
 

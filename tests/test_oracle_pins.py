@@ -780,3 +780,75 @@ def test_P27_without_the_papers_wall_extensions_air_leaves_the_tank():
     (ekw2, eka2), f2 = _ek_by_phase(cfg2, o2)
     assert o2.stats()["escaped"] >= 1
     assert eka2 > 100.0 * eka, (eka, eka2)
+
+
+# ------------------------------------------------------------------ P28-P29: the unequal-c solver and the fluid-wall pair
+def test_P28_acoustic_solver_satisfies_the_characteristic_relations():
+    """Reading A3 away from c_L = c_R.  The linearised (acoustic) Riemann problem has a textbook solution (Toro 1989,
+    cited at PAPER.md:77) fixed by the two characteristic relations
+        p* - p_L = Z_L (U_L - U*),   p* - p_R = Z_R (U* - U_R),   Z = rho c.
+    The oracle's U* must satisfy both with the fully dissipative p* (limiter saturated, beta = c~: U_L - U_R >= c~/3),
+    its p* must equal that textbook p* there, and below saturation p* must lie between the non-dissipative average and
+    the textbook value, reaching the average when the states separate (U_L <= U_R, the limiter of Eq. 2.8)."""
+    rng = np.random.Generator(np.random.PCG64(28))
+    for _ in range(200):
+        rL, rR = rng.uniform(0.5, 2000.0, 2)
+        cL, cR = rng.uniform(5.0, 2000.0, 2)
+        pL, pR = rng.uniform(-1e4, 1e4, 2)
+        ZL, ZR = rL * cL, rR * cR
+        ctil = (ZL + ZR) / (rL + rR)
+        UR = rng.uniform(-5.0, 5.0)
+        # saturated limiter
+        UL = UR + ctil * rng.uniform(0.34, 3.0)
+        s = orc.riemann(rL, UL, pL, cL, rR, UR, pR, cR, mode=2)
+        scale = abs(pL) + abs(pR) + ZL * abs(UL) + ZR * abs(UR) + 1.0
+        assert abs((s["pstar"] - pL) - ZL * (UL - s["Ustar"])) < 1e-12 * scale
+        assert abs((s["pstar"] - pR) - ZR * (s["Ustar"] - UR)) < 1e-12 * scale
+        # separating states: no dissipation, p* = impedance-weighted average, U* unchanged in form
+        UL2 = UR - rng.uniform(0.0, 5.0)
+        s2 = orc.riemann(rL, UL2, pL, cL, rR, UR, pR, cR, mode=2)
+        assert abs(s2["pstar"] - (ZL * pR + ZR * pL) / (ZL + ZR)) < 1e-12 * scale
+        assert abs((ZL + ZR) * s2["Ustar"] - (ZL * UL2 + ZR * UR + pL - pR)) < 1e-12 * scale
+        # in between: monotone in the limiter
+        UL3 = UR + ctil * rng.uniform(0.0, 0.33)
+        s3 = orc.riemann(rL, UL3, pL, cL, rR, UR, pR, cR, mode=2)
+        p_avg = (ZL * pR + ZR * pL) / (ZL + ZR)
+        p_full = p_avg + ZL * ZR / (ZL + ZR) * (UL3 - UR)
+        assert p_avg - 1e-9 * scale <= s3["pstar"] <= p_full + 1e-9 * scale
+    # the dispatcher takes the paper's formulas at equal c and the acoustic ones otherwise
+    a = orc.riemann(1000.0, 1.0, 50.0, 30.0, 1.0, -2.0, 10.0, 30.0, mode=0)
+    b = orc.riemann(1000.0, 1.0, 50.0, 30.0, 1.0, -2.0, 10.0, 30.0, mode=1)
+    assert a == b
+    c = orc.riemann(1000.0, 1.0, 50.0, 30.0, 1.0, -2.0, 10.0, 900.0, mode=0)
+    d = orc.riemann(1000.0, 1.0, 50.0, 30.0, 1.0, -2.0, 10.0, 900.0, mode=2)
+    assert c == d
+
+
+def test_P29_one_fluid_particle_over_one_wall_particle_closed_form():
+    """Eq. 2.12, the wall density of reading A5 and Eq. 2.11 on the smallest case that separates them: one fluid
+    particle a distance d above one wall particle, a slow sound speed so that rho_w = rho0 + p_w / c^2 is far from
+    rho_f.  By hand: p_w = p_f + rho_f g . r_wf (one neighbour: the Shepard average is the value, the lever is the
+    printed one), p* = (rho_f p_w + rho_w p_f) / (rho_f + rho_w), a = g - 2 V0 (p* / rho_f) W'(d) e, e = r_fw / d.
+    Swapping the weights of Eq. 2.11, taking rho_w = rho_f, or dropping / flipping the lever each changes a by > 5 %."""
+    dp, c0, rho0 = 1.0 / 64, 1.0, 1000.0
+    d = 1.1 * dp
+    rho_f = 1100.0
+    g = (0.0, -50.0, 0.0)
+    pos = [[0.0, d], [0.0, 0.0]]
+    cfg = custom(2, pos, [0, -1], [rho_f, rho0], dp=dp, c0=(c0,), g=g, penalty_phase_mask=0)
+    cfg["pos"] = np.asarray([[0.0, d, 0.0], [0.0, 0.0, 0.0]], np.float32)
+    f = run(cfg).fields()
+    d32 = float(cfg["pos"][0, 1])
+    h = 1.3 * dp
+    p_f = c0 ** 2 * (rho_f - rho0)
+    p_w = p_f + rho_f * (g[1] * (0.0 - d32))          # r_wf = r_w - r_f = (0, -d)
+    rho_w = rho0 + p_w / c0 ** 2
+    assert rho_w > 1.5 * rho_f                          # the case does separate the readings
+    pstar = (rho_f * p_w + rho_w * p_f) / (rho_f + rho_w)
+    dw = orc.kernel_dw(2, h, d32)
+    ay = g[1] - 2.0 * dp * dp * (pstar / rho_f) * dw * 1.0    # grad_i W = W' (r_i - r_w) / d = W' (0, 1)
+    assert abs(f["p"][1] - p_w) < 1e-9 * abs(p_w)
+    assert abs(f["acc"][0, 1] - ay) < 1e-9 * abs(ay) and abs(f["acc"][0, 0]) < 1e-12
+    wrong = [(rho_w * p_w + rho_f * p_f) / (rho_f + rho_w), 0.5 * (p_w + p_f)]
+    for pw in wrong:
+        assert abs((g[1] - 2.0 * dp * dp * (pw / rho_f) * dw) - ay) > 0.05 * abs(ay)
