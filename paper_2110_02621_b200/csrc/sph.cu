@@ -89,7 +89,9 @@ struct sph_ctx {
   float *stage_pos = nullptr, *stage_vel = nullptr, *stage_rho = nullptr;
   int32_t* stage_tag = nullptr;
   float* stage_out = nullptr;
-  int* class_idx = nullptr;   // device: caller indices of one class during sph_set_particles
+  // device scratch of the classification in sph_set_particles (stable sort of (class, caller index))
+  unsigned *clsKa = nullptr, *clsVa = nullptr, *clsKb = nullptr, *clsVb = nullptr, *clsHist = nullptr, *clsRow = nullptr;
+  unsigned long long* clsCnt = nullptr;
   // PINNED host bounce buffer of the host-pointer entry points: pageable caller memory goes through it in two
   // halves (the copy of one half overlaps the memcpy of the other), so their speed does not depend on the
   // caller pinning its arrays; memory that is already pinned or registered is copied directly
@@ -180,7 +182,7 @@ void free_all(sph_ctx* c) {
   void* ptrs[] = {c->R0, c->R1, c->TX, c->A, c->TB, c->ACC, c->SIG, c->DRHO, c->NL, c->NC, c->NLW, c->NCW, c->NLF, c->NCF, c->ID0, c->ID1,
                   c->keyA, c->valA, c->keyB, c->valB, c->hist, c->rowsum, c->lbF, c->lbW, c->WR,
                   c->WA, c->WN, c->WG, c->WK, c->WID, c->wnear, c->S, c->dt_seq, c->stat,
-                  c->stage_pos, c->stage_vel, c->stage_rho, c->stage_tag, c->stage_out, c->class_idx,
+                  c->stage_pos, c->stage_vel, c->stage_rho, c->stage_tag, c->stage_out, c->clsKa, c->clsVa, c->clsKb, c->clsVb, c->clsHist, c->clsRow, c->clsCnt,
                   c->WX0, c->WXB, c->WN0, c->WID0, c->dKa, c->dVa, c->dKb, c->dVb, c->dID, c->dWID, c->dG, c->dWG, c->dlbF, c->dlbW, c->WkeyA, c->WkeyB, c->WvalA, c->WvalB,
                   c->WTX, c->WTB, c->Whist, c->Wrowsum};
   for (void* p : ptrs)
@@ -792,18 +794,35 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
   cudaStream_t st = (cudaStream_t)stream;
   c->loaded = false;
   if (c->gexec) { cudaGraphExecDestroy(c->gexec); c->gexec = nullptr; }  // buffers are reallocated below
-  // classify on the host (one-off): caller indices of fluid and wall particles, order kept
-  std::vector<int32_t> htag((size_t)n);
-  if (n) CK(cudaMemcpyAsync(htag.data(), tag, sizeof(int32_t) * n, cudaMemcpyDeviceToHost, st));
-  CK(cudaStreamSynchronize(st));
-  std::vector<int32_t> fid, wid;
-  fid.reserve(n); wid.reserve(n / 4 + 1);
-  for (int64_t i = 0; i < n; ++i) {
-    if (htag[i] == SPH_TAG_WALL) wid.push_back((int32_t)i);
-    else if (htag[i] >= 0 && htag[i] < c->prm.n_phases) fid.push_back((int32_t)i);
-    else { c->err = "tag out of range"; return SPH_EINVAL; }
+  // classify on the device (one-off): caller indices of the fluid entries, then of the wall entries, each in
+  // ascending order: a stable one-pass radix sort of (class, index); only the three class counts come to the host
+  unsigned* cls_idx = nullptr;
+  {
+    const size_t m = (size_t)std::max<int64_t>(n, 1);
+    int rc0 = dalloc(c, &c->clsKa, m);
+    if (!rc0) rc0 = dalloc(c, &c->clsVa, m);
+    if (!rc0) rc0 = dalloc(c, &c->clsKb, m);
+    if (!rc0) rc0 = dalloc(c, &c->clsVb, m);
+    if (!rc0) rc0 = dalloc(c, &c->clsHist, (size_t)512 * cdiv(m, RS_THREADS * rs_items(m)));
+    if (!rc0) rc0 = dalloc(c, &c->clsRow, 512);
+    if (rc0) return rc0;
+    CK(cudaMemsetAsync(c->clsRow, 0, 512 * sizeof(unsigned), st));
+    unsigned long long hcnt[3] = {0, 0, 0};
+    if (dalloc(c, &c->clsCnt, 3)) return SPH_ENOMEM;
+    unsigned long long* counts = c->clsCnt;
+    CK(cudaMemsetAsync(counts, 0, 3 * sizeof(unsigned long long), st));
+    unsigned *ks = c->clsKa, *vs = c->clsVa;
+    if (n) {
+      LAUNCH(k_classify, cdiv(n, 256), 256, st, (int)n, c->prm.n_phases, tag, c->clsKa, c->clsVa, counts);
+      int rcs = radix_sort(c, st, (int)n, 2, c->clsKa, c->clsVa, c->clsKb, c->clsVb, &ks, &vs, c->clsHist, c->clsRow);
+      if (rcs) return rcs;
+    }
+    CK(cudaMemcpyAsync(hcnt, counts, sizeof(hcnt), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    if (hcnt[2]) { c->err = "tag out of range"; return SPH_EINVAL; }
+    c->n = n; c->nf = (int64_t)hcnt[0]; c->nw = (int64_t)hcnt[1];
+    cls_idx = vs;
   }
-  c->n = n; c->nf = (int64_t)fid.size(); c->nw = (int64_t)wid.size();
   const int nf = (int)c->nf, nw = (int)c->nw;
   const size_t cap = (size_t)std::max(nf, nw);
   int rc = SPH_OK;
@@ -856,12 +875,11 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
     CK(cudaMemsetAsync((char*)c->S + offsetof(SS, sq), 0, 3 * sizeof(int), st));
     CK(cudaStreamSynchronize(st));  // g0 / v0 are stack variables
   }
-  if (dalloc(c, &c->class_idx, std::max<size_t>(cap, 1))) return SPH_ECUDA;  // kept across calls
-  int* idx = c->class_idx;
+  const int* idx_f = reinterpret_cast<const int*>(cls_idx);            // fluid caller ids, ascending
+  const int* idx_w = reinterpret_cast<const int*>(cls_idx) + c->nf;    // wall caller ids, ascending
   // ---- wall structure, built once ----
   if (nw > 0) {
-    CK(cudaMemcpyAsync(idx, wid.data(), sizeof(int) * nw, cudaMemcpyHostToDevice, st));
-    LAUNCH(k_load, cdiv(nw, 256), 256, st, c->dp, nw, 1, idx, pos, vel, rho, tag, c->TX, c->TB, c->ID0, c->keyA, c->valA);
+    LAUNCH(k_load, cdiv(nw, 256), 256, st, c->dp, nw, 1, idx_w, pos, vel, rho, tag, c->TX, c->TB, c->ID0, c->keyA, c->valA);
     if (c->moving) {  // NEXT-1: keep the set-up order for the per-step re-sort
       rc = dalloc(c, &c->WX0, nw);
       if (!rc) rc = dalloc(c, &c->WXB, nw);
@@ -901,11 +919,9 @@ int sph_set_particles(sph_ctx* c, int64_t n, const float* pos, const float* vel,
     LAUNCH(k_cell_bounds, cdiv(c->ncell + 1, 256), 256, st, c->keyA, 0, (int)c->ncell, c->lbW, 0);
   }
   LAUNCH(k_wnear, cdiv(c->ncell, 256), 256, st, c->dp, (int)c->ncell, c->lbW, c->wnear);
-  CK(cudaStreamSynchronize(st));  // wid host buffer / idx reuse
   // ---- fluid: load, then the common pipeline in init mode (dt = 0: sigma_i, p_w, (dv/dt)^0) ----
   if (nf > 0) {
-    CK(cudaMemcpyAsync(idx, fid.data(), sizeof(int) * nf, cudaMemcpyHostToDevice, st));
-    LAUNCH(k_load, cdiv(nf, 256), 256, st, c->dp, nf, 0, idx, pos, vel, rho, tag, c->TX, c->TB, c->IDcur, c->keyA, c->valA);
+    LAUNCH(k_load, cdiv(nf, 256), 256, st, c->dp, nf, 0, idx_f, pos, vel, rho, tag, c->TX, c->TB, c->IDcur, c->keyA, c->valA);
   }
   Prof pf(c, st);
   pf.on = false;

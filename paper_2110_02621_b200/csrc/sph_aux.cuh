@@ -37,6 +37,26 @@ __global__ void k_load(DP p, int n, int is_wall, const int* __restrict__ idx, co
   vals[i] = (unsigned)i;
 }
 
+// sph_set_particles: class of every caller entry as a sort key (0 fluid, 1 wall, 2 tag out of range) with its index;
+// a stable sort by this key leaves the fluid entries first, then the wall entries, each in ascending caller order.
+__global__ void __launch_bounds__(256)
+k_classify(int n, int n_phases, const int* __restrict__ tag, unsigned* __restrict__ keys, unsigned* __restrict__ vals,
+           unsigned long long* __restrict__ counts) {
+  __shared__ unsigned sm[3];
+  if (threadIdx.x < 3) sm[threadIdx.x] = 0u;
+  __syncthreads();
+  const int i = blockIdx.x * 256 + threadIdx.x;
+  if (i < n) {
+    const int t = tag[i];
+    const unsigned k = t == SPH_TAG_WALL ? 1u : (t >= 0 && t < n_phases ? 0u : 2u);
+    keys[i] = k;
+    vals[i] = (unsigned)i;
+    atomicAdd(&sm[k], 1u);
+  }
+  __syncthreads();
+  if (threadIdx.x < 3 && sm[threadIdx.x]) atomicAdd(&counts[threadIdx.x], (unsigned long long)sm[threadIdx.x]);
+}
+
 // NEXT-1: the wall normals are invariant under the rigid translation: kept in set-up order (k_unsort4 at
 // the set-up), gathered into the new cell order every step (k_gather4) instead of being recomputed.
 __global__ void __launch_bounds__(256)

@@ -1,14 +1,13 @@
-// sph_pair.cuh — the neighbour walk and the three pair kernels (wall extrapolation, pass A, pass B).
+// sph_pair.cuh — the neighbour-list builds and the pair kernels (wall extrapolation, pass A, pass B).
 // Included by sph.cu only.  DESIGN.md §5 describes the scheme:
 //   one thread per particle i (cell-sorted order, so a warp covers ~2 cells);
-//   phase 1  each lane walks the 9 (3-D) / 3 (2-D) x-rows of its own 27 / 9-cell stencil, every
-//            row one contiguous index range; the candidate float4 (centred image, |x|^2) is the
-//            same address for all lanes of a cell (one L1 wavefront per cell present in the warp);
-//            filter r^2 = |xj|^2 - 2 xi.xj + |xi|^2 < rc^2 + margin: 3 FFMA + 1 FSETP;
-//            survivors are appended to the lane's private shared-memory queue q[k][tid];
-//   phase 2  when any lane's queue is nearly full (and at the end) every lane drains its own queue:
-//            exact geometry from the fixed-point positions (integer subtract + I2F), then the
-//            pair physics.  Filter false positives (margin) have r >= 2h and add exactly zero.
+//   list builds (k_build, k_wall_build; only on the steps that rebuild the lists): each lane walks the 9 (3-D) /
+//            3 (2-D) x-rows of its own 27 / 9-cell stencil, every row one contiguous index range; a conservative
+//            filter (float16 staged tile in k_build, float32 otherwise) with radius 2h(1 + skin); survivors are
+//            staged in the lane's shared-memory queue and written four at a time to the warp's slot-major list;
+//   list walks (k_wall, k_pass_a, k_pass_b; every step): one coalesced 16-byte load gives 4 neighbour indices,
+//            their 256-bit records are gathered together; exact geometry from the fixed-point positions (integer
+//            subtract + I2F), then the pair physics.  Entries beyond 2h add exactly zero.
 #pragma once
 #include <cuda_fp16.h>
 
@@ -26,56 +25,15 @@
 #ifndef SPH_CH
 #define SPH_CH 4
 #endif
-#ifndef SPH_DU
-#define SPH_DU 4
-#endif
 constexpr int PB = SPH_PB;     // threads per block in the pair kernels
 constexpr int QCAP = SPH_QCAP; // queue entries per lane (QCAP * PB * 4 bytes of shared memory per block)
 constexpr int CH = SPH_CH;     // candidates per lane between two queue-occupancy votes (loads issued together)
-constexpr int DU = SPH_DU;     // queue entries drained together (their gathers issued together)
 
 // Body = struct with  Ld load(unsigned j) const  and  void apply(const Ld&)  so that the gathers of
-// DU entries are issued before the arithmetic of the first one.
+// four list entries are issued before the arithmetic of the first one.
 //
-// Sinks of the filter walk (what happens to a candidate that passes the filter):
-//   QueueSink  the lane's private shared-memory queue q[k * PB], drained by the whole warp when any
-//              lane is nearly full and at the end (used for the wall walks and by k_wall);
-//   ListSink   the per-warp neighbour list in global memory, slot-major: NL[(warp * caps + slot) * 32 + lane]
-//              (used by k_build; the fluid pair passes then read it with coalesced loads).
-template <class Body>
-struct QueueSink {
-  unsigned* q;
-  unsigned qa0, qa;
-  Body& body;
-  __device__ __forceinline__ QueueSink(unsigned* q_, Body& b) : q(q_), body(b) {
-    qa0 = (unsigned)__cvta_generic_to_shared(q_);
-    qa = qa0;
-  }
-  __device__ __forceinline__ void push(const unsigned j) {
-    asm volatile("st.shared.u32 [%0], %1;" ::"r"(qa), "r"(j) : "memory");
-    qa += PB * 4;
-  }
-  __device__ __forceinline__ void drain() {  // all lanes of the warp together
-    const int qn = (int)(qa - qa0) / (PB * 4);
-    const int nm = __reduce_max_sync(FULL, qn);
-#pragma unroll 1
-    for (int k = 0; k < nm; k += DU) {
-      decltype(body.load(0u)) ld[DU];
-#pragma unroll
-      for (int u = 0; u < DU; ++u)
-        if (k + u < qn) ld[u] = body.load(q[(k + u) * PB]);
-#pragma unroll
-      for (int u = 0; u < DU; ++u)
-        if (k + u < qn) body.apply(ld[u]);
-    }
-    qa = qa0;
-  }
-  __device__ __forceinline__ void after_chunk(const int ch = CH) {
-    if (__any_sync(FULL, qa > qa0 + (QCAP - ch) * PB * 4)) drain();
-  }
-  __device__ __forceinline__ void finish() { drain(); }
-};
-
+// ListSink: what happens to a candidate that passes the filter: the per-warp neighbour list in global memory,
+// slot-major: NL[(warp * caps + slot) * 32 + lane] (the list walks then read it with coalesced loads).
 struct ListSink {
   // Survivors are staged in the lane's shared-memory queue and written out four at a time as one
   // 16-byte store: NL is an array of uint4 groups, group g of lane l of warp w at
@@ -290,15 +248,6 @@ __device__ __forceinline__ void walk_f(const DP& p, const float4* __restrict__ A
     }
   }
   sink.finish();
-}
-
-// Queue walk = filter walk into the shared-memory queue (wall walks, k_wall).
-template <int DIM, bool EXACT, class Body>
-__device__ __forceinline__ void walk_q(const DP& p, const float4* __restrict__ A, const int* __restrict__ lb,
-                                       const bool act, const float4 ai, const int cx, const int cy,
-                                       const int cz, unsigned* __restrict__ q, Body& body) {
-  QueueSink<Body> sink(q, body);
-  walk_f<DIM, EXACT, false>(p, A, lb, act, ai, cx, cy, cz, nullptr, HCtx{}, sink, p.rc2m, p.thr_h2);
 }
 
 // List walk: every lane runs over its own column of the warp's neighbour groups; the loop is

@@ -239,3 +239,69 @@ def test_x1_hydrostatic_tank_study():
     # +-0.002 between realisations (chaotic air motion, residual acoustic wave), so the bounds are on the time averages
     assert rows[0]["l2_avg"] > 1.1 * rows[1]["l2_avg"]      # measured 0.0156 / 0.0125 and 0.0181 / 0.0117
     assert rows[1]["l2_avg"] < 0.015 and rows[2]["l2_avg"] < 0.015
+
+
+# ------------------------------------------------------------------------- the launch configuration bench.py times, at full sizes
+def _sampled_sigma_check(cfg, g, nsample=24, seed=5):
+    """sigma_i of sampled fluid particles, one by one, from the oracle's kernel (orc.kernel_w, pin P1) over ALL particles
+    at the library's current positions (brute force in float64), against the sigma_i the last pass A summed."""
+    pos = g.get_fields(device=False, which=("pos",))["pos"]
+    sig, _ = g.debug_sigma()
+    fl = np.flatnonzero(cfg["tag"] >= 0)
+    pick = np.random.default_rng(seed).choice(fl, nsample, replace=False)
+    h, dim = cfg["h"], cfg["dim"]
+    s0 = orc.sigma0(dim, h, cfg["dp"])
+    p64 = pos.astype(np.float64)
+    worst = 0.0
+    for i in pick:
+        d = p64 - p64[i]
+        near = np.flatnonzero((np.abs(d) < 2.0 * h).all(axis=1))
+        r = np.sqrt((d[near] ** 2).sum(axis=1))
+        s = sum(orc.kernel_w(dim, h, float(x)) for x in r[r < 2.0 * h])     # includes the self term r = 0
+        worst = max(worst, abs(float(sig[i]) - s) / s0)
+    return worst
+
+
+def test_cfg4_256_graph_replay_is_the_direct_path_bitwise_and_sampled_sigma():
+    """The configuration `python bench.py` times (config 4 at 16.8 M, sph_step = CUDA-graph replay with the rebuild
+    branch as an IF node, device-computed dt) against the plain-launch path the oracle comparisons above drive
+    (`test_cfg4_256_fields_after_setup_and_2_steps`): 6 steps, every field bit for bit; then sigma_i of sampled particles
+    against the oracle's kernel summed by brute force."""
+    cfg = inputs.box_sweep_3d(n=256)
+    out = []
+    for flags in (cfg["flags"], cfg["flags"] | sph.FLAG_NO_GRAPH):
+        g = sph.Sph(dict(cfg, flags=flags))
+        g.set_particles(cfg["pos"], cfg["vel"], cfg["rho"], cfg["tag"])
+        g.step(6)
+        s = g.get_stats(with_pairs=False)
+        assert s["steps"] == 6 and s["escaped"] == 0 and s["nonfinite"] == 0 and s["rebuilds"] >= 2
+        out.append((g.get_fields(device=False), s["rebuilds"], s["dt"]))
+        if flags == cfg["flags"]:
+            # float32 positions at 2.6 m carry 2.4e-7 m: sigma from them is good to 1e-5 sigma0 (the library sums it from
+            # its 32-bit fixed-point positions); a dropped neighbour would show as >= 1e-3 sigma0
+            assert _sampled_sigma_check(cfg, g) < 5e-5
+        g.close()
+    assert out[0][1] == out[1][1] and out[0][2] == out[1][2]
+    for k in out[0][0]:
+        assert np.array_equal(out[0][0][k], out[1][0][k]), k
+
+
+def test_cfg4_400_64m_properties_and_sampled_sigma():
+    """Config 4 at its largest size (64 M fluid + 2.9 M wall particles, 84 GB on the device): what holds at any size
+    (mass, no escapes, no list overflow, the pair count against the lattice count of pin P2, finite fields) after the
+    set-up and 3 graph-replayed steps, and sigma_i of sampled particles against the oracle's kernel by brute force."""
+    n = 400
+    cfg = inputs.box_sweep_3d(n=n)
+    g = sph.Sph(cfg)
+    g.set_particles(cfg["pos"], cfg["vel"], cfg["rho"], cfg["tag"])
+    g.step(3)
+    s = g.get_stats()
+    assert s["n_fluid"] == n ** 3 and s["escaped"] == 0 and s["nonfinite"] == 0 and s["steps"] == 3
+    assert abs(s["mass"] - 1000.0 * (n * cfg["dp"]) ** 3) < 1e-6 * s["mass"]
+    assert 78.0 < s["npairs"] / n ** 3 < 81.0
+    assert _sampled_sigma_check(cfg, g, nsample=12) < 1e-4        # float32 positions at 4 m: 4.8e-7 m
+    f = g.get_fields(device=False, which=("acc", "rho"))
+    fl = cfg["tag"] >= 0
+    assert np.isfinite(f["acc"]).all() and np.all(f["acc"][~fl] == 0)
+    assert np.all(np.abs(f["rho"][fl] / 1000.0 - 1.0) < 0.01)
+    g.close()
