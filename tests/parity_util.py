@@ -81,3 +81,44 @@ def extra_bound(cfg):
     """Largest share of list entries that may lie outside 2h: the lists are built with radius 2h(1 + s) (Verlet
     skin, include/sph.h list_skin) by a conservative filter whose own margin is below 7 %."""
     return 1.0 - 1.0 / (1.07 * (1.0 + skin_of(cfg)) ** cfg["dim"])
+
+
+def check_step_lists(cfg, g, grid):
+    """Host-side check of the lists the passes READ (sph_debug_step_lists: NL + NLW per fluid particle, NLF
+    per wall particle) against the oracle's float32 contract lists at the library's current positions:
+    every contract neighbour is in the row; every other entry is the self entry or a filter extra whose
+    distance is within the documented margin (r < 1.03 * 2h (1 + s) at the list build, and the
+    pair has moved apart by at most 2 h s since, s = list_skin; it adds exactly 0)."""
+    pos = g.get_fields(device=False, which=("pos",))["pos"]
+    tag = cfg["tag"]
+    off, ids = g.debug_step_lists()
+    roff, rids = orc.f32_neighbours(cfg, pos, tag, grid=grid)
+    n = len(tag)
+    assert len(off) == n + 1 and len(roff) == n + 1
+    p64 = pos.astype(np.float64)
+    rc = 2.0 * cfg["h"]
+    rl = rc * (1.0 + skin_of(cfg))
+    n_extra = 0
+    cnt = off[1:] - off[:-1]
+    rcnt = roff[1:] - roff[:-1]
+    assert np.all(cnt >= rcnt)
+    # rows as (row id, neighbour id) keys: set algebra in numpy (rows of 4.5 M particles in seconds)
+    rowg = np.repeat(np.arange(n, dtype=np.int64), cnt)
+    rowr = np.repeat(np.arange(n, dtype=np.int64), rcnt)
+    keyg = rowg * n + ids.astype(np.int64)
+    keyr = rowr * n + rids.astype(np.int64)
+    assert len(np.unique(keyg)) == len(keyg), "duplicate entry in a list row"
+    missing = np.setdiff1d(keyr, keyg, assume_unique=True)
+    assert missing.size == 0, ("contract neighbours missing from the lists the passes read", missing[:5] // n, missing[:5] % n)
+    extra = np.setdiff1d(keyg, keyr, assume_unique=True)
+    ei, ej = extra // n, extra % n
+    self_entry = ei == ej
+    assert np.all(tag[ei[self_entry]] >= 0)                       # only fluid rows hold a self entry
+    assert self_entry.sum() == int((tag >= 0).sum())              # ... and every fluid row holds exactly one
+    xi, xj = ei[~self_entry], ej[~self_entry]
+    d = np.linalg.norm(p64[xi] - p64[xj], axis=1)
+    assert np.all(d >= rc * (1.0 - 1e-6)) and np.all(d < 1.03 * rl + (rl - rc))   # built within 1.03 rl, apart by at most 2 h s since, (d.min() if d.size else None, d.max() if d.size else None)
+    # a wall row holds fluid entries only, a fluid row fluid and wall entries
+    assert np.all(tag[ej[tag[ei] < 0]] >= 0)
+    n_extra = int(xi.size)
+    return n_extra, int(len(keyg))
