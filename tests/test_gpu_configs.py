@@ -308,3 +308,46 @@ def test_cfg4_400_64m_properties_and_sampled_sigma():
     dev = np.abs(f["rho"][fl] / 1000.0 - 1.0)     # hydrostatic 0.5 % + the jittered lattice's sigma spread through Eq. 2.17
     assert float(dev.mean()) < 0.03 and float(dev.max()) < 0.25, (float(dev.mean()), float(dev.max()))
     g.close()
+
+
+# ------------------------------------------------------------------------- long runs: integral quantities (BASELINE.json north_star)
+def _long_run(cfg, nsteps, chunk, ek_tol=0.01, front=True):
+    """sph_step (graph replay, device-computed dt, kept lists) against the oracle's own run with its own dt, `nsteps`
+    steps (BASELINE.json's step count of the configuration): total mass exact, kinetic energy and surge front within
+    1 % at every `chunk` steps, no particle lost, the lists rebuilt now and then but not every step."""
+    o, g = make_pair(cfg)
+    m0 = g.get_stats(with_pairs=False)["mass"]
+    done = 0
+    while done < nsteps:
+        o.step(chunk)
+        g.step(chunk)
+        done += chunk
+        so, sg = o.stats(), g.get_stats(with_pairs=False)
+        assert sg["escaped"] == 0 and sg["nonfinite"] == 0 and so["escaped"] == 0, (done, sg)
+        assert sg["mass"] == m0 and abs(m0 - so["mass"]) <= 1e-9 * so["mass"]
+        assert abs(sg["t"] - so["t"]) < 1e-4 * so["t"], (done, sg["t"], so["t"])
+        assert abs(sg["ek"] - so["ek"]) <= ek_tol * so["ek"] + 1e-12, (done, sg["ek"], so["ek"])
+        if front:
+            assert abs(sg["x_front"] - so["x_front"]) < 0.01 * abs(so["x_front"]), (done, sg["x_front"], so["x_front"])
+    assert 2 <= sg["rebuilds"] < nsteps, sg["rebuilds"]
+    return so, sg
+
+
+def test_cfg1_geometry_1000_steps_integral_quantities():
+    """Config 1 (3-D dam break with the box obstacle) over its 1000 steps at dp = 0.02 (83 875 fluid particles: the
+    oracle takes a minute)."""
+    cfg = inputs.dam_break_3d_box(dp=0.02)
+    _long_run(cfg, 1000, 250)
+
+
+@pytest.mark.parametrize("equal_c", [True, False])
+def test_cfg2_geometry_2000_steps_integral_quantities(equal_c):
+    """Config 2 (2-D water / air dam break, density ratio 1000) over its 2000 steps at dp = 0.025 (25 680 fluid)."""
+    cfg = inputs.two_phase_2d(dp=0.025, equal_c=equal_c)
+    _long_run(cfg, 2000, 500)
+
+
+def test_cfg3_geometry_500_steps_integral_quantities():
+    """Config 3 (sloshing box with 8 seeded spheres, gravity tilting) over its 500 steps at dp = 0.02."""
+    cfg = inputs.sloshing_spheres_3d(dp=0.02)
+    _long_run(cfg, 500, 250, front=False)      # a filled box has no surge front; E_k and mass are the integral quantities
