@@ -404,7 +404,7 @@ k_build(const DP p, SS* __restrict__ S, const int nf, const float4* __restrict__
   const bool act = i0 < nf;
   const int i = act ? i0 : nf - 1;
   const float4 ai = A[i];
-  const unsigned key = K[i];
+  const unsigned key = K[i] >> p.sub_bits;   // the cell id sits above the sub-cell Morton bits of the sort key
   int cx, cy, cz;
   cell_of_key(p, key, cx, cy, cz);
   HCtx hc;
@@ -456,7 +456,7 @@ k_wall_build(const DP p, SS* __restrict__ S, const int nw, const float4* __restr
   uint4* col = NLF + (size_t)(w0 >> 5) * (capsf >> 2) * 32 + (threadIdx.x & 31);
   const float4 ai = WA[w];
   int cx, cy, cz;
-  cell_of_key(p, WK[w], cx, cy, cz);
+  cell_of_key(p, WK[w] >> p.sub_bits, cx, cy, cz);
   ListSink sink(qs + threadIdx.x, col, capsf >> 2);
   walk_f<DIM, EXACT, false>(p, A, lbF, act, ai, cx, cy, cz, nullptr, HCtx{}, sink, S->rl2m, S->thr_h2);
   if (act) {
