@@ -689,24 +689,35 @@ int sph_create(const sph_params* prm, sph_ctx** out) {
       }
     }
     d.sub_per_m = 1024.0 / d.Q;
-    d.Qf = (float)d.Q; d.qh = (float)(d.Q / h); d.qhD = d.Q / h;
-    d.mhqD[0] = -0.5 * d.qhD; d.mhqD[1] = d.mhqD[0] / 1024.0; d.tqD[0] = 2.0 * d.qhD; d.tqD[1] = d.tqD[0] / 1024.0;
-    // sigma from residual-exact separations (k_pass_a<.., SUBQ>, +15 % on pass A) when the quantum is coarse for
-    // the case: positions rounded to Q leave about 15 (Q / h) (L_g / h) |g| in the acceleration, L_g the extent
-    // of the domain along gravity (measured: 5.5e-4 |g| at config 4's 16.8 M size, Q / h = 1.4e-7, L_g / h = 200;
-    // 5.5e-5 with the residuals in p); the 1e-4 bar decides.  Multi-phase runs always.
+    d.Qs = d.Q / 1024.0;
+    // pair unit Qp = Q / 2^mbits (sph_common.cuh "fixed-point master positions"): the largest mbits <= 10 for which
+    // 2.5 list radii — more than any two particles of one stencil are apart along an axis — stay below 2^30 Qp, so
+    // that a wrapping 32-bit subtraction is their exact separation and the 64-bit integer r^2 cannot overflow
+    d.mbits = 0;
+    while (d.mbits < 10 && 2.5 * rl / (d.Q / (double)(2 << d.mbits)) < 1073741824.0) ++d.mbits;
+    if (getenv("SPH_MBITS")) d.mbits = std::min(d.mbits, std::max(0, atoi(getenv("SPH_MBITS"))));   // measurement switch
+    d.lobits = 10 - d.mbits;
+    d.Qp = d.Q / (double)(1 << d.mbits);
+    d.sub_scale = (float)(1 << d.lobits); d.sub_half_inv = 0.5f / (float)(1 << d.lobits);
+    d.Qf = (float)d.Qp; d.qh = (float)(d.Qp / h); d.qhD = d.Qp / h;
+    d.mhqD[0] = -0.5 * d.qhD; d.mhqD[1] = -0.5 * d.Qs / h; d.tqD[0] = 2.0 * d.qhD; d.tqD[1] = 2.0 * d.Qs / h;
+    // sigma from separations that include the bits below the record's word (k_pass_a<.., SUBQ>, +15 % on pass A) when
+    // the pair unit is coarse for the case: positions rounded to a unit U leave about 15 (U / h) (L_g / h) |g| in the
+    // acceleration, L_g the extent of the domain along gravity (measured with U = Q: 5.5e-4 |g| at config 4's 16.8 M
+    // size, Q / h = 1.4e-7, L_g / h = 200); the 1e-4 bar decides.  With the pair unit Qp = Q / 2^mbits this is off for
+    // every single-phase configuration of BASELINE.json; multi-phase runs always take it.
     {
       double gn = 0, Lg = 0;
       for (int k = 0; k < prm->dim; ++k) gn += prm->g[k] * prm->g[k];
       for (int k = 0; k < prm->dim; ++k)
         Lg += (gn > 0 ? fabs(prm->g[k]) / sqrt(gn) : 0.0) * (prm->domain_max[k] - prm->domain_min[k]);
       if (!(gn > 0)) Lg = Lmax;
-      d.subq = (prm->n_phases > 1 || 15.0 * (d.Q / h) * (Lg / h) > 1e-4) ? 1 : 0;
+      d.subq = (prm->n_phases > 1 || 15.0 * (d.Qp / h) * (Lg / h) > 1e-4) ? 1 : 0;
       if (getenv("SPH_FORCE_SUBQ")) d.subq = 1;   // measurement switches (profiles/): not part of the interface
       if (getenv("SPH_NO_SUBQ") && prm->n_phases == 1) d.subq = 0;
     }
-    d.gradcQ = (float)(-5.0 * alpha / (h * h) * d.Q);
-    d.two_over_dp = (float)(2.0 * d.Q / dp);
+    d.gradcQ = (float)(-5.0 * alpha / (h * h) * d.Qp);
+    d.two_over_dp = (float)(2.0 * d.Qp / dp);
     // candidate filter margin: rounding of the expanded form |xj|^2 - 2 xi.xj + |xi|^2 on images
     // of magnitude <= R, plus the rounding of the images themselves
     const double R = sqrt(R2), u = ldexp(1.0, -24);

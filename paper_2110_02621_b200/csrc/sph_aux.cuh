@@ -5,7 +5,6 @@
 
 #include "sph_common.cuh"
 
-constexpr unsigned RES_MID = (512u << 22) | (512u << 12) | (512u << 2);  // zero residual on every axis
 
 // ------------------------------------------------------------------------------------------
 // Loading (sph_set_particles): split caller arrays into the fluid / wall structures.
@@ -19,11 +18,12 @@ __global__ void k_load(DP p, int n, int is_wall, const int* __restrict__ idx, co
   const int o = idx[i];
   const int ph = is_wall ? 0 : tag[o];
   uint4 x;
-  unsigned rx, ry, rz = 512u;
-  x.x = fx_from_double((double)pos[3 * o], p.O[0], p.Q, rx);
-  x.y = fx_from_double((double)pos[3 * o + 1], p.O[1], p.Q, ry);
-  x.z = p.dim == 3 ? fx_from_double((double)pos[3 * o + 2], p.O[2], p.Q, rz) : 0u;
-  x.w = (rx << 22) | (ry << 12) | (rz << 2) | (unsigned)ph;
+  unsigned fx, fy, fz = 0u;
+  fx_split(p, fx_tot_from_double((double)pos[3 * o], p.O[0], p.Q), x.x, fx);
+  fx_split(p, fx_tot_from_double((double)pos[3 * o + 1], p.O[1], p.Q), x.y, fy);
+  x.z = 0u;
+  if (p.dim == 3) fx_split(p, fx_tot_from_double((double)pos[3 * o + 2], p.O[2], p.Q), x.z, fz);
+  x.w = fx_pack(fx, fy, fz, (unsigned)ph);
   TX[i] = x;
   if (is_wall) {
     TB[i] = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -32,8 +32,7 @@ __global__ void k_load(DP p, int n, int is_wall, const int* __restrict__ idx, co
     TB[i] = make_float4(vel[3 * o], vel[3 * o + 1], p.dim == 3 ? vel[3 * o + 2] : 0.0f, drho);
   }
   ID[i] = (unsigned)o;
-  keys[i] = sort_key(p, fx_image(x.x, p.O[0], p.Q), fx_image(x.y, p.O[1], p.Q),
-                     p.dim == 3 ? fx_image(x.z, p.O[2], p.Q) : 0.0f);
+  keys[i] = sort_key(p, fx_image(p, x, 0), fx_image(p, x, 1), p.dim == 3 ? fx_image(p, x, 2) : 0.0f);
   vals[i] = (unsigned)i;
 }
 
@@ -76,6 +75,18 @@ k_gatherx(int n, const unsigned* __restrict__ vals, const uint4* __restrict__ in
   if (s < n) out[s] = in[vals[s]];
 }
 
+// a wall particle's set-up position displaced by the wall motion of t^{n+1} (S->sq: units of Q = 1024 units of the
+// 42-bit coordinate); the sum stays inside the span because the domain box contains the whole excursion
+__device__ __forceinline__ uint4 wall_shifted(const DP& p, const SS* __restrict__ S, uint4 x) {
+  unsigned f[3] = {fx_field(x, 0), fx_field(x, 1), fx_field(x, 2)};
+  unsigned w[3] = {x.x, x.y, x.z};
+  for (int k = 0; k < p.dim; ++k) {
+    const long long t = (long long)fx_tot(p, w[k], f[k]) + ((long long)S->sq[k] << 10);
+    fx_split(p, (unsigned long long)min(max(t, 0ll), 4398046511103ll), w[k], f[k]);
+  }
+  return make_uint4(w[0], w[1], w[2], fx_pack(f[0], f[1], f[2], x.w & 3u));
+}
+
 // NEXT-1 (moving walls): wall particles in set-up order at their displaced positions X0 + sq, with the
 // cell hash of the new position; input of the per-step wall re-sort.
 __global__ void __launch_bounds__(256)
@@ -83,13 +94,10 @@ k_wall_shift(DP p, const SS* __restrict__ S, int nw, const uint4* __restrict__ X
              float4* __restrict__ TB, unsigned* __restrict__ keys, unsigned* __restrict__ vals) {
   const int i = blockIdx.x * 256 + threadIdx.x;
   if (i >= nw) return;
-  uint4 x = X0[i];
-  x.x += (unsigned)S->sq[0]; x.y += (unsigned)S->sq[1];
-  if (p.dim == 3) x.z += (unsigned)S->sq[2];
+  const uint4 x = wall_shifted(p, S, X0[i]);
   TX[i] = x;
   TB[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-  keys[i] = sort_key(p, fx_image(x.x, p.O[0], p.Q), fx_image(x.y, p.O[1], p.Q),
-                     p.dim == 3 ? fx_image(x.z, p.O[2], p.Q) : 0.0f);
+  keys[i] = sort_key(p, fx_image(p, x, 0), fx_image(p, x, 1), p.dim == 3 ? fx_image(p, x, 2) : 0.0f);
   vals[i] = (unsigned)i;
 }
 
@@ -181,16 +189,12 @@ k_dt(DP p, SS* __restrict__ S, int nf, const float4* __restrict__ B, const doubl
   S->escaped = 0ull;
 }
 
-// One axis of the drift Eq. 2.20 on the fixed-point master position: (X, residual) is a 42-bit
-// integer in units of Q/1024; the displacement dt*v is rounded to that unit.
-__device__ __forceinline__ unsigned drift_axis(unsigned X, unsigned& res, double disp_sub) {
-  long long tot = ((long long)X << 10) + ((long long)res - 512) + __double2ll_rn(disp_sub);
-  long long Xn = (tot + 512) >> 10;
-  long long rn = tot - (Xn << 10) + 512;
-  if (Xn < 0) { Xn = 0; rn = 512; }
-  if (Xn > 4294967295ll) { Xn = 4294967295ll; rn = 512; }
-  res = (unsigned)rn;
-  return (unsigned)Xn;
+// One axis of the drift Eq. 2.20 on the fixed-point master position: the coordinate is a 42-bit integer in units
+// of Q/1024; the displacement dt*v is rounded to that unit.
+__device__ __forceinline__ void drift_axis(const DP& p, unsigned& mid, unsigned& field, double disp_sub) {
+  long long tot = (long long)fx_tot(p, mid, field) + __double2ll_rn(disp_sub);
+  tot = min(max(tot, 0ll), 4398046511103ll);
+  fx_split(p, (unsigned long long)tot, mid, field);
 }
 
 // Predictor: density reinitialisation Eq. 2.17 / 2.18 from the sigma_i of the last pass A
@@ -234,11 +238,11 @@ k_predict(DP p, SS* __restrict__ S, int nf, const XB* __restrict__ R, float4* __
       const bool fin = isfinite(b.x) && isfinite(b.y) && isfinite(b.z);
       if (fin) {
         const double k = S->dt_d * p.sub_per_m;
-        unsigned rx = (x.w >> 22) & 1023u, ry = (x.w >> 12) & 1023u, rz = (x.w >> 2) & 1023u;
-        x.x = drift_axis(x.x, rx, k * (double)b.x);
-        x.y = drift_axis(x.y, ry, k * (double)b.y);
-        if (p.dim == 3) x.z = drift_axis(x.z, rz, k * (double)b.z);
-        x.w = (rx << 22) | (ry << 12) | (rz << 2) | (unsigned)ph;
+        unsigned fx = fx_field(x, 0), fy = fx_field(x, 1), fz = fx_field(x, 2);
+        drift_axis(p, x.x, fx, k * (double)b.x);
+        drift_axis(p, x.y, fy, k * (double)b.y);
+        if (p.dim == 3) drift_axis(p, x.z, fz, k * (double)b.z);
+        x.w = fx_pack(fx, fy, fz, (unsigned)ph);
         // this step's displacement, rounded up: |dx| <= dt |v| (1 + 2^-20) + one sub-quantum per axis
         const float dtf = S->dt * 1.000001f;
         d2 = dtf * dtf * fmaf(b.z, b.z, fmaf(b.y, b.y, b.x * b.x));
@@ -246,8 +250,8 @@ k_predict(DP p, SS* __restrict__ S, int nf, const XB* __restrict__ R, float4* __
         atomicAdd(&S->nonfinite, 1ull);
       }
       TX[i] = x;
-      const float gx = fx_image(x.x, p.O[0], p.Q), gy = fx_image(x.y, p.O[1], p.Q);
-      const float gz = p.dim == 3 ? fx_image(x.z, p.O[2], p.Q) : 0.0f;
+      const float gx = fx_image(p, x, 0), gy = fx_image(p, x, 1);
+      const float gz = p.dim == 3 ? fx_image(p, x, 2) : 0.0f;
       bool out = gx < p.dmin[0] || gx >= p.dmax[0] || gy < p.dmin[1] || gy >= p.dmax[1];
       if (p.dim == 3) out = out || gz < p.dmin[2] || gz >= p.dmax[2];
       if (out || !fin) atomicAdd(&S->escaped, 1ull);
@@ -314,10 +318,7 @@ __global__ void __launch_bounds__(256)
 k_wall_move(DP p, const SS* __restrict__ S, int nw, const uint4* __restrict__ WXB, XB* __restrict__ WR) {
   const int i = blockIdx.x * 256 + threadIdx.x;
   if (i >= nw) return;
-  uint4 x = WXB[i];
-  x.x += (unsigned)S->sq[0]; x.y += (unsigned)S->sq[1];
-  if (p.dim == 3) x.z += (unsigned)S->sq[2];
-  WR[i].x = x;
+  WR[i].x = wall_shifted(p, S, WXB[i]);
 }
 
 // Wall normals, Eq. 2.16, once, in float64 (reading A10).
@@ -347,8 +348,8 @@ __global__ void k_normals(DP p, int nw, const XB* __restrict__ WR, const unsigne
       for (int j = s; j < e; ++j) {
         if (j == w) continue;
         const uint4 xj = WR[j].x;
-        const double dx = p.Q * (double)(int)(xi.x - xj.x), dyy = p.Q * (double)(int)(xi.y - xj.y),
-                     dzz = DIM == 3 ? p.Q * (double)(int)(xi.z - xj.z) : 0.0;
+        const double dx = p.Qp * (double)(int)(xi.x - xj.x), dyy = p.Qp * (double)(int)(xi.y - xj.y),
+                     dzz = DIM == 3 ? p.Qp * (double)(int)(xi.z - xj.z) : 0.0;
         const double r2 = dx * dx + dyy * dyy + dzz * dzz;
         if (!(r2 < rc2) || r2 == 0.0) continue;
         const double r = sqrt(r2), q = r / h, t = 1.0 - 0.5 * q;

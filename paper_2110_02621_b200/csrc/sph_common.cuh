@@ -3,11 +3,11 @@
 //
 // Data layout.  Fluid and wall particles live in separate cell-sorted arrays:
 //   (X4 and B4 are interleaved in one 32-byte record XB per particle)
-//   X4  uint4   fixed-point master position (X, Y, Z) in units of Q = 2^-k m from the origin O,
-//               .w = residual of each axis in units of Q/1024 (3 x 10 bits, biased by 512) << 2 | phase
+//   X4  uint4   fixed-point master position: the middle 32 bits of each 42-bit coordinate (units of Qp = Q / 2^mbits,
+//               modulo 2^32; Q = 2^-k m), .w = the 10 bits above and below them per axis (3 x 10 bits) << 2 | phase
 //   A4  float4  float32 image centred on the domain centre (xc, yc, zc, |xc|^2): candidate test only
 //   B4  float4  (vx, vy, vz, rho - rho0_phase); walls: (v_w, p_w)
-// Pair geometry is an exact integer subtraction of X4 followed by int->float, in units of Q.
+// Pair geometry is an exact wrapping integer subtraction of X4 followed by int->float, in units of Qp.
 #pragma once
 #include <cuda_runtime.h>
 #include <math.h>
@@ -23,20 +23,23 @@ struct DP {
   int subq;          // 1: sigma from separations that include the 10-bit residuals (k_pass_a<.., SUBQ>)
   float inv_h;       // float16 filter of k_build: coordinates in units of h
   unsigned thr_h2;   // its threshold on r^2 / h^2 (half2, both halves): 4.08 + the float32 image margin
-  float qh;        // Q / h: q = r_Q * qh
-  float Qf;        // Q
-  float gradcQ;    // W'(r)/r * r_ij = gradcQ * (1 - q/2)^3 * d_Q,   gradc = -5 alpha / h^2
+  int mbits, lobits;  // pair unit Qp = Q / 2^mbits; lobits = 10 - mbits bits of a coordinate lie below the record's word
+  float sub_scale, sub_half_inv;  // 2^lobits and 0.5 / 2^lobits (float64 sigma term with the low bits, w64)
+  float qh;        // Qp / h: q = r_Qp * qh
+  float Qf;        // Qp
+  float gradcQ;    // W'(r)/r * r_ij = gradcQ * (1 - q/2)^3 * d_Qp,   gradc = -5 alpha / h^2
   float alpha, V0;
   float rho0[SPH_MAX_PHASES], c0[SPH_MAX_PHASES], c2[SPH_MAX_PHASES], inv_c2[SPH_MAX_PHASES],
       mass[SPH_MAX_PHASES];
-  float gamma_p, two_over_dp;  // two_over_dp holds 2 Q / dp (delta of Eq. 2.15 from Q units)
+  float gamma_p, two_over_dp;  // two_over_dp holds 2 Qp / dp (delta of Eq. 2.15 from Qp units)
   unsigned pen_mask, fs_mask, flags;
   float ox, oy, oz, inv_edge;  // contract cell hash (reading A24)
   int nx, ny, nz;
   float dmin[3], dmax[3];
   double O[3], C[3], Q, sub_per_m;  // fixed point: origin, image centre, quantum, 1024 / Q
-  double cmax, cfl, hD, dpD, qhD;  // qhD = Q / h
-  double mhqD[2], tqD[2];          // -q/2 and 2q per unit of r: [0] r in Q, [1] r in Q/1024 (w64)
+  double Qs, Qp;                    // Q / 1024 (unit of the 42-bit coordinate), Q / 2^mbits (unit of the pair geometry)
+  double cmax, cfl, hD, dpD, qhD;  // qhD = Qp / h
+  double mhqD[2], tqD[2];          // -q/2 and 2q per unit of r: [0] r in Qp, [1] r in Q/1024 (w64)
   double massD[SPH_MAX_PHASES];
   double a_over_s0;
   double g[3], gamp[3], gperiod;
@@ -123,30 +126,47 @@ __device__ __forceinline__ float warp_sum(float v) {
 }
 
 // ---- fixed-point master positions ---------------------------------------------------------
-// x -> (X, residual): the position in units of Q/1024 rounded to an integer, split into the 32-bit
-// fixed-point word and the 10-bit residual (biased by 512).  Saturates outside the span; NaN -> 0.
-__device__ __forceinline__ unsigned fx_from_double(double x, double O, double Q, unsigned& res) {
+// A coordinate is a 42-bit unsigned integer T in units of Q/1024 from the origin O (span 2^32 Q >= 1.5 L + 16 h).
+// The record does not hold its top 32 bits but its MIDDLE 32 bits, T >> lobits (lobits = 10 - mbits): positions
+// modulo 2^32 quanta of Qp = Q / 2^mbits.  The separation of two particles that are within a stencil of each other
+// is then still one exact wrapping 32-bit subtraction (mbits is chosen so that 2.5 list radii stay below 2^30 Qp),
+// but in units 2^mbits times finer than Q: on metre-sized domains the pair geometry resolves 10^-11 m instead of
+// 10^-9 m at no cost in the pair loops.  The mbits bits above and the lobits bits below the word sit in a 10-bit
+// field per axis of the record's fourth word, (top << lobits) | low; only the drift, the cell hash, the output and
+// (multi-phase runs) the residual-exact sigma term read them.  Saturates outside the span; NaN -> 0.
+__device__ __forceinline__ unsigned long long fx_tot_from_double(double x, double O, double Q) {
   double u = rint((x - O) / Q * 1024.0);
-  u = fmin(fmax(u, 0.0), 4294967295.0 * 1024.0);
-  const long long tot = (long long)u;
-  long long X = (tot + 512) >> 10;
-  if (X > 4294967295ll) X = 4294967295ll;
-  res = (unsigned)(tot - (X << 10) + 512);
-  if (res > 1023u) res = 512u;
-  return (unsigned)X;
+  u = fmin(fmax(u, 0.0), 4398046511103.0);   // 2^42 - 1
+  return (unsigned long long)u;
 }
-__device__ __forceinline__ double fx_to_double(unsigned X, double O, double Q) {
-  return fma((double)X, Q, O);  // exact: Q is a power of two, O a multiple of Q
+__device__ __forceinline__ unsigned long long fx_tot(const DP& p, unsigned mid, unsigned field) {
+  const unsigned lomask = (1u << p.lobits) - 1u;
+  return ((unsigned long long)(field >> p.lobits) << (32 + p.lobits)) | ((unsigned long long)mid << p.lobits) |
+         (unsigned long long)(field & lomask);
+}
+__device__ __forceinline__ void fx_split(const DP& p, unsigned long long tot, unsigned& mid, unsigned& field) {
+  const unsigned lomask = (1u << p.lobits) - 1u;
+  mid = (unsigned)(tot >> p.lobits);
+  field = ((unsigned)(tot >> (32 + p.lobits)) << p.lobits) | ((unsigned)tot & lomask);
+}
+__device__ __forceinline__ unsigned fx_field(const uint4& x, int k) { return (x.w >> (22 - 10 * k)) & 1023u; }
+__device__ __forceinline__ unsigned fx_word(const uint4& x, int k) { return k == 0 ? x.x : (k == 1 ? x.y : x.z); }
+__device__ __forceinline__ unsigned fx_pack(unsigned fx, unsigned fy, unsigned fz, unsigned phase) {
+  return (fx << 22) | (fy << 12) | (fz << 2) | phase;
+}
+// the coordinate in metres: exact (Q a power of two, O a multiple of Q, 42 + few bits)
+__device__ __forceinline__ double fx_pos(const DP& p, const uint4& x, int k) {
+  return fma((double)fx_tot(p, fx_word(x, k), fx_field(x, k)), p.Qs, p.O[k]);
 }
 // float32 image of the master position (what sph_get_fields returns and the cell hash sees)
-__device__ __forceinline__ float fx_image(unsigned X, double O, double Q) { return (float)fx_to_double(X, O, Q); }
+__device__ __forceinline__ float fx_image(const DP& p, const uint4& x, int k) { return (float)fx_pos(p, x, k); }
 
 __device__ __forceinline__ int phase_of(const uint4& x) { return (int)(x.w & 3u); }
 
 __device__ __forceinline__ float4 centred_image(const DP& p, const uint4& x) {
-  const float a = (float)(fx_to_double(x.x, p.O[0], p.Q) - p.C[0]);
-  const float b = (float)(fx_to_double(x.y, p.O[1], p.Q) - p.C[1]);
-  const float c = p.dim == 3 ? (float)(fx_to_double(x.z, p.O[2], p.Q) - p.C[2]) : 0.0f;
+  const float a = (float)(fx_pos(p, x, 0) - p.C[0]);
+  const float b = (float)(fx_pos(p, x, 1) - p.C[1]);
+  const float c = p.dim == 3 ? (float)(fx_pos(p, x, 2) - p.C[2]) : 0.0f;
   return make_float4(a, b, c, fmaf(c, c, fmaf(b, b, a * a)));
 }
 

@@ -8,8 +8,7 @@ __global__ void k_image(DP p, int n, const XB* __restrict__ R, float4* __restric
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   const uint4 x = R[i].x;
-  G[i] = make_float4(fx_image(x.x, p.O[0], p.Q), fx_image(x.y, p.O[1], p.Q),
-                     p.dim == 3 ? fx_image(x.z, p.O[2], p.Q) : 0.0f, 0.0f);
+  G[i] = make_float4(fx_image(p, x, 0), fx_image(p, x, 1), p.dim == 3 ? fx_image(p, x, 2) : 0.0f, 0.0f);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -83,9 +82,9 @@ __global__ void k_get(DP p, int n, int is_wall, const XB* __restrict__ R, const 
   const float4 b = B ? B[i] : R[i].b;
   const size_t o = ID[i];
   if (pos) {
-    pos[3 * o] = fx_image(x.x, p.O[0], p.Q);
-    pos[3 * o + 1] = fx_image(x.y, p.O[1], p.Q);
-    pos[3 * o + 2] = p.dim == 3 ? fx_image(x.z, p.O[2], p.Q) : 0.0f;
+    pos[3 * o] = fx_image(p, x, 0);
+    pos[3 * o + 1] = fx_image(p, x, 1);
+    pos[3 * o + 2] = p.dim == 3 ? fx_image(p, x, 2) : 0.0f;
   }
   if (vel) { vel[3 * o] = b.x; vel[3 * o + 1] = b.y; vel[3 * o + 2] = b.z; }
   if (is_wall) {  // B = (v_w, p_w)
@@ -141,8 +140,8 @@ k_stats(DP p, int nf, const XB* __restrict__ R, const float4* __restrict__ B, St
     ek += 0.5 * p.massD[ph] * ((double)v.x * v.x + (double)v.y * v.y + (double)v.z * v.z);
 #pragma unroll
     for (int k = 0; k < SPH_MAX_PHASES; ++k) cnt[k] += (ph == k);
-    const float zz = up == 2 ? fx_image(x.z, p.O[2], p.Q) : fx_image(x.y, p.O[1], p.Q);
-    if (ph == 0 && zz < zlim) xf = fmaxf(xf, fx_image(x.x, p.O[0], p.Q));
+    const float zz = fx_image(p, x, up);
+    if (ph == 0 && zz < zlim) xf = fmaxf(xf, fx_image(p, x, 0));
   }
   for (int o = 16; o > 0; o >>= 1) {
     ek += __shfl_xor_sync(FULL, ek, o);

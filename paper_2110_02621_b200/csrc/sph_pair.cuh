@@ -274,7 +274,7 @@ __device__ __forceinline__ void walk_l(const uint4* g, const int cnt, Body& body
   }
 }
 
-// Exact pair geometry in units of Q from the fixed-point positions: d = X_i - X_j (wrapping
+// Exact pair geometry in units of Qp from the fixed-point positions: d = X_i - X_j (wrapping
 // integer subtract, exact), r^2, 1/r (r = 0 -> r = 0 with a finite 1/r), q = r/h and the
 // Wendland C2 factors (reading A1): w = (1 - q/2)^4 (1 + 2q) = W / alpha_d,  f = (1 - q/2)^3.
 // MUFU.RSQ / MUFU.RCP are accurate to about 2^-22 and their error is a smooth function of the
@@ -341,14 +341,16 @@ __device__ __forceinline__ double w64(const DP& p, const uint4& xi, const uint4&
   const long long dx = (int)(xi.x - xj.x), dy = (int)(xi.y - xj.y), dz = DIM == 3 ? (int)(xi.z - xj.z) : 0;
   double r2, r0, hy;
   if (SUBQ) {
-    // multi-phase: include the 10-bit residuals (units of Q/1024).  For a light phase with its own
-    // large c0 (config 2b: c_air^2 = 1000 c_w^2) sigma must be good to 1e-11, i.e. positions to 1e-12 m.
-    const double ex = (double)((dx << 10) + (int)((xi.w >> 22) & 1023u) - (int)((xj.w >> 22) & 1023u));
-    const double ey = (double)((dy << 10) + (int)((xi.w >> 12) & 1023u) - (int)((xj.w >> 12) & 1023u));
-    const double ez = DIM == 3 ? (double)((dz << 10) + (int)((xi.w >> 2) & 1023u) - (int)((xj.w >> 2) & 1023u)) : 0.0;
+    // include the lobits bits of each coordinate below the record's word (units of Q/1024): every multi-phase run
+    // (for a light phase with its own large c0, config 2b: c_air^2 = 1000 c_w^2, sigma must be good to 1e-11, i.e.
+    // positions to 1e-12 m) and single-phase runs whose pair unit Qp is coarse for their size (DP::subq)
+    const unsigned lm = (1u << p.lobits) - 1u;
+    const double ex = (double)((dx << p.lobits) + (int)((xi.w >> 22) & lm) - (int)((xj.w >> 22) & lm));
+    const double ey = (double)((dy << p.lobits) + (int)((xi.w >> 12) & lm) - (int)((xj.w >> 12) & lm));
+    const double ez = DIM == 3 ? (double)((dz << p.lobits) + (int)((xi.w >> 2) & lm) - (int)((xj.w >> 2) & lm)) : 0.0;
     r2 = fma(ez, ez, fma(ey, ey, ex * ex));
-    r0 = (double)(g.r * 1024.0f);
-    hy = (double)(g.rinv * (0.5f / 1024.0f));
+    r0 = (double)(g.r * p.sub_scale);
+    hy = (double)(g.rinv * p.sub_half_inv);
   } else {
     r2 = (double)(dx * dx + dy * dy + dz * dz);
     r0 = (double)g.r;

@@ -29,8 +29,8 @@ k_probe_pressure(const DP p, const int nf, const int m, const float* __restrict_
       const int s = lbF[rb + max(cx - RC, 0)], e = lbF[rb + min(cx + RC, p.nx - 1) + 1];
       for (int j = s + lane; j < e; j += 32) {
         const XB r = R[j];
-        const double ddx = fx_to_double(r.x.x, p.O[0], p.Q) - x, ddy = fx_to_double(r.x.y, p.O[1], p.Q) - y;
-        const double ddz = p.dim == 3 ? fx_to_double(r.x.z, p.O[2], p.Q) - z : 0.0;
+        const double ddx = fx_pos(p, r.x, 0) - x, ddy = fx_pos(p, r.x, 1) - y;
+        const double ddz = p.dim == 3 ? fx_pos(p, r.x, 2) - z : 0.0;
         const double q = sqrt(ddx * ddx + ddy * ddy + ddz * ddz) * ih;
         if (q < 2.0) {
           const double t = 1.0 - 0.5 * q, t2 = t * t;
@@ -66,9 +66,9 @@ k_probe_gauge(const DP p, const int nf, const int m, const float* __restrict__ x
   for (int j = threadIdx.x; j < nf; j += 256) {
     const XB r = R[j];
     if (phase_of(r.x) != 0) continue;
-    const double px = fx_to_double(r.x.x, p.O[0], p.Q), py = fx_to_double(r.x.y, p.O[1], p.Q);
+    const double px = fx_pos(p, r.x, 0), py = fx_pos(p, r.x, 1);
     const double ddx = px - x, ddy = p.dim == 3 ? py - y : 0.0;
-    if (ddx * ddx + ddy * ddy < h2) best = fmax(best, up == 2 ? fx_to_double(r.x.z, p.O[2], p.Q) : py);
+    if (ddx * ddx + ddy * ddy < h2) best = fmax(best, up == 2 ? fx_pos(p, r.x, 2) : py);
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) best = fmax(best, __shfl_xor_sync(FULL, best, o));
