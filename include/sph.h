@@ -18,11 +18,15 @@
  *    SPH_TAG_WALL for wall dummy particles.  Results come back in the same
  *    order; the internal cell-sorted order is visible only through sph_debug_*.
  *  - Pair arithmetic is float32 on the device ("fully developed on single precision");
- *    density is held as the deviation rho - rho0 of the particle's phase, positions as 32-bit fixed
- *    point (quantum Q = 2^-k m, about 1 nm for metre-sized domains) so that |x_in - x_held| <= Q/2 and
- *    sph_get_fields returns the float32 rounding of the held position; the number density sigma_i
- *    is summed in float64 (DESIGN.md §4 says why).
+ *    density is held as the deviation rho - rho0 of the particle's phase, positions as 42-bit fixed
+ *    point (units of Q/1024, Q = 2^-k m about 1 nm for metre-sized domains; the pair kernels read it modulo
+ *    2^32 units of Q / 2^m) so that float32 inputs are held exactly and sph_get_fields returns the float32
+ *    rounding of the held position; the number density sigma_i is summed in float64 (DESIGN.md §4 says why).
  *  - There is no CPU fallback: every call fails with SPH_ECUDA if no CUDA device is usable.
+ *  - No global state.  sph_create reads six environment variables that exist only so that the experiments of
+ *    profiles/r02_README.md can be repeated from the committed build (SPH_SKIN: largest skin; SPH_SUB_BITS: sub-cell
+ *    Morton bits in the sort key; SPH_REACH=2: cell edge h with a 125-cell walk; SPH_MBITS: cap on m above;
+ *    SPH_FORCE_SUBQ / SPH_NO_SUBQ: the low position bits in sigma on / off).  None is needed for normal use.
  */
 #ifndef SPH_H_
 #define SPH_H_
