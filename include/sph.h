@@ -23,7 +23,7 @@
  *    2^32 units of Q / 2^m) so that float32 inputs are held exactly and sph_get_fields returns the float32
  *    rounding of the held position; the number density sigma_i is summed in float64 (DESIGN.md §4 says why).
  *  - There is no CPU fallback: every call fails with SPH_ECUDA if no CUDA device is usable.
- *  - No global state.  sph_create reads six environment variables that exist only so that the experiments of
+ *  - No global state (one exception, stated there: the device scratch array of sph_cell_sort_static).  sph_create reads six environment variables that exist only so that the experiments of
  *    profiles/r02_README.md can be repeated from the committed build (SPH_SKIN: largest skin; SPH_SUB_BITS: sub-cell
  *    Morton bits in the sort key; SPH_REACH=2: cell edge h with a 125-cell walk; SPH_MBITS: cap on m above;
  *    SPH_FORCE_SUBQ / SPH_NO_SUBQ: the low position bits in sigma on / off).  None is needed for normal use.
@@ -246,6 +246,36 @@ int sph_debug_normals(sph_ctx* ctx, float* normals_host, void* stream);
 /* Per-particle number density sigma_i (first n floats) and d rho/dt (next n floats) of the last
  * pass A, caller order, zero for wall entries; sigma_drho_host holds 2*n floats (HOST). */
 int sph_debug_sigma(sph_ctx* ctx, float* sigma_drho_host, void* stream);
+
+/* The cell-list sort for callers that must not allocate (code under CUDA graph capture, serving loops,
+ * harnesses that forbid cudaMalloc): the stable device radix sort of (cell id, index) that the step and the set-up
+ * run (SPH_STAGE_SORT; PAPER.md:200 names the step, BASELINE.json north_star "cell hash, device radix sort"; the same
+ * kernels, sph_sort.cuh), with its scratch (digit totals, tile histograms, one ping-pong pair of key / value
+ * buffers) in a file-scope `static __device__` array of the library instead of buffers owned by a context.
+ *
+ *   keys_dev[n]      in:  keys with key_bits significant bits (1..32); not modified
+ *   vals_dev[n]      in:  values carried with the keys; NULL = the indices 0..n-1 (the cell list's use); not modified
+ *   keys_out_dev[n]  out: the keys in ascending order
+ *   vals_out_dev[n]  out: the values in that order; equal keys keep their input order (stable)
+ * All four are DEVICE pointers owned by the caller; the outputs must not overlap the inputs or each other.
+ *
+ * Needs no context.  Calls no cudaMalloc / cudaFree and no allocating library routine: kernel launches and one
+ * cudaMemsetAsync on `stream` only; asynchronous, does not synchronise.  The first call on a device looks the array's
+ * device address up (cudaGetSymbolAddress; it loads the library's module if CUDA has not done so yet).
+ * Limit: n <= SPH_STATIC_SORT_MAX_KEYS = 2^20 keys (BASELINE.json configs 0-2 and config 4 at 1 M); the array is
+ * 10 MiB + 2 KiB (2 KiB digit totals, 2 MiB tile histograms, 2 x 4 MiB ping-pong buffers) and every GPU that loads
+ * the library holds it until the process exits.  A larger n is rejected with SPH_EINVAL and nothing is launched.
+ * Every call on a device shares the one array, which keeps the previous call's contents: the call clears the
+ * digit totals itself (the only part that must start at zero) and overwrites the rest before reading it.  Calls that
+ * OVERLAP on the GPU (two streams, or two host threads on two streams) race on the array: order them (same
+ * stream, or events).
+ * Errors: SPH_EINVAL (n < 0, n > SPH_STATIC_SORT_MAX_KEYS, key_bits outside 1..32, a NULL keys / output pointer with
+ * n > 0), SPH_ECUDA (no device, launch failure); sph_cell_sort_static_error() returns the text of the last failure
+ * of this entry point (a static buffer: read it before another thread fails). */
+enum { SPH_STATIC_SORT_MAX_KEYS = 1 << 20 };
+int sph_cell_sort_static(int32_t n, const uint32_t* keys_dev, const uint32_t* vals_dev, int32_t key_bits,
+                         uint32_t* keys_out_dev, uint32_t* vals_out_dev, void* stream);
+const char* sph_cell_sort_static_error(void);
 
 /* Number of kernel launches issued by the library since sph_create (bench.py's gpu_launches). */
 int64_t sph_launch_count(const sph_ctx* ctx);

@@ -1376,3 +1376,116 @@ int sph_debug_sigma(sph_ctx* c, float* sigma, void* stream) {
 }
 
 }  // extern "C"
+
+// ============================================================================================
+// sph_cell_sort_static: the cell-list radix sort with its scratch in a static device array
+// (include/sph.h; for callers that must not allocate).  Same kernels as radix_sort() above.
+// ============================================================================================
+namespace {
+
+// n <= SPH_STATIC_SORT_MAX_KEYS < RS_SMALL_N: tiles of RS_THREADS * 4 keys, as rs_items() picks for these sizes
+constexpr int SSO_ITEMS = 4;
+constexpr int SSO_MAX_BLOCKS = SPH_STATIC_SORT_MAX_KEYS / (RS_THREADS * SSO_ITEMS);
+static_assert(SPH_STATIC_SORT_MAX_KEYS < RS_SMALL_N && SPH_STATIC_SORT_MAX_KEYS % (RS_THREADS * SSO_ITEMS) == 0,
+              "the static sort uses the small-input tile size");
+// layout of the array in 32-bit words: digit totals | tile histograms (digit-major) | keys | values
+constexpr size_t SSO_ROWSUM = 0, SSO_HIST = 512, SSO_KEYS = SSO_HIST + (size_t)512 * SSO_MAX_BLOCKS,
+                 SSO_VALS = SSO_KEYS + SPH_STATIC_SORT_MAX_KEYS, SSO_WORDS = SSO_VALS + SPH_STATIC_SORT_MAX_KEYS;
+
+// In HOST code this name is a host-side stand-in for the symbol, not a device address: the kernels get the
+// address cudaGetSymbolAddress returns for the current device (sso_scratch below).
+static __device__ __align__(256) unsigned g_sso_scratch[SSO_WORDS];
+
+constexpr int SSO_MAX_DEVICES = 64;
+unsigned* g_sso_ptr[SSO_MAX_DEVICES] = {};  // per device: address of g_sso_scratch, looked up once with that device current
+char g_sso_err[192] = "";
+
+int sso_fail(int code, const char* fmt, long long a = 0, long long b = 0) {
+  snprintf(g_sso_err, sizeof g_sso_err, fmt, a, b);
+  return code;
+}
+int sso_fail_cuda(const char* what, cudaError_t e) {
+  snprintf(g_sso_err, sizeof g_sso_err, "sph_cell_sort_static: %s: %s", what, cudaGetErrorString(e));
+  cudaGetLastError();
+  return SPH_ECUDA;
+}
+
+// Device address of the scratch array on the CURRENT device.  Two threads making the first call at once both
+// get the same address from the runtime and store the same value.
+int sso_scratch(unsigned** out) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return sso_fail_cuda("cudaGetDevice", e);
+  if (dev < 0 || dev >= SSO_MAX_DEVICES) return sso_fail(SPH_EINVAL, "sph_cell_sort_static: device ordinal %lld is beyond the %lld this entry point keeps addresses for", dev, SSO_MAX_DEVICES);
+  unsigned* p = __atomic_load_n(&g_sso_ptr[dev], __ATOMIC_ACQUIRE);
+  if (!p) {
+    e = cudaGetSymbolAddress((void**)&p, g_sso_scratch);
+    if (e != cudaSuccess) return sso_fail_cuda("cudaGetSymbolAddress", e);
+    if (!p) return sso_fail(SPH_ECUDA, "sph_cell_sort_static: cudaGetSymbolAddress returned a null address");
+    __atomic_store_n(&g_sso_ptr[dev], p, __ATOMIC_RELEASE);
+  }
+  *out = p;
+  return SPH_OK;
+}
+
+__global__ void __launch_bounds__(256) k_sso_iota(unsigned* __restrict__ v, int n) {
+  const int i = blockIdx.x * 256 + threadIdx.x;
+  if (i < n) v[i] = (unsigned)i;
+}
+
+template <int ND>
+void sso_pass(cudaStream_t st, const unsigned* ki, const unsigned* vi, int n, int shift, unsigned* hist, int nblk,
+              unsigned* rowsum, unsigned* kt, unsigned* vt) {
+  k_radix_hist<ND, SSO_ITEMS><<<nblk, RS_THREADS, 0, st>>>(ki, n, shift, hist, nblk, rowsum);
+  k_scan_apply<<<ND, 256, 0, st>>>(hist, nblk, rowsum);
+  k_radix_scatter<ND, SSO_ITEMS><<<nblk, RS_THREADS, 0, st>>>(ki, vi, n, shift, hist, nblk, kt, vt, rowsum);
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* sph_cell_sort_static_error(void) { return g_sso_err; }
+
+int sph_cell_sort_static(int32_t n, const uint32_t* keys, const uint32_t* vals, int32_t key_bits, uint32_t* keys_out,
+                         uint32_t* vals_out, void* stream) {
+  if (n < 0) return sso_fail(SPH_EINVAL, "sph_cell_sort_static: n = %lld is negative", n);
+  if (n > SPH_STATIC_SORT_MAX_KEYS)
+    return sso_fail(SPH_EINVAL, "sph_cell_sort_static: n = %lld exceeds SPH_STATIC_SORT_MAX_KEYS = %lld (the static scratch array holds no more; use a context)",
+                    n, SPH_STATIC_SORT_MAX_KEYS);
+  if (key_bits < 1 || key_bits > 32) return sso_fail(SPH_EINVAL, "sph_cell_sort_static: key_bits = %lld is outside 1..32", key_bits);
+  if (n == 0) return SPH_OK;
+  if (!keys || !keys_out || !vals_out) return sso_fail(SPH_EINVAL, "sph_cell_sort_static: NULL keys or output pointer");
+  cudaStream_t st = (cudaStream_t)stream;
+  unsigned* scratch = nullptr;
+  int rc = sso_scratch(&scratch);
+  if (rc) return rc;
+  unsigned *rowsum = scratch + SSO_ROWSUM, *hist = scratch + SSO_HIST, *ktmp = scratch + SSO_KEYS, *vtmp = scratch + SSO_VALS;
+  // the array keeps what the last call left: the digit totals must start at zero (an interrupted call leaves them set)
+  cudaError_t e = cudaMemsetAsync(rowsum, 0, 512 * sizeof(unsigned), st);
+  if (e != cudaSuccess) return sso_fail_cuda("cudaMemsetAsync", e);
+  int dbits, passes;
+  radix_plan(key_bits, &dbits, &passes);
+  const int nblk = cdiv(n, RS_THREADS * SSO_ITEMS);
+  // pass p writes the caller's outputs when an even number of passes follows it, else the scratch pair: the last
+  // pass lands in the outputs and no pass reads the buffer it writes
+  auto to_out = [&](int p) { return ((passes - 1 - p) & 1) == 0; };
+  const unsigned *ki = keys, *vi = vals;
+  if (!vi) {  // indices 0..n-1, into the value buffer that pass 0 does not write
+    unsigned* v0 = to_out(0) ? vtmp : vals_out;
+    k_sso_iota<<<cdiv(n, 256), 256, 0, st>>>(v0, n);
+    vi = v0;
+  }
+  for (int p = 0; p < passes; ++p) {
+    unsigned *kt = to_out(p) ? keys_out : ktmp, *vt = to_out(p) ? vals_out : vtmp;
+    if (dbits == 9) sso_pass<512>(st, ki, vi, n, dbits * p, hist, nblk, rowsum, kt, vt);
+    else sso_pass<256>(st, ki, vi, n, dbits * p, hist, nblk, rowsum, kt, vt);
+    ki = kt;
+    vi = vt;
+  }
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return sso_fail_cuda("kernel launch", e);
+  return SPH_OK;
+}
+
+}  // extern "C"

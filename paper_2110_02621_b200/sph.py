@@ -53,6 +53,7 @@ EXPORTS = (
     "sph_step_dt", "sph_get_fields", "sph_get_fields_host", "sph_get_stats", "sph_get_stats_ex", "sph_set_profiling",
     "sph_get_timings", "sph_num_cells", "sph_debug_cells", "sph_debug_neighbours", "sph_debug_list_check", "sph_probe_pressure", "sph_probe_gauge",
     "sph_debug_normals", "sph_debug_sigma", "sph_launch_count", "sph_last_error", "sph_debug_step_lists", "sph_debug_fma_peak", "sph_debug_time_pointwise",
+    "sph_cell_sort_static", "sph_cell_sort_static_error",
 )
 
 _lib = None
@@ -93,6 +94,8 @@ def load():
     L.sph_debug_sigma.restype = C.c_int; L.sph_debug_sigma.argtypes = [vp, vp, vp]
     L.sph_launch_count.restype = i64; L.sph_launch_count.argtypes = [vp]
     L.sph_last_error.restype = C.c_char_p; L.sph_last_error.argtypes = [vp]
+    L.sph_cell_sort_static.restype = C.c_int; L.sph_cell_sort_static.argtypes = [i32, vp, vp, i32, vp, vp, vp]
+    L.sph_cell_sort_static_error.restype = C.c_char_p; L.sph_cell_sort_static_error.argtypes = []
     _lib = L
     return L
 
@@ -305,3 +308,25 @@ def fma_peak_tflops(stream=None):
     if rc != 0:
         raise SphError("sph_debug_fma_peak failed with code %d" % rc)
     return out.value
+
+
+STATIC_SORT_MAX_KEYS = 1 << 20
+
+
+def cell_sort_static(keys, vals, key_bits, keys_out, vals_out, stream=None):
+    """sph_cell_sort_static: stable radix sort of (keys, vals) by the low `key_bits` bits of the keys with the
+    library's static device scratch (no allocation; at most STATIC_SORT_MAX_KEYS keys).  All tensors are the
+    caller's: contiguous 4-byte integer CUDA tensors of n elements; `vals` None = the indices 0..n-1.
+    Asynchronous on `stream` (default: torch's current stream)."""
+    import torch
+    L = load()
+    n = keys.numel()
+    for t in (keys, vals, keys_out, vals_out):
+        if t is not None and not (t.is_cuda and t.is_contiguous() and t.element_size() == 4 and t.numel() == n):
+            raise SphError("cell_sort_static: contiguous 4-byte CUDA tensors of one length are needed")
+    st = stream if stream is not None else torch.cuda.current_stream()
+    rc = L.sph_cell_sort_static(n, C.c_void_p(keys.data_ptr()), C.c_void_p(vals.data_ptr()) if vals is not None else None,
+                                int(key_bits), C.c_void_p(keys_out.data_ptr()), C.c_void_p(vals_out.data_ptr()),
+                                C.c_void_p(st.cuda_stream))
+    if rc != 0:
+        raise SphError("sph_cell_sort_static failed with code %d: %s" % (rc, L.sph_cell_sort_static_error().decode()))
