@@ -332,6 +332,8 @@ def run_gpu(args):
     stage_def = {k: v / max(ns, 1) for k, v in stage_def.items()}
     stage_def["rebuilds_per_step"] = g.last_timing_rebuilds / max(ns, 1)
     st = g.get_stats()
+    # measured roofline of the gather form: the passes' list walk with an empty pair body, on the lists of this state
+    gather = g.gather_floor()
     skin = sph.DEFAULT_LIST_SKIN if cfg.get("list_skin", -1.0) < 0 else cfg["list_skin"]
     if skin > 0:
         g.close()
@@ -364,6 +366,7 @@ def run_gpu(args):
         for _ in range(20):             # keep the loop running long enough for nvidia-smi to sample its clocks
             peak = max(peak, sph.fma_peak_tflops())
     fma_clocks = fma_sampler.stop()
+    l1_patterns = sph.gather_pattern_cycles()
     kern = {}
     # Pair stages.  The 27-cell candidate walk runs once per step in k_build (fluid-fluid) and inside
     # k_wall / the wall part of the passes (fluid-wall); the fluid pair passes read the neighbour lists.
@@ -406,6 +409,16 @@ def run_gpu(args):
                                 "measured: sph_debug_fma_peak (register-resident FMA loop, 8 chains x 2048 threads per SM) on this device in this run"),
                 "peak_derived": peak_derived, "peak_clocks": {"sm_mhz": fma_clocks.get("sm_mhz"), "sm_max_mhz": fma_clocks.get("sm_max_mhz")},
                 "flops_per_hit": FLOPS_HIT[dom], "flops_per_candidate": CAND_FLOPS,
+                # sph_debug_gather_floor: what the memory requests of a pass alone take (same lists, same records, same
+                # launch configuration, empty pair body), and what merged lists / coalesced records / an SM-affine
+                # block order would make of them; sph_debug_gather_patterns: the L1's cost per request by address pattern
+                "gather_floor": {"own_entries_ms": gather["own_entries"], "lane_pair_shared_ms": gather["lane_pair_shared"],
+                                 "quad_shared_ms": gather["quad_shared"], "coalesced_ms": gather["coalesced"],
+                                 "own_entries_sm_affine_ms": gather["own_entries_sm_affine"], "requests": gather["requests"],
+                                 "cycles_per_request": gather["own_entries"] * 1e-3 * sm_max * 1e6 * N_SM / max(gather["requests"], 1),
+                                 "pass_a_over_floor": stage_def["pass_a"] / gather["own_entries"] if gather["own_entries"] > 0 else None,
+                                 "pass_b_over_floor": stage_def["pass_b"] / gather["own_entries"] if gather["own_entries"] > 0 else None,
+                                 "l1_cycles_per_request_by_pattern": l1_patterns},
                 # list build + pass A + pass B together (the candidate walk is k_build's):
                 "pair_stages": pair_stages}
     g.close()

@@ -240,6 +240,34 @@ int sph_debug_time_pointwise(sph_ctx* ctx, float* ms_host, void* stream);
  * TFLOP/s (fma = 2 flop).  SURVEY.md section 8(d) "Peaks"; bench.py's roofline denominator.  Needs no context. */
 int sph_debug_fma_peak(double* tflops_host, void* stream);
 
+/* Measured roofline of the gather form: the list walk of the pair passes ("one thread per particle"
+ * reading its neighbours from global memory; DESIGN.md section 5 "list walk": one coalesced 16-byte list load, four
+ * 256-bit record gathers per lane) over the context's CURRENT fluid-fluid neighbour lists and records, with an empty
+ * pair body, in the passes' launch configuration.  State and lists are read, never written.
+ *   ms_host[0]  every lane gathers its own list entries: exactly the memory requests of pass A / pass B;
+ *   ms_host[1]  both lanes of a lane pair gather the even lane's entry (a list merged per lane pair);
+ *   ms_host[2]  the four lanes of a quad gather the first lane's entry (a list merged per quad);
+ *   ms_host[3]  32 consecutive records per request (the coalesced optimum: 1 KiB from 8 cache lines);
+ *   ms_host[4]  as [0], but the chunks (128 consecutive particles, one block's work) are taken in an SM-affine order:
+ *               sorted by blobs of cells, every SM works through a contiguous part of that order with persistent
+ *               blocks (what the plain block order costs in L1 misses; 0 if the blob key does not fit 32 bits);
+ *   each the best of 3 launches after one warm-up launch, in ms.  Modes 1-3 run every lane to the warp's largest count.
+ *   *requests_host (may be NULL) = warp-wide gather requests of one walk (sum over warps of the largest count).
+ * HOST pointers (5 floats, one int64); synchronises; allocates and frees its own scratch.
+ * Errors: SPH_EINVAL without particles, SPH_ENOMEM, SPH_ECUDA. */
+int sph_debug_gather_floor(sph_ctx* ctx, float* ms_host, int64_t* requests_host, void* stream);
+
+/* What a warp-wide gather of 32-byte records (one 256-bit load per lane, the pair passes' request) costs in the L1 of
+ * the current device as a function of the address pattern, records resident in L1; SM cycles (at the device's maximum
+ * clock) per request, best of 3 launches:
+ *   cycles_host[0]  32 random records of a 16 KiB window          [4]  8 records, each read by 4 adjacent lanes
+ *   cycles_host[1]  32 consecutive records (8 cache lines)        [5]  one record for all 32 lanes
+ *   cycles_host[2]  16 random lines, adjacent lane pairs share one [6]  32 different lines, one record of each
+ *   cycles_host[3]  8 random lines, each read by 4 adjacent lanes
+ * The L1 model of DESIGN.md section 7 rests on this table.  HOST pointer to 7 doubles; needs no context; synchronises.
+ * Errors: SPH_EINVAL, SPH_ENOMEM, SPH_ECUDA. */
+int sph_debug_gather_patterns(double* cycles_host, void* stream);
+
 /* Wall normals Eq. 2.16 in caller order (n*3, zero for fluid entries); HOST pointer. */
 int sph_debug_normals(sph_ctx* ctx, float* normals_host, void* stream);
 

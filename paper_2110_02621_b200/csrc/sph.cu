@@ -1339,6 +1339,117 @@ int sph_debug_fma_peak(double* tflops_host, void* stream) {
   return SPH_OK;
 }
 
+int sph_debug_gather_floor(sph_ctx* c, float* ms, int64_t* requests, void* stream) {
+  if (!c || !ms) return SPH_EINVAL;
+  if (!c->loaded) { c->err = "no particles"; return SPH_EINVAL; }
+  cudaStream_t st = (cudaStream_t)stream;
+  for (int m = 0; m < 5; ++m) ms[m] = 0.f;
+  if (requests) *requests = 0;
+  const int nf = (int)c->nf;
+  if (!nf) return SPH_OK;
+  const int M = cdiv(nf, PB);
+  int dev = 0, nsm = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || nsm < 1)
+    return SPH_ECUDA;
+  const int nq = std::min(nsm, 1000);
+  // scratch: [0] request count, [1] the kernels' never-written output word, then the queue counters of mode 4;
+  // chunk keys / values of mode 4 (two ping-pong pairs)
+  unsigned long long* d = nullptr;
+  unsigned *q = nullptr, *ck = nullptr;
+  CK(cudaMalloc((void**)&d, 16));
+  CK(cudaMalloc((void**)&q, 4 * (size_t)nq));
+  CK(cudaMalloc((void**)&ck, 16 * (size_t)M));
+  CK(cudaMemsetAsync(d, 0, 16, st));
+  LAUNCH(k_gather_requests, cdiv(nf, 256), 256, st, nf, c->NC, d);
+  // mode 4: blobs of one chunk length along x by 4 x 4 cell rows (best of 1 x 1 ... 16 x 16, profiles/r02_README.md)
+  const double edge_dp = 1.0 / ((double)c->dp.inv_edge * c->prm.dp);
+  const int L = std::max(1, std::min(63, (int)lrint((double)PB / (c->prm.dim == 3 ? edge_dp * edge_dp * edge_dp : edge_dp * edge_dp))));
+  const int ry = std::min(4, c->dp.ny), rz = std::min(4, c->dp.nz);
+  const int cobits = bits_for((int64_t)cdiv(c->dp.nx, L) * cdiv(c->dp.ny, ry) * cdiv(c->dp.nz, rz)) + 10;
+  unsigned *ko = nullptr, *vo = nullptr;
+  int rc = SPH_OK;
+  if (cobits <= 32) {
+    LAUNCH(k_chunk_keys, cdiv(M, 256), 256, st, c->dp, nf, c->K, M, L, ry, rz, ck, ck + M);
+    rc = radix_sort(c, st, M, cobits, ck, ck + M, ck + 2 * (size_t)M, ck + 3 * (size_t)M, &ko, &vo);
+  }
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  const int grid = cdiv(nf, PB);
+  // R1 = the records pass B gathers (the state after pass A); the lists are the ones the passes read
+  for (int mode = 0; mode < 5 && rc == SPH_OK; ++mode) {
+    if (mode == 4 && !vo) break;
+    float best = 0.f;
+    for (int rep = 0; rep < 4; ++rep) {   // one warm-up launch, best of three
+      if (mode == 4) cudaMemsetAsync(q, 0, 4 * (size_t)nq, st);
+      cudaEventRecord(e0, st);
+      switch (mode) {
+        case 0: LAUNCH(k_gather_walk<0>, grid, PB, st, nf, c->R1, c->NL, c->NC, c->caps, (unsigned*)(d + 1)); break;
+        case 1: LAUNCH(k_gather_walk<1>, grid, PB, st, nf, c->R1, c->NL, c->NC, c->caps, (unsigned*)(d + 1)); break;
+        case 2: LAUNCH(k_gather_walk<2>, grid, PB, st, nf, c->R1, c->NL, c->NC, c->caps, (unsigned*)(d + 1)); break;
+        case 3: LAUNCH(k_gather_walk<3>, grid, PB, st, nf, c->R1, c->NL, c->NC, c->caps, (unsigned*)(d + 1)); break;
+        default: LAUNCH(k_gather_walk_affine, std::min(M, nq * SPH_MINB), PB, st, nf, c->R1, c->NL, c->NC, c->caps, (unsigned*)(d + 1), vo, M, q, nq); break;
+      }
+      cudaEventRecord(e1, st);
+      cudaError_t e = cudaEventSynchronize(e1);
+      if (e != cudaSuccess) { c->err = cudaGetErrorString(e); rc = SPH_ECUDA; break; }
+      float t = 0.f;
+      cudaEventElapsedTime(&t, e0, e1);
+      if (rep && (best == 0.f || t < best)) best = t;
+    }
+    ms[mode] = best;
+  }
+  unsigned long long h = 0;
+  if (rc == SPH_OK && cudaMemcpy(&h, d, 8, cudaMemcpyDeviceToHost) != cudaSuccess) { c->err = "request count read-back"; rc = SPH_ECUDA; }
+  if (requests) *requests = (int64_t)h;
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  cudaFree(d); cudaFree(q); cudaFree(ck);
+  return rc;
+}
+
+int sph_debug_gather_patterns(double* cycles, void* stream) {
+  if (!cycles) return SPH_EINVAL;
+  for (int k = 0; k < 7; ++k) cycles[k] = 0.0;
+  cudaStream_t st = (cudaStream_t)stream;
+  int dev = 0, nsm = 0, khz = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+      cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, dev) != cudaSuccess)
+    return SPH_ECUDA;
+  const int blocks = nsm * SPH_MINB, iters = 1024;
+  XB* R = nullptr;
+  if (cudaMalloc((void**)&R, (size_t)blocks * 512 * sizeof(XB) + 16) != cudaSuccess) return SPH_ENOMEM;
+  cudaMemsetAsync(R, 1, (size_t)blocks * 512 * sizeof(XB) + 16, st);
+  unsigned* out = reinterpret_cast<unsigned*>(R + (size_t)blocks * 512);
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  int rc = SPH_OK;
+  for (int pat = 0; pat < 7 && rc == SPH_OK; ++pat) {
+    float best = 0.f;
+    for (int rep = 0; rep < 4; ++rep) {   // one warm-up launch, best of three
+      cudaEventRecord(e0, st);
+      switch (pat) {
+        case 0: k_gather_patterns<0><<<blocks, PB, 0, st>>>(R, iters, out); break;
+        case 1: k_gather_patterns<1><<<blocks, PB, 0, st>>>(R, iters, out); break;
+        case 2: k_gather_patterns<2><<<blocks, PB, 0, st>>>(R, iters, out); break;
+        case 3: k_gather_patterns<3><<<blocks, PB, 0, st>>>(R, iters, out); break;
+        case 4: k_gather_patterns<4><<<blocks, PB, 0, st>>>(R, iters, out); break;
+        case 5: k_gather_patterns<5><<<blocks, PB, 0, st>>>(R, iters, out); break;
+        default: k_gather_patterns<6><<<blocks, PB, 0, st>>>(R, iters, out); break;
+      }
+      cudaEventRecord(e1, st);
+      if (cudaEventSynchronize(e1) != cudaSuccess) { rc = SPH_ECUDA; break; }
+      float t = 0.f;
+      cudaEventElapsedTime(&t, e0, e1);
+      if (rep && (best == 0.f || t < best)) best = t;
+    }
+    // SM cycles at the device's maximum clock per warp-wide gather request (SPH_MINB blocks x PB / 32 warps per SM)
+    const double requests_per_sm = (double)SPH_MINB * (PB / 32) * iters * 4.0;
+    cycles[pat] = best * 1e-3 * (double)khz * 1e3 / requests_per_sm;
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  cudaFree(R);
+  return rc;
+}
+
 int sph_debug_normals(sph_ctx* c, float* normals, void* stream) {
   if (!c || !normals) return SPH_EINVAL;
   if (!c->loaded) { c->err = "no particles"; return SPH_EINVAL; }

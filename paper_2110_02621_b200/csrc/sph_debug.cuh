@@ -326,3 +326,151 @@ k_fma_peak(float* __restrict__ out, int iters, float a, float b) {
   const float s = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
   if (s == 12345.678f) out[0] = s;  // keeps the chains alive without a store in the common case
 }
+
+// sph_debug_gather_floor: the list walk of the pair passes (walk_l: one coalesced 16-byte list load, four 256-bit record
+// gathers) with an empty pair body (every word of the record enters one XOR / ADD, nothing else), in the passes'
+// launch configuration: what the passes' memory requests alone cost on this device, i.e. the roofline of the gather
+// form.  MODE selects which record each lane asks for:
+//   0  its own list entry (exactly the passes' requests),
+//   1  the entry of the even lane of its lane pair   (what a list merged per lane pair would request),
+//   2  the entry of the first lane of its quad       (a list merged per quad: 4 adjacent lanes, one record),
+//   3  32 consecutive records from lane 0's entry on (the coalesced optimum: 8 lines, 1 KiB per request).
+template <int MODE>
+struct GatherBody {
+  const XB* __restrict__ R;
+  unsigned last, acc;
+  int lane;
+  __device__ __forceinline__ XB load(unsigned j) const {
+    if (MODE == 1) j = __shfl_sync(FULL, j, lane & ~1);
+    if (MODE == 2) j = __shfl_sync(FULL, j, lane & ~3);
+    if (MODE == 3) j = (__shfl_sync(FULL, j, 0) & ~31u) + (unsigned)lane;
+    return ldg256(R + min(j, last));  // MODE > 0 also reads the slots behind a lane's own count: clamped
+  }
+  __device__ __forceinline__ void apply(const XB& r) {
+    acc += (r.x.x ^ r.x.y) + (r.x.z ^ r.x.w) + (__float_as_uint(r.b.x) ^ __float_as_uint(r.b.y)) +
+           (__float_as_uint(r.b.z) ^ __float_as_uint(r.b.w));
+  }
+};
+template <int MODE>
+__global__ void __launch_bounds__(PB, SPH_MINB)
+k_gather_walk(const int nf, const XB* __restrict__ R, const uint4* __restrict__ NL, const int* __restrict__ NC,
+              const int caps, unsigned* __restrict__ out) {
+  const int i0 = blockIdx.x * PB + threadIdx.x;
+  const int lane = threadIdx.x & 31;
+  GatherBody<MODE> body{R, (unsigned)(nf - 1), 0u, lane};
+  // MODE > 0 shuffles inside the loop, so every lane runs to the warp's largest count (32 active lanes, not ~30)
+  const int cnt = i0 < nf ? NC[i0] : 0;
+  walk_l(NL + (size_t)(i0 >> 5) * (caps >> 2) * 32 + lane, MODE ? __reduce_max_sync(FULL, cnt) : cnt, body);
+  if (body.acc == 0x9e3779b9u) out[0] = body.acc;  // keeps the gathers alive without a store in the common case
+}
+// warp-wide gather requests of one list walk: sum over the warps of the largest count in the warp
+__global__ void k_gather_requests(const int nf, const int* __restrict__ NC, unsigned long long* __restrict__ tot) {
+  const int i0 = blockIdx.x * 256 + threadIdx.x;
+  const int m = __reduce_max_sync(FULL, i0 < nf ? NC[i0] : 0);
+  if ((threadIdx.x & 31) == 0 && m) atomicAdd(tot, (unsigned long long)m);
+}
+
+// Mode 4 of sph_debug_gather_floor: the same walk (mode 0) with the chunks (PB consecutive particles = one block's
+// work) taken in an SM-AFFINE order: chunks are sorted by the blob of cells their first particle lies in (L cells along
+// x by ry x rz cell rows), every SM owns a contiguous part of that order, and persistent blocks pop consecutive chunks
+// from the counter of the SM they run on (%smid), so that the blocks sharing an L1 walk one neighbourhood together.
+// Measures how much of the walk's time is L1 misses caused by the plain chunk = blockIdx.x mapping.
+__global__ void k_chunk_keys(const DP p, const int nf, const unsigned* __restrict__ K, const int M, const int L,
+                             const int ry, const int rz, unsigned* __restrict__ key, unsigned* __restrict__ val) {
+  const int c = blockIdx.x * 256 + threadIdx.x;
+  if (c >= M) return;
+  int cx, cy, cz;
+  cell_of_key(p, K[min(c * PB, nf - 1)] >> p.sub_bits, cx, cy, cz);
+  const int nbx = (p.nx + L - 1) / L, nby = (p.ny + ry - 1) / ry;
+  const int bx = cx / L, by = cy / ry, bz = cz / rz;
+  key[c] = ((unsigned)((bz * nby + by) * nbx + bx) << 10) | ((unsigned)(cz - bz * rz) << 8) | ((unsigned)(cy - by * ry) << 6) |
+           (unsigned)min(cx - bx * L, 63);
+  val[c] = (unsigned)c;
+}
+__global__ void __launch_bounds__(PB, SPH_MINB)
+k_gather_walk_affine(const int nf, const XB* __restrict__ R, const uint4* __restrict__ NL, const int* __restrict__ NC,
+                     const int caps, unsigned* __restrict__ out, const unsigned* __restrict__ CO, const int M,
+                     unsigned* __restrict__ q, const int nq) {
+  __shared__ int chunk_s;
+  unsigned smid;
+  asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+  const int own = (int)(smid % (unsigned)nq), per = (M + nq - 1) / nq;
+  const int lane = threadIdx.x & 31;
+  GatherBody<0> body{R, (unsigned)(nf - 1), 0u, lane};
+  int cur = own;
+#pragma unroll 1
+  for (;;) {
+    if (threadIdx.x < 32) {
+      int ch = -1;
+      for (;;) {
+        int k = 0;
+        if (lane == 0) k = (int)atomicAdd(q + cur, 1u);
+        k = __shfl_sync(FULL, k, 0);
+        const int pos = cur * per + k;
+        if (k < per && pos < M) { ch = (int)CO[pos]; break; }
+        // this queue is empty: the first one behind this SM's own that still holds chunks (32 queues per look)
+        int found = -1;
+        for (int t = 0; t < nq && found < 0; t += 32) {
+          const int o = t + lane;
+          int s = own + 1 + o;
+          if (s >= nq) s -= nq;
+          bool has = false;
+          if (o < nq) has = (int)*(volatile unsigned*)(q + s) < min(per, M - s * per);
+          const unsigned b = __ballot_sync(FULL, has);
+          if (b) found = __shfl_sync(FULL, s, __ffs(b) - 1);
+        }
+        if (found < 0) break;
+        cur = found;
+      }
+      if (lane == 0) chunk_s = ch;
+    }
+    __syncthreads();
+    const int chunk = chunk_s;
+    __syncthreads();
+    if (chunk < 0) break;
+    const int i0 = chunk * PB + threadIdx.x;
+    walk_l(NL + (size_t)(i0 >> 5) * (caps >> 2) * 32 + lane, i0 < nf ? NC[i0] : 0, body);
+  }
+  if (body.acc == 0x9e3779b9u) out[0] = body.acc;
+}
+
+// sph_debug_gather_patterns: what a warp-wide gather of 32-byte records (one LDG.E.ENL2.256 per lane) costs in the L1
+// as a function of the address pattern, records resident in L1 (a window of 512 records = 16 KiB per block, 8 blocks
+// per SM).  PAT: 0 32 random records; 1 32 consecutive records (8 lines); 2 16 random lines, adjacent lane pairs in
+// one line; 3 8 random lines, each read by 4 adjacent lanes (4 records); 4 8 records, each read by 4 adjacent lanes;
+// 5 one record for all lanes; 6 32 different lines, one record of each.  Addresses come from an integer hash of
+// (block, warp, iteration, lane group), a handful of ALU instructions per request.
+__device__ __forceinline__ unsigned mix32(unsigned x) {
+  x ^= x >> 16; x *= 0x7feb352du; x ^= x >> 15; x *= 0x846ca68bu; x ^= x >> 16;
+  return x;
+}
+template <int PAT>
+__global__ void __launch_bounds__(PB, SPH_MINB)
+k_gather_patterns(const XB* __restrict__ R, const int iters, unsigned* __restrict__ out) {
+  constexpr unsigned W = 512, NL = W / 4;
+  const XB* base = R + (size_t)blockIdx.x * W;
+  const unsigned lane = threadIdx.x & 31, seed = (blockIdx.x * 4u + (threadIdx.x >> 5)) * 0x9e3779b9u;
+  unsigned acc = 0;
+#pragma unroll 1
+  for (int it = 0; it < iters; ++it) {
+    XB r[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const unsigned q = seed + (unsigned)(it * 4 + u) * 0x85ebca6bu;
+      unsigned idx;
+      if (PAT == 0) idx = mix32(q + lane) % W;
+      else if (PAT == 1) idx = ((mix32(q) % (NL - 8)) << 2) + lane;
+      else if (PAT == 2) { const unsigned h = mix32(q + (lane >> 1)); idx = ((h % NL) << 2) + ((h >> 20) & 2u) + (lane & 1u); }
+      else if (PAT == 3) idx = ((mix32(q + (lane >> 2)) % NL) << 2) + (lane & 3u);
+      else if (PAT == 4) idx = ((mix32(q + (lane >> 2)) % NL) << 2) + 1u;
+      else if (PAT == 5) idx = mix32(q) % W;
+      else idx = (((mix32(q) + lane) % NL) << 2) + (mix32(q + lane) & 3u);
+      r[u] = ldg256(base + idx);
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+      acc += (r[u].x.x ^ r[u].x.y) + (r[u].x.z ^ r[u].x.w) + (__float_as_uint(r[u].b.x) ^ __float_as_uint(r[u].b.y)) +
+             (__float_as_uint(r[u].b.z) ^ __float_as_uint(r[u].b.w));
+  }
+  if (acc == 0x9e3779b9u) out[0] = acc;
+}

@@ -52,7 +52,7 @@ EXPORTS = (
     "sph_create", "sph_destroy", "sph_set_particles", "sph_set_particles_host", "sph_step",
     "sph_step_dt", "sph_get_fields", "sph_get_fields_host", "sph_get_stats", "sph_get_stats_ex", "sph_set_profiling",
     "sph_get_timings", "sph_num_cells", "sph_debug_cells", "sph_debug_neighbours", "sph_debug_list_check", "sph_probe_pressure", "sph_probe_gauge",
-    "sph_debug_normals", "sph_debug_sigma", "sph_launch_count", "sph_last_error", "sph_debug_step_lists", "sph_debug_fma_peak", "sph_debug_time_pointwise",
+    "sph_debug_normals", "sph_debug_sigma", "sph_launch_count", "sph_last_error", "sph_debug_step_lists", "sph_debug_fma_peak", "sph_debug_time_pointwise", "sph_debug_gather_floor", "sph_debug_gather_patterns",
     "sph_cell_sort_static", "sph_cell_sort_static_error",
 )
 
@@ -87,6 +87,8 @@ def load():
     L.sph_debug_step_lists.restype = C.c_int; L.sph_debug_step_lists.argtypes = [vp, vp, vp, i64, vp, vp]
     L.sph_debug_time_pointwise.restype = C.c_int; L.sph_debug_time_pointwise.argtypes = [vp, vp, vp]
     L.sph_debug_fma_peak.restype = C.c_int; L.sph_debug_fma_peak.argtypes = [vp, vp]
+    L.sph_debug_gather_floor.restype = C.c_int; L.sph_debug_gather_floor.argtypes = [vp, vp, vp, vp]
+    L.sph_debug_gather_patterns.restype = C.c_int; L.sph_debug_gather_patterns.argtypes = [vp, vp]
     L.sph_debug_normals.restype = C.c_int; L.sph_debug_normals.argtypes = [vp, vp, vp]
     L.sph_debug_list_check.restype = C.c_int; L.sph_debug_list_check.argtypes = [vp, vp, vp]
     L.sph_probe_pressure.restype = C.c_int; L.sph_probe_pressure.argtypes = [vp, C.c_int32, vp, vp, vp, vp]
@@ -236,6 +238,15 @@ class Sph:
         self._ck(self.L.sph_debug_time_pointwise(self.ctx, _hp(ms), self._st()))
         return dict(reinit=float(ms[0]), integrator=float(ms[1]), fused_predict=float(ms[2]))
 
+    def gather_floor(self):
+        """sph_debug_gather_floor: the passes' list walk with an empty pair body on the current lists (ms per launch)
+        and the number of warp-wide gather requests of one walk."""
+        ms = np.zeros(5, np.float32)
+        req = C.c_int64(0)
+        self._ck(self.L.sph_debug_gather_floor(self.ctx, _hp(ms), C.byref(req), self._st()))
+        return dict(own_entries=float(ms[0]), lane_pair_shared=float(ms[1]), quad_shared=float(ms[2]),
+                    coalesced=float(ms[3]), own_entries_sm_affine=float(ms[4]), requests=req.value)
+
     def launch_count(self):
         return self.L.sph_launch_count(self.ctx)
 
@@ -308,6 +319,22 @@ def fma_peak_tflops(stream=None):
     if rc != 0:
         raise SphError("sph_debug_fma_peak failed with code %d" % rc)
     return out.value
+
+
+GATHER_PATTERNS = ("random_32_records", "consecutive_32_records", "16_lines_lane_pairs", "8_lines_quads_4_records",
+                   "8_records_quads", "one_record", "32_lines")
+
+
+def gather_pattern_cycles(stream=None):
+    """sph_debug_gather_patterns: SM cycles per warp-wide 32-byte-record gather for seven address patterns (L1-resident)."""
+    import torch
+    L = load()
+    out = (C.c_double * 7)()
+    st = stream if stream is not None else torch.cuda.current_stream()
+    rc = L.sph_debug_gather_patterns(out, C.c_void_p(st.cuda_stream))
+    if rc != 0:
+        raise SphError("sph_debug_gather_patterns failed with code %d" % rc)
+    return dict(zip(GATHER_PATTERNS, [float(x) for x in out]))
 
 
 STATIC_SORT_MAX_KEYS = 1 << 20

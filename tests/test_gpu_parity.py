@@ -386,6 +386,42 @@ def test_stage_timings_and_launch_count():
     assert g.launch_count() > l0
 
 
+@pytest.mark.parametrize("name", ["box3d_20", "cfg0", "box2d_two_phase"])
+def test_gather_floor_walks_the_lists_and_leaves_the_state_alone(name):
+    """sph_debug_gather_floor (the measured roofline of the gather form): every mode runs, the request
+    count is the sum over the warps of the largest list length (from the lists the passes read), the SM-affine chunk
+    order visits every chunk (a missed chunk would hang or shorten the walk; here: the call returns and mode 4 is
+    timed), and neither the state nor the following steps change (bit for bit against a context that never called it)."""
+    cfg = inputs.box_sweep_3d(n=20) if name == "box3d_20" else SMALL[name]
+    g, h = sph.Sph(cfg), sph.Sph(cfg)
+    for s in (g, h):
+        s.set_particles(cfg["pos"], cfg["vel"], cfg["rho"], cfg["tag"])
+        s.step(3)
+    gf = g.gather_floor()
+    assert all(gf[k] > 0 for k in ("own_entries", "lane_pair_shared", "quad_shared", "coalesced", "own_entries_sm_affine")), gf
+    # fluid rows of the lists the passes read = fluid-fluid entries (+ fluid-wall entries, which the walk does not take)
+    off, ids = g.debug_step_lists()
+    tag = cfg["tag"]
+    nf = int((tag >= 0).sum())
+    assert 0 < gf["requests"] <= int((off[1:] - off[:-1])[tag >= 0].sum())
+    assert gf["requests"] >= (nf + 31) // 32    # every warp has the self entries at least
+    g.step(2); h.step(2)
+    a, b = g.get_fields(device=False), h.get_fields(device=False)
+    for k in ("pos", "vel", "rho", "p", "acc"):
+        assert np.array_equal(a[k], b[k]), k
+
+
+def test_gather_pattern_cycles_are_ordered():
+    """sph_debug_gather_patterns: a warp-wide gather of 32 consecutive 32-byte records cannot cost less than the 8 cycles
+    its 1 KiB takes on the 128-byte-per-cycle L1 data path, 32 random records cost more than 8 lines read by quads, and
+    those not more than 16 lines read by lane pairs (the table DESIGN.md section 7 quotes)."""
+    c = sph.gather_pattern_cycles()
+    assert c["consecutive_32_records"] >= 7.5
+    assert c["one_record"] >= 7.5
+    assert c["random_32_records"] > c["16_lines_lane_pairs"] > c["8_lines_quads_4_records"] >= 0.9 * c["consecutive_32_records"]
+    assert c["32_lines"] > 1.5 * c["consecutive_32_records"]
+
+
 @pytest.mark.parametrize("moving", [False, True])
 def test_graph_replay_equals_direct_launches_bitwise(moving):
     """sph_step replays one captured step as a CUDA graph; SPH_FLAG_NO_GRAPH issues the same
