@@ -263,8 +263,8 @@ int sph_debug_gather_floor(sph_ctx* ctx, float* ms_host, int64_t* requests_host,
  *   cycles_host[0]  32 random records of a 16 KiB window          [4]  8 records, each read by 4 adjacent lanes
  *   cycles_host[1]  32 consecutive records (8 cache lines)        [5]  one record for all 32 lanes
  *   cycles_host[2]  16 random lines, adjacent lane pairs share one [6]  32 different lines, one record of each
- *   cycles_host[3]  8 random lines, each read by 4 adjacent lanes
- * The L1 model of DESIGN.md section 7 rests on this table.  HOST pointer to 7 doubles; needs no context; synchronises.
+ *   cycles_host[3]  8 random lines, each read by 4 adjacent lanes  [7]  32 random records of a 64-record window (16 lines)
+ * The L1 model of DESIGN.md section 7 rests on this table.  HOST pointer to 8 doubles; needs no context; synchronises.
  * Errors: SPH_EINVAL, SPH_ENOMEM, SPH_ECUDA. */
 int sph_debug_gather_patterns(double* cycles_host, void* stream);
 

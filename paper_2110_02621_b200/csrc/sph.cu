@@ -1408,7 +1408,7 @@ int sph_debug_gather_floor(sph_ctx* c, float* ms, int64_t* requests, void* strea
 
 int sph_debug_gather_patterns(double* cycles, void* stream) {
   if (!cycles) return SPH_EINVAL;
-  for (int k = 0; k < 7; ++k) cycles[k] = 0.0;
+  for (int k = 0; k < 8; ++k) cycles[k] = 0.0;
   cudaStream_t st = (cudaStream_t)stream;
   int dev = 0, nsm = 0, khz = 0;
   if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
@@ -1422,7 +1422,7 @@ int sph_debug_gather_patterns(double* cycles, void* stream) {
   cudaEvent_t e0, e1;
   cudaEventCreate(&e0); cudaEventCreate(&e1);
   int rc = SPH_OK;
-  for (int pat = 0; pat < 7 && rc == SPH_OK; ++pat) {
+  for (int pat = 0; pat < 8 && rc == SPH_OK; ++pat) {
     float best = 0.f;
     for (int rep = 0; rep < 4; ++rep) {   // one warm-up launch, best of three
       cudaEventRecord(e0, st);
@@ -1433,7 +1433,8 @@ int sph_debug_gather_patterns(double* cycles, void* stream) {
         case 3: k_gather_patterns<3><<<blocks, PB, 0, st>>>(R, iters, out); break;
         case 4: k_gather_patterns<4><<<blocks, PB, 0, st>>>(R, iters, out); break;
         case 5: k_gather_patterns<5><<<blocks, PB, 0, st>>>(R, iters, out); break;
-        default: k_gather_patterns<6><<<blocks, PB, 0, st>>>(R, iters, out); break;
+        case 6: k_gather_patterns<6><<<blocks, PB, 0, st>>>(R, iters, out); break;
+        default: k_gather_patterns<7><<<blocks, PB, 0, st>>>(R, iters, out); break;
       }
       cudaEventRecord(e1, st);
       if (cudaEventSynchronize(e1) != cudaSuccess) { rc = SPH_ECUDA; break; }

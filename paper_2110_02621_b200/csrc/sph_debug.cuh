@@ -438,7 +438,8 @@ k_gather_walk_affine(const int nf, const XB* __restrict__ R, const uint4* __rest
 // as a function of the address pattern, records resident in L1 (a window of 512 records = 16 KiB per block, 8 blocks
 // per SM).  PAT: 0 32 random records; 1 32 consecutive records (8 lines); 2 16 random lines, adjacent lane pairs in
 // one line; 3 8 random lines, each read by 4 adjacent lanes (4 records); 4 8 records, each read by 4 adjacent lanes;
-// 5 one record for all lanes; 6 32 different lines, one record of each.  Addresses come from an integer hash of
+// 5 one record for all lanes; 6 32 different lines, one record of each; 7 32 random records of a 64-record window (16
+// lines: lanes that share a line are not neighbours in the warp).  Addresses come from an integer hash of
 // (block, warp, iteration, lane group), a handful of ALU instructions per request.
 __device__ __forceinline__ unsigned mix32(unsigned x) {
   x ^= x >> 16; x *= 0x7feb352du; x ^= x >> 15; x *= 0x846ca68bu; x ^= x >> 16;
@@ -464,7 +465,8 @@ k_gather_patterns(const XB* __restrict__ R, const int iters, unsigned* __restric
       else if (PAT == 3) idx = ((mix32(q + (lane >> 2)) % NL) << 2) + (lane & 3u);
       else if (PAT == 4) idx = ((mix32(q + (lane >> 2)) % NL) << 2) + 1u;
       else if (PAT == 5) idx = mix32(q) % W;
-      else idx = (((mix32(q) + lane) % NL) << 2) + (mix32(q + lane) & 3u);
+      else if (PAT == 6) idx = (((mix32(q) + lane) % NL) << 2) + (mix32(q + lane) & 3u);
+      else idx = ((mix32(q) % (NL - 16)) << 2) + (mix32(q + lane) & 63u);
       r[u] = ldg256(base + idx);
     }
 #pragma unroll

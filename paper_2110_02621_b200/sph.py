@@ -322,14 +322,14 @@ def fma_peak_tflops(stream=None):
 
 
 GATHER_PATTERNS = ("random_32_records", "consecutive_32_records", "16_lines_lane_pairs", "8_lines_quads_4_records",
-                   "8_records_quads", "one_record", "32_lines")
+                   "8_records_quads", "one_record", "32_lines", "random_32_of_64_records")
 
 
 def gather_pattern_cycles(stream=None):
-    """sph_debug_gather_patterns: SM cycles per warp-wide 32-byte-record gather for seven address patterns (L1-resident)."""
+    """sph_debug_gather_patterns: SM cycles per warp-wide 32-byte-record gather for eight address patterns (L1-resident)."""
     import torch
     L = load()
-    out = (C.c_double * 7)()
+    out = (C.c_double * 8)()
     st = stream if stream is not None else torch.cuda.current_stream()
     rc = L.sph_debug_gather_patterns(out, C.c_void_p(st.cuda_stream))
     if rc != 0:
