@@ -244,6 +244,9 @@ int sph_debug_fma_peak(double* tflops_host, void* stream);
  * reading its neighbours from global memory; DESIGN.md section 5 "list walk": one coalesced 16-byte list load, four
  * 256-bit record gathers per lane) over the context's CURRENT fluid-fluid neighbour lists and records, with an empty
  * pair body, in the passes' launch configuration.  State and lists are read, never written.
+ *   body_fma    0: empty pair body (every word of the record enters one XOR / ADD); > 0: a synthetic body of that many
+ *               FFMAs per pair in four dependent chains on top of it, to see how a pass with as much arithmetic as the
+ *               real ones (66-82 instructions per pair) would follow a cheaper walk; at most 4096;
  *   ms_host[0]  every lane gathers its own list entries: exactly the memory requests of pass A / pass B;
  *   ms_host[1]  both lanes of a lane pair gather the even lane's entry (a list merged per lane pair);
  *   ms_host[2]  the four lanes of a quad gather the first lane's entry (a list merged per quad);
@@ -254,8 +257,8 @@ int sph_debug_fma_peak(double* tflops_host, void* stream);
  *   each the best of 3 launches after one warm-up launch, in ms.  Modes 1-3 run every lane to the warp's largest count.
  *   *requests_host (may be NULL) = warp-wide gather requests of one walk (sum over warps of the largest count).
  * HOST pointers (5 floats, one int64); synchronises; allocates and frees its own scratch.
- * Errors: SPH_EINVAL without particles, SPH_ENOMEM, SPH_ECUDA. */
-int sph_debug_gather_floor(sph_ctx* ctx, float* ms_host, int64_t* requests_host, void* stream);
+ * Errors: SPH_EINVAL without particles or body_fma out of range, SPH_ENOMEM, SPH_ECUDA. */
+int sph_debug_gather_floor(sph_ctx* ctx, int32_t body_fma, float* ms_host, int64_t* requests_host, void* stream);
 
 /* What a warp-wide gather of 32-byte records (one 256-bit load per lane, the pair passes' request) costs in the L1 of
  * the current device as a function of the address pattern, records resident in L1; SM cycles (at the device's maximum

@@ -1339,8 +1339,8 @@ int sph_debug_fma_peak(double* tflops_host, void* stream) {
   return SPH_OK;
 }
 
-int sph_debug_gather_floor(sph_ctx* c, float* ms, int64_t* requests, void* stream) {
-  if (!c || !ms) return SPH_EINVAL;
+int sph_debug_gather_floor(sph_ctx* c, int32_t body_fma, float* ms, int64_t* requests, void* stream) {
+  if (!c || !ms || body_fma < 0 || body_fma > 4096) return SPH_EINVAL;
   if (!c->loaded) { c->err = "no particles"; return SPH_EINVAL; }
   cudaStream_t st = (cudaStream_t)stream;
   for (int m = 0; m < 5; ++m) ms[m] = 0.f;
@@ -1382,13 +1382,22 @@ int sph_debug_gather_floor(sph_ctx* c, float* ms, int64_t* requests, void* strea
     for (int rep = 0; rep < 4; ++rep) {   // one warm-up launch, best of three
       if (mode == 4) cudaMemsetAsync(q, 0, 4 * (size_t)nq, st);
       cudaEventRecord(e0, st);
+#define GW(MODE)                                                                                                              \
+  do {                                                                                                                        \
+    if (body_fma) LAUNCH((k_gather_walk<MODE, true>), grid, PB, st, nf, c->R1, c->NL, c->NC, c->caps, (unsigned*)(d + 1), body_fma); \
+    else LAUNCH((k_gather_walk<MODE, false>), grid, PB, st, nf, c->R1, c->NL, c->NC, c->caps, (unsigned*)(d + 1), 0);       \
+  } while (0)
       switch (mode) {
-        case 0: LAUNCH(k_gather_walk<0>, grid, PB, st, nf, c->R1, c->NL, c->NC, c->caps, (unsigned*)(d + 1)); break;
-        case 1: LAUNCH(k_gather_walk<1>, grid, PB, st, nf, c->R1, c->NL, c->NC, c->caps, (unsigned*)(d + 1)); break;
-        case 2: LAUNCH(k_gather_walk<2>, grid, PB, st, nf, c->R1, c->NL, c->NC, c->caps, (unsigned*)(d + 1)); break;
-        case 3: LAUNCH(k_gather_walk<3>, grid, PB, st, nf, c->R1, c->NL, c->NC, c->caps, (unsigned*)(d + 1)); break;
-        default: LAUNCH(k_gather_walk_affine, std::min(M, nq * SPH_MINB), PB, st, nf, c->R1, c->NL, c->NC, c->caps, (unsigned*)(d + 1), vo, M, q, nq); break;
+        case 0: GW(0); break;
+        case 1: GW(1); break;
+        case 2: GW(2); break;
+        case 3: GW(3); break;
+        default:
+          if (body_fma) LAUNCH(k_gather_walk_affine<true>, std::min(M, nq * SPH_MINB), PB, st, nf, c->R1, c->NL, c->NC, c->caps, (unsigned*)(d + 1), vo, M, q, nq, body_fma);
+          else LAUNCH(k_gather_walk_affine<false>, std::min(M, nq * SPH_MINB), PB, st, nf, c->R1, c->NL, c->NC, c->caps, (unsigned*)(d + 1), vo, M, q, nq, 0);
+          break;
       }
+#undef GW
       cudaEventRecord(e1, st);
       cudaError_t e = cudaEventSynchronize(e1);
       if (e != cudaSuccess) { c->err = cudaGetErrorString(e); rc = SPH_ECUDA; break; }

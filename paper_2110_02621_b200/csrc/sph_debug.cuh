@@ -335,11 +335,13 @@ k_fma_peak(float* __restrict__ out, int iters, float a, float b) {
 //   1  the entry of the even lane of its lane pair   (what a list merged per lane pair would request),
 //   2  the entry of the first lane of its quad       (a list merged per quad: 4 adjacent lanes, one record),
 //   3  32 consecutive records from lane 0's entry on (the coalesced optimum: 8 lines, 1 KiB per request).
-template <int MODE>
+// HEAVY: a synthetic pair body of `fma` dependent-chain FFMAs per record (4 chains) on top of the XOR / ADD, to see how
+// a pass with that much arithmetic per pair follows a cheaper walk (the real bodies issue 66-82 instructions per pair).
+template <int MODE, bool HEAVY>
 struct GatherBody {
   const XB* __restrict__ R;
   unsigned last, acc;
-  int lane;
+  int lane, fma;
   __device__ __forceinline__ XB load(unsigned j) const {
     if (MODE == 1) j = __shfl_sync(FULL, j, lane & ~1);
     if (MODE == 2) j = __shfl_sync(FULL, j, lane & ~3);
@@ -349,15 +351,21 @@ struct GatherBody {
   __device__ __forceinline__ void apply(const XB& r) {
     acc += (r.x.x ^ r.x.y) + (r.x.z ^ r.x.w) + (__float_as_uint(r.b.x) ^ __float_as_uint(r.b.y)) +
            (__float_as_uint(r.b.z) ^ __float_as_uint(r.b.w));
+    if (HEAVY) {
+      float a = r.b.x, b = r.b.y, c = r.b.z, d = r.b.w;
+#pragma unroll 4
+      for (int u = 0; u < fma; u += 4) { a = fmaf(a, 1.0001f, b); b = fmaf(b, 0.9999f, c); c = fmaf(c, 1.0002f, d); d = fmaf(d, 0.9998f, a); }
+      acc += __float_as_uint((a + b) + (c + d));
+    }
   }
 };
-template <int MODE>
+template <int MODE, bool HEAVY>
 __global__ void __launch_bounds__(PB, SPH_MINB)
 k_gather_walk(const int nf, const XB* __restrict__ R, const uint4* __restrict__ NL, const int* __restrict__ NC,
-              const int caps, unsigned* __restrict__ out) {
+              const int caps, unsigned* __restrict__ out, const int fma) {
   const int i0 = blockIdx.x * PB + threadIdx.x;
   const int lane = threadIdx.x & 31;
-  GatherBody<MODE> body{R, (unsigned)(nf - 1), 0u, lane};
+  GatherBody<MODE, HEAVY> body{R, (unsigned)(nf - 1), 0u, lane, fma};
   // MODE > 0 shuffles inside the loop, so every lane runs to the warp's largest count (32 active lanes, not ~30)
   const int cnt = i0 < nf ? NC[i0] : 0;
   walk_l(NL + (size_t)(i0 >> 5) * (caps >> 2) * 32 + lane, MODE ? __reduce_max_sync(FULL, cnt) : cnt, body);
@@ -387,16 +395,17 @@ __global__ void k_chunk_keys(const DP p, const int nf, const unsigned* __restric
            (unsigned)min(cx - bx * L, 63);
   val[c] = (unsigned)c;
 }
+template <bool HEAVY>
 __global__ void __launch_bounds__(PB, SPH_MINB)
 k_gather_walk_affine(const int nf, const XB* __restrict__ R, const uint4* __restrict__ NL, const int* __restrict__ NC,
                      const int caps, unsigned* __restrict__ out, const unsigned* __restrict__ CO, const int M,
-                     unsigned* __restrict__ q, const int nq) {
+                     unsigned* __restrict__ q, const int nq, const int fma) {
   __shared__ int chunk_s;
   unsigned smid;
   asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
   const int own = (int)(smid % (unsigned)nq), per = (M + nq - 1) / nq;
   const int lane = threadIdx.x & 31;
-  GatherBody<0> body{R, (unsigned)(nf - 1), 0u, lane};
+  GatherBody<0, HEAVY> body{R, (unsigned)(nf - 1), 0u, lane, fma};
   int cur = own;
 #pragma unroll 1
   for (;;) {

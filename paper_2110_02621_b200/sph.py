@@ -87,7 +87,7 @@ def load():
     L.sph_debug_step_lists.restype = C.c_int; L.sph_debug_step_lists.argtypes = [vp, vp, vp, i64, vp, vp]
     L.sph_debug_time_pointwise.restype = C.c_int; L.sph_debug_time_pointwise.argtypes = [vp, vp, vp]
     L.sph_debug_fma_peak.restype = C.c_int; L.sph_debug_fma_peak.argtypes = [vp, vp]
-    L.sph_debug_gather_floor.restype = C.c_int; L.sph_debug_gather_floor.argtypes = [vp, vp, vp, vp]
+    L.sph_debug_gather_floor.restype = C.c_int; L.sph_debug_gather_floor.argtypes = [vp, i32, vp, vp, vp]
     L.sph_debug_gather_patterns.restype = C.c_int; L.sph_debug_gather_patterns.argtypes = [vp, vp]
     L.sph_debug_normals.restype = C.c_int; L.sph_debug_normals.argtypes = [vp, vp, vp]
     L.sph_debug_list_check.restype = C.c_int; L.sph_debug_list_check.argtypes = [vp, vp, vp]
@@ -238,12 +238,13 @@ class Sph:
         self._ck(self.L.sph_debug_time_pointwise(self.ctx, _hp(ms), self._st()))
         return dict(reinit=float(ms[0]), integrator=float(ms[1]), fused_predict=float(ms[2]))
 
-    def gather_floor(self):
+    def gather_floor(self, body_fma=0):
         """sph_debug_gather_floor: the passes' list walk with an empty pair body on the current lists (ms per launch)
-        and the number of warp-wide gather requests of one walk."""
+        and the number of warp-wide gather requests of one walk; body_fma > 0: with a synthetic pair body of that many
+        FFMAs per pair."""
         ms = np.zeros(5, np.float32)
         req = C.c_int64(0)
-        self._ck(self.L.sph_debug_gather_floor(self.ctx, _hp(ms), C.byref(req), self._st()))
+        self._ck(self.L.sph_debug_gather_floor(self.ctx, int(body_fma), _hp(ms), C.byref(req), self._st()))
         return dict(own_entries=float(ms[0]), lane_pair_shared=float(ms[1]), quad_shared=float(ms[2]),
                     coalesced=float(ms[3]), own_entries_sm_affine=float(ms[4]), requests=req.value)
 

@@ -399,6 +399,11 @@ def test_gather_floor_walks_the_lists_and_leaves_the_state_alone(name):
         s.step(3)
     gf = g.gather_floor()
     assert all(gf[k] > 0 for k in ("own_entries", "lane_pair_shared", "quad_shared", "coalesced", "own_entries_sm_affine")), gf
+    gh = g.gather_floor(body_fma=32)     # the synthetic pair body: same walks, same request count
+    assert all(gh[k] > 0 for k in ("own_entries", "lane_pair_shared", "quad_shared", "coalesced", "own_entries_sm_affine")), gh
+    assert gh["requests"] == gf["requests"]
+    with pytest.raises(sph.SphError):
+        g.gather_floor(body_fma=-1)
     # fluid rows of the lists the passes read = fluid-fluid entries (+ fluid-wall entries, which the walk does not take)
     off, ids = g.debug_step_lists()
     tag = cfg["tag"]
