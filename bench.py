@@ -334,7 +334,7 @@ def run_gpu(args):
     st = g.get_stats()
     # measured roofline of the gather form: the passes' list walk with an empty pair body, on the lists of this state
     gather = g.gather_floor()
-    gather64 = g.gather_floor(body_fma=64)   # the same walks under a synthetic pair body of 64 FFMAs per pair (about 76 instructions)
+    gather32 = g.gather_floor(body_fma=32)   # the same walks under a synthetic pair body of 32 FFMAs (about 70 instructions per pair in all)
     skin = sph.DEFAULT_LIST_SKIN if cfg.get("list_skin", -1.0) < 0 else cfg["list_skin"]
     if skin > 0:
         g.close()
@@ -419,7 +419,7 @@ def run_gpu(args):
                                  "cycles_per_request": gather["own_entries"] * 1e-3 * sm_max * 1e6 * N_SM / max(gather["requests"], 1),
                                  "pass_a_over_floor": stage_def["pass_a"] / gather["own_entries"] if gather["own_entries"] > 0 else None,
                                  "pass_b_over_floor": stage_def["pass_b"] / gather["own_entries"] if gather["own_entries"] > 0 else None,
-                                 "with_synthetic_body_of_64_fma_per_pair_ms": {k: gather64[k] for k in ("own_entries", "lane_pair_shared", "quad_shared", "coalesced", "own_entries_sm_affine")},
+                                 "with_synthetic_body_of_32_fma_per_pair_ms": {k: gather32[k] for k in ("own_entries", "lane_pair_shared", "quad_shared", "coalesced", "own_entries_sm_affine")},
                                  "l1_cycles_per_request_by_pattern": l1_patterns},
                 # list build + pass A + pass B together (the candidate walk is k_build's):
                 "pair_stages": pair_stages}
