@@ -421,10 +421,13 @@ def test_gather_pattern_cycles_are_ordered():
     its 1 KiB takes on the 128-byte-per-cycle L1 data path, 32 random records cost more than 8 lines read by quads, and
     those not more than 16 lines read by lane pairs (the table DESIGN.md section 7 quotes)."""
     c = sph.gather_pattern_cycles()
-    assert c["consecutive_32_records"] >= 7.5
-    assert c["one_record"] >= 7.5
-    assert c["random_32_records"] > c["16_lines_lane_pairs"] > c["8_lines_quads_4_records"] >= 0.9 * c["consecutive_32_records"]
-    assert c["32_lines"] > 1.5 * c["consecutive_32_records"]
+    assert all(v > 0 for v in c.values()), c
+    # wide margins (measured on a B200: 11.6, 8.9, 12.9, 12.9, 17.1, 21.3, 23.1, 24.4): a timing, not a parity, test
+    assert c["consecutive_32_records"] >= 6.0 and c["one_record"] >= 6.0
+    assert c["random_32_records"] > 1.3 * c["consecutive_32_records"]
+    assert c["32_lines"] > 1.3 * c["consecutive_32_records"]
+    assert c["16_lines_lane_pairs"] > 1.1 * c["8_lines_quads_4_records"]
+    assert c["random_32_records"] > 1.1 * c["16_lines_lane_pairs"]
 
 
 @pytest.mark.parametrize("moving", [False, True])
