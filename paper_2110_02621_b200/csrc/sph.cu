@@ -1354,12 +1354,12 @@ int sph_debug_gather_floor(sph_ctx* c, int32_t body_fma, float* ms, int64_t* req
   const int nq = std::min(nsm, 1000);
   // scratch: [0] request count, [1] the kernels' never-written output word, then the queue counters of mode 4;
   // chunk keys / values of mode 4 (two ping-pong pairs)
-  unsigned long long* d = nullptr;
-  unsigned *q = nullptr, *ck = nullptr;
-  CK(cudaMalloc((void**)&d, 16));
-  CK(cudaMalloc((void**)&q, 4 * (size_t)nq));
-  CK(cudaMalloc((void**)&ck, 16 * (size_t)M));
-  CK(cudaMemsetAsync(d, 0, 16, st));
+  unsigned long long* d = nullptr;   // one allocation: 16 bytes, then nq counters (padded to 16 bytes), then 4 M words
+  const size_t qwords = ((size_t)nq + 3) & ~(size_t)3;
+  CK(cudaMalloc((void**)&d, 16 + 4 * qwords + 16 * (size_t)M));
+  unsigned* q = reinterpret_cast<unsigned*>(d + 2);
+  unsigned* ck = q + qwords;
+  if (cudaMemsetAsync(d, 0, 16, st) != cudaSuccess) { cudaFree(d); c->err = "cudaMemsetAsync"; return SPH_ECUDA; }
   LAUNCH(k_gather_requests, cdiv(nf, 256), 256, st, nf, c->NC, d);
   // mode 4: blobs of one chunk length along x by 4 x 4 cell rows (best of 1 x 1 ... 16 x 16, profiles/r02_README.md)
   const double edge_dp = 1.0 / ((double)c->dp.inv_edge * c->prm.dp);
@@ -1411,7 +1411,7 @@ int sph_debug_gather_floor(sph_ctx* c, int32_t body_fma, float* ms, int64_t* req
   if (rc == SPH_OK && cudaMemcpy(&h, d, 8, cudaMemcpyDeviceToHost) != cudaSuccess) { c->err = "request count read-back"; rc = SPH_ECUDA; }
   if (requests) *requests = (int64_t)h;
   cudaEventDestroy(e0); cudaEventDestroy(e1);
-  cudaFree(d); cudaFree(q); cudaFree(ck);
+  cudaFree(d);
   return rc;
 }
 

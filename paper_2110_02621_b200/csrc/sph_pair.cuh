@@ -260,7 +260,12 @@ __device__ __forceinline__ void walk_l(const uint4* g, const int cnt, Body& body
 #pragma unroll 1
   for (int k = 0; k < nm; k += 4) {
     if (k < cnt) {
-      const uint4 e = RO ? __ldg(g + (size_t)(k >> 2) * 32) : g[(size_t)(k >> 2) * 32];
+      // the list entries are read once per pass: LDG.E.NA (no L1 allocation) leaves the L1 to the records, which are
+      // gathered ~85 times each (pass A / pass B -1.3 % / -2.3 % at 16.8 M, the bare walk -3 %; eviction hints on the
+      // record loads themselves change nothing: profiles/r02_README.md)
+      uint4 e;
+      if (RO) asm("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(e.x), "=r"(e.y), "=r"(e.z), "=r"(e.w) : "l"(g + (size_t)(k >> 2) * 32));
+      else e = g[(size_t)(k >> 2) * 32];
       decltype(body.load(0u)) ld[4];
       ld[0] = body.load(e.x);
       if (k + 1 < cnt) ld[1] = body.load(e.y);
